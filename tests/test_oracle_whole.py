@@ -1,0 +1,130 @@
+"""Whole-path pins for the oracle: the direct DFT (the plain definition, north_star), closed
+forms for point sources, stage consistency.  Config 1 (tiny)."""
+import numpy as np
+
+import oracle
+from paper_2601_19714_b200 import synth
+
+C0 = 299792458.0
+
+
+def _uvw_lambda(wl):
+    s = wl.freq_hz / C0
+    u = (wl.uvw_m[:, 0:1] * s[None, :]).ravel()
+    v = (wl.uvw_m[:, 1:2] * s[None, :]).ravel()
+    w = (wl.uvw_m[:, 2:3] * s[None, :]).ravel()
+    return u, v, w
+
+
+def _rel(a, b):
+    return np.linalg.norm(a - b) / np.linalg.norm(b)
+
+
+def test_against_w_snapped_and_exact_dft(cfg1, cfg1_oracle):
+    wl, r = cfg1, cfg1_oracle
+    N = wl.n
+    idx = oracle.index(wl.uvw_m, wl.freq_hz, N, wl.n_wplanes, wl.support, wl.pixel_rad, 16)
+    keep = idx["key"] != 0xFFFFFFFF
+    assert r["stats"]["n_gridded"] == int(keep.sum())
+    assert r["stats"]["n_dropped"] == int((~keep).sum()) and r["stats"]["n_dropped"] > 0
+    u, v, w = _uvw_lambda(wl)
+    dw = (idx["w_max"][0] - idx["w_min"][0]) / wl.n_wplanes
+    w_snap = idx["w_min"][0] + (idx["ip"] + 0.5) * dw
+    D = oracle.dft(u, v, w_snap, wl.vis, None, keep, N, wl.pixel_rad)
+    I = r["image"]
+    inner = slice(N // 4, 3 * N // 4)
+    e_inner = _rel(I[inner, inner], D[inner, inner])
+    mid = slice(N // 8, 7 * N // 8)
+    e_mid = _rel(I[mid, mid], D[mid, mid])
+    e_full = _rel(I, D)
+    print(f"vs w-snapped DFT: inner half {e_inner:.3e}, inner 75% {e_mid:.3e}, full {e_full:.3e}")
+    assert e_inner < 1e-5                       # kernel aliasing only (SURVEY probe: 3.9e-7)
+    assert e_mid < 1e-2 and e_full < 0.5        # unpadded edge: reported, loose
+    # exact DFT: per-pixel bound pi * dw * (1-n) * sum |w V| (w quantisation) + aliasing
+    De = oracle.dft(u, v, w, wl.vis, None, keep, N, wl.pixel_rad)
+    l = (np.arange(N) - N // 2) * wl.pixel_rad
+    one_minus_n = 1 - np.sqrt(1 - l[None, :] ** 2 - l[:, None] ** 2)
+    bound = np.pi * dw * one_minus_n * np.abs(wl.vis.ravel()[keep]).sum()
+    err = np.abs(I - De)
+    alias = np.abs(I - D)
+    assert np.all(err[inner, inner] <= bound[inner, inner] + alias[inner, inner] + 1e-9)
+    assert _rel(I[inner, inner], De[inner, inner]) < 1e-2
+
+
+def test_unit_source_at_phase_centre(cfg1):
+    wl = synth.unit_vis(cfg1)
+    r = oracle.image(wl.uvw_m, wl.freq_hz, wl.vis, None, wl.n, wl.n_wplanes, wl.support, wl.pixel_rad)
+    I, N = r["image"], wl.n
+    assert abs(I[N // 2, N // 2] / r["stats"]["sum_w"] - 1) < 1e-6      # peak = sum of weights
+    inner = slice(N // 4, 3 * N // 4)
+    pk = np.unravel_index(np.argmax(I[inner, inner]), (N // 2, N // 2))
+    assert (pk[0] + N // 4, pk[1] + N // 4) == (N // 2, N // 2)
+    # with weights: peak = sum of the weights of the gridded visibilities
+    rng = np.random.default_rng(11)
+    wgt = rng.uniform(0.5, 1.5, wl.vis.shape).astype(np.float32)
+    rw = oracle.image(wl.uvw_m, wl.freq_hz, wl.vis, wgt, wl.n, wl.n_wplanes, wl.support, wl.pixel_rad)
+    idx = oracle.index(wl.uvw_m, wl.freq_hz, N, wl.n_wplanes, wl.support, wl.pixel_rad, 16)
+    sw = wgt.ravel()[idx["key"] != 0xFFFFFFFF].astype(np.float64).sum()
+    assert abs(rw["stats"]["sum_w"] - sw) < 1e-9 * sw
+    assert abs(rw["image"][N // 2, N // 2] / sw - 1) < 1e-6
+
+
+def test_offset_source_lands_on_predicted_pixel(cfg1):
+    """A noise-free source at (a dl, b dl) peaks at [N/2+b][N/2+a] with value F/n0 * sum w."""
+    wl = cfg1
+    a, b = 20, -37
+    l0, m0 = a * wl.pixel_rad, b * wl.pixel_rad
+    n0 = np.sqrt(1 - l0 * l0 - m0 * m0)
+    u, v, w = _uvw_lambda(wl)
+    F = 0.7
+    vis = (F / n0) * np.exp(-2j * np.pi * (u * l0 + v * m0 + w * (n0 - 1))).reshape(wl.vis.shape)
+    r = oracle.image(wl.uvw_m, wl.freq_hz, vis, None, wl.n, wl.n_wplanes, wl.support, wl.pixel_rad)
+    I, N = r["image"], wl.n
+    inner = slice(N // 4, 3 * N // 4)
+    pk = np.unravel_index(np.argmax(I[inner, inner]), (N // 2, N // 2))
+    assert (pk[0] + N // 4, pk[1] + N // 4) == (N // 2 + b, N // 2 + a)
+    # w quantisation only dephases by <= pi dw (1-n0): tiny at this offset
+    assert abs(I[N // 2 + b, N // 2 + a] / (F / n0 * r["stats"]["sum_w"]) - 1) < 1e-4
+
+
+def test_stage_outputs_are_consistent(cfg1, cfg1_oracle):
+    wl, r = cfg1, cfg1_oracle
+    N, Nw = wl.n, wl.n_wplanes
+    sg, sf = r["stack_grid"], r["stack_fft"]
+    assert sg.shape == (Nw, N, N)
+    idx = oracle.index(wl.uvw_m, wl.freq_hz, N, Nw, wl.support, wl.pixel_rad, 16)
+    keep = idx["key"] != 0xFFFFFFFF
+    # per-plane Parseval and FFT == numpy on the gridded plane
+    for z in range(Nw):
+        assert abs((np.abs(sf[z]) ** 2).sum() / (N * N * (np.abs(sg[z]) ** 2).sum()) - 1) < 1e-12
+        ref = np.fft.fftshift(np.fft.ifft2(np.fft.ifftshift(sg[z]))) * (N * N)
+        assert np.abs(sf[z] - ref).max() < 1e-12 * np.abs(ref).max()
+        # plane z holds exactly the visibilities with ip == z
+        lst = np.nonzero(keep & (idx["ip"] == z))[0]
+        G = oracle.grid_plane(lst, wl.vis, None, idx["iu"], idx["iv"], idx["xu"], idx["xv"], N,
+                              wl.support, 2.34 * wl.support)
+        assert np.array_equal(G, sg[z])
+    # planes are independent: the image is the sum of per-plane corrections, then the taper
+    dw = (idx["w_max"][0] - idx["w_min"][0]) / Nw
+    raw = np.zeros((N, N))
+    for z in range(Nw):
+        oracle.wcorrect_accumulate(sf[z], wl.pixel_rad, idx["w_min"][0] + (z + 0.5) * dw, image=raw)
+    assert np.array_equal(raw, r["raw_image"])
+    c = np.array([oracle.taper((p - N // 2) / N, wl.support, 2.34 * wl.support) for p in range(N)])
+    assert np.abs(r["image"] - raw / (c[None, :] * c[:, None])).max() <= 1e-15 * np.abs(r["image"]).max()
+    assert np.array_equal(oracle.gridcorrect(raw, wl.support, 2.34 * wl.support), r["image"])
+
+
+def test_cube_mode_equals_per_channel_runs():
+    wl = synth.make_config(5, n_times=4, n=128, n_chan=3, n_wplanes=4, n_src=5)
+    r = oracle.image(wl.uvw_m, wl.freq_hz, wl.vis, None, wl.n, wl.n_wplanes, wl.support, wl.pixel_rad, cube=1)
+    assert r["image"].shape == (3, wl.n, wl.n)
+    for c in range(3):
+        rc = oracle.image(wl.uvw_m, wl.freq_hz[c:c + 1], wl.vis[:, c:c + 1], None, wl.n, wl.n_wplanes,
+                          wl.support, wl.pixel_rad, cube=0)
+        assert np.array_equal(rc["image"], r["image"][c])
+
+
+def test_empty_input_gives_zero_image():
+    r = oracle.image(np.zeros((0, 3)), np.array([C0]), np.zeros((0, 1), complex), None, 64, 4, 7, 1e-3)
+    assert np.all(r["image"] == 0) and r["stats"]["n_vis"] == 0
