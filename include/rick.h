@@ -1,0 +1,150 @@
+/*
+ * rick.h -- C ABI of librick_b200: the w-stacking imaging hot path of RICK 2.0
+ * (arxiv/paper_2601_19714) for one NVIDIA B200 (sm_100a).
+ *
+ * Path, every step a CUDA kernel:
+ *   a0  w range + per-channel scale                       (reading R4)
+ *   a1  cell / plane index + sort key                     ("closest w-plane", Eq. 5 :129)
+ *   a2  stable device radix sort by (image, plane, uv tile)  (single-GPU analogue of the
+ *                                                          paper's bucket sort, :82, :102)
+ *   a3  convolutional gridding, Kaiser-Bessel             (Eq. 3 :64, :62)
+ *   a4  2-D complex FFT of every w-plane                  (:53, :68)
+ *   a5  w-term phase screen + sum over planes             (Eq. 2 :50, :69)
+ *   a6  grid correction (division by the kernel transform)  (paper silent; reading R12)
+ *
+ * Notation: R rows (baseline x time), C channels, M = R*C visibilities (k = r*C + c),
+ * N grid edge, N_w w-planes, S kernel support (odd), h = (S-1)/2, dl pixel scale [rad],
+ * du = 1/(N dl) cell size [wavelengths].  Grid cell (j,i): row j = v, column i = u,
+ * u fastest; cell i <-> u = (i - N/2) du.  Image pixel (q,p): row q = m, column p = l,
+ * pixel p <-> l = (p - N/2) dl.
+ *
+ * Conventions
+ *   Pointers: "device" = CUDA device memory of the current device, 16-byte aligned;
+ *     "host" = ordinary host memory.  Said per argument.
+ *   Ownership: the caller owns every input and output buffer; the library borrows
+ *     them until the work it enqueued on the plan's stream has completed and never
+ *     frees them.  The plan owns keys, permutation, plane stack, image, tables and
+ *     frees them in rick_plan_destroy.
+ *   Stream: every call enqueues on the plan's stream and returns without
+ *     synchronising, except rick_get_stats, rick_image_host and rick_plan_destroy.
+ *   Errors: int return, 0 = RICK_OK, negative = error.  Nothing throws or aborts
+ *     across the ABI.  Argument errors are detected before any work is enqueued.
+ *     CUDA errors are sticky on the plan; rick_last_error gives the text.
+ *   State machine: rick_grid -> rick_fft_wplanes -> rick_wcorrect_accumulate ->
+ *     rick_gridcorrect; out of order returns RICK_ERR_STATE.  With
+ *     plane_batch < n_wplanes or cube = 1 only rick_image / rick_image_host are
+ *     valid (the staged calls need the whole stack of one image resident).
+ *   Off-grid visibilities (footprint leaves the grid) are not an error: they are
+ *     skipped and counted in n_dropped.
+ *   Threading: a plan is not thread-safe; distinct plans are independent.
+ *   There is no CPU fallback: without a CUDA device rick_plan returns RICK_ERR_CUDA.
+ */
+#ifndef RICK_B200_H
+#define RICK_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct rick_plan_s rick_plan_t; /* opaque; owns all device scratch */
+
+enum { RICK_OK = 0, RICK_ERR_INVALID = -1, RICK_ERR_STATE = -2, RICK_ERR_CUDA = -3, RICK_ERR_OOM = -4 };
+enum { RICK_GRID_F64 = 0, RICK_GRID_F32 = 1 };
+enum { RICK_VIS_C64 = 0, RICK_VIS_C128 = 1 };
+
+typedef struct {
+    int32_t n;           /* grid edge N: power of two, 64 <= N <= 32768                         */
+    int32_t n_wplanes;   /* N_w >= 1                                                            */
+    int32_t support;     /* S, odd, 3..15 (Eq. 5: full kernel width in cells)                   */
+    double  pixel_rad;   /* dl, radians per pixel, > 0                                          */
+    double  kb_beta;     /* Kaiser-Bessel beta; <= 0 -> 2.34*S (reading R5)                     */
+    int32_t grid_prec;   /* RICK_GRID_F64 (complex double mesh) | RICK_GRID_F32   */
+    int32_t tile;        /* sort-tile edge B in cells (power of two, 8..64); 0 -> 16            */
+    int32_t plane_batch; /* w-planes resident at once; 0 -> all N_w                             */
+    int32_t cube;        /* 0: all channels into one image; 1: one image per channel (R16)      */
+    int32_t reserved;    /* must be 0                                                           */
+    double  w_min, w_max; /* wavelengths; NaN -> derived from the data in rick_grid (R4)        */
+} rick_plan_desc;
+
+typedef struct {
+    int64_t n_vis;       /* M of the last rick_grid / rick_image                                */
+    int64_t n_gridded;   /* on-grid visibilities                                                */
+    int64_t n_dropped;   /* off-grid visibilities (key = 0xFFFFFFFF)                            */
+    double  sum_w;       /* sum of weights over gridded visibilities                            */
+    double  w_min, w_max; /* of image 0 (wavelengths)                                           */
+    int64_t n_launches;  /* kernels launched by this plan since creation                        */
+} rick_stats;
+
+/* Create a plan: validates `d`, allocates the plane stack
+ * (min(plane_batch, N_w) * N*N complex of grid_prec), the image (N*N double, or the
+ * caller's cube slice by slice), tables (FFT twiddles, taper, kernel coefficients)
+ * -- the tables are computed by kernels on `cuda_stream` (a cudaStream_t, may be 0).
+ * Returns RICK_ERR_INVALID (bad descriptor), RICK_ERR_CUDA (no device / CUDA
+ * failure), RICK_ERR_OOM.  *out is NULL on failure. */
+int rick_plan(rick_plan_t** out, const rick_plan_desc* d, void* cuda_stream);
+
+/* Synchronises the plan's stream and frees everything the plan owns. NULL is OK. */
+int rick_plan_destroy(rick_plan_t* p);
+
+/* a0..a3: w range, index + key, stable sort, zero the stack, grid (Eq. 3).
+ *   vis          device, [R][C] interleaved (re,im); float pairs if vis_dtype ==
+ *                RICK_VIS_C64, double pairs if RICK_VIS_C128
+ *   uvw_m        device, [R][3] double, metres
+ *   weights      device, [R][C] float, or NULL (all 1: natural weighting)
+ *   chan_freq_hz HOST, [C] double, > 0
+ *   n_chan       C >= 1;  n_rows  R >= 0 (R = 0 gives an all-zero stack)
+ * M = R*C must be < 2^32 - 1.  Scratch for keys / permutation grows as needed
+ * (RICK_ERR_OOM if it cannot).  Requires plane_batch == N_w and cube == 0. */
+int rick_grid(rick_plan_t* p, const void* vis, int32_t vis_dtype, const double* uvw_m,
+              const float* weights, const double* chan_freq_hz, int32_t n_chan, int64_t n_rows);
+
+/* a4: centred, unnormalised, + sign 2-D transform of every resident plane, in place:
+ * P_z[q][p] = sum_{j,i} G_z[j][i] exp(+2 pi i ((i-N/2)(p-N/2) + (j-N/2)(q-N/2))/N). */
+int rick_fft_wplanes(rick_plan_t* p);
+
+/* a5: I_raw[q][p] = sum_z Re(P_z[q][p] exp(+2 pi i w_z (n-1))), n = sqrt(1-l^2-m^2),
+ * w_z = w_min + (z+0.5)(w_max-w_min)/N_w; pixels with l^2+m^2 >= 1 are 0.  Into the
+ * plan's image (no taper). */
+int rick_wcorrect_accumulate(rick_plan_t* p);
+
+/* a6: I[q][p] = I_raw[q][p] / (c((p-N/2)/N) c((q-N/2)/N)), c = transform of the kernel. */
+int rick_gridcorrect(rick_plan_t* p);
+
+/* a0..a6 in one call, fused / streamed as the plan requires (plane batches, cube).
+ * Arguments as rick_grid.  image_out: device, [N][N] double, or [C][N][N] when
+ * cube = 1; may be NULL (the result stays in the plan, cube = 0 only). */
+int rick_image(rick_plan_t* p, const void* vis, int32_t vis_dtype, const double* uvw_m,
+               const float* weights, const double* chan_freq_hz, int32_t n_chan,
+               int64_t n_rows, double* image_out);
+
+/* Same as rick_image with every buffer in HOST memory (pinned memory makes the copies
+ * asynchronous): copies the inputs to plan-owned device staging, runs a0..a6, copies
+ * the image back to image_out_host and SYNCHRONISES the stream before returning. */
+int rick_image_host(rick_plan_t* p, const void* vis_host, int32_t vis_dtype, const double* uvw_m_host,
+                    const float* weights_host, const double* chan_freq_hz, int32_t n_chan,
+                    int64_t n_rows, double* image_out_host);
+
+/* Copy of the plan's image ([N][N] double) into dst_device (cube = 0 only). */
+int rick_get_image(rick_plan_t* p, double* dst_device);
+
+/* SYNCHRONISES the stream; fills *out. */
+int rick_get_stats(rick_plan_t* p, rick_stats* out);
+
+/* Text of the last error on this plan ("" if none); valid until the next call. */
+const char* rick_last_error(const rick_plan_t* p);
+
+/* Debug accessors for stage-wise parity: device pointers owned by the plan, valid
+ * until the next rick_* call on it; NULL if that stage has not run. */
+const uint32_t* rick_debug_keys(rick_plan_t* p);   /* [M] keys in visibility order          */
+const uint32_t* rick_debug_perm(rick_plan_t* p);   /* [M] stable permutation (sorted order) */
+void*           rick_debug_planes(rick_plan_t* p); /* [N_w][N][N] complex of grid_prec      */
+
+/* Library identification, e.g. "librick_b200 0.1 sm_100a". */
+const char* rick_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RICK_B200_H */

@@ -1,0 +1,130 @@
+// common.cuh -- internal declarations of librick_b200 (not part of the C ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <string.h>
+#include <string>
+#include <vector>
+
+#include "../../include/rick.h"
+
+#define RICK_C0 299792458.0
+#define RICK_MAX_CHAN 4096
+#define RICK_KEY_DROPPED 0xFFFFFFFFu
+#define RICK_MAX_KB_TERMS 96
+
+// Per-image w-plane geometry, computed on the device by k_wrange_finish (a0).
+struct WRange {
+    double w_min, w_max, dw, inv_dw;
+};
+
+// Small block of device-resident scalars (zeroed at the start of every rick_grid).
+struct DevCounters {
+    unsigned long long wmin_bits;   // ordered encoding of min over rows of w [m]
+    unsigned long long wmax_bits;   // ordered encoding of max over rows of w [m]
+    unsigned long long n_gridded;   // on-grid visibilities
+    unsigned long long n_dropped;
+    double sum_w;                   // sum of weights over gridded visibilities
+    unsigned int grid_chunk;        // dynamic work counter of the gridder
+    unsigned int pad;
+};
+
+struct rick_plan_s {
+    rick_plan_desc d;
+    int N, Nw, S, h, B, T, log2N;
+    int f32;                 // grid precision
+    int batch;               // resident planes
+    double beta, dl, inv_du;
+    cudaStream_t stream;
+    int n_sm;
+    int state;               // 0 idle, 1 gridded, 2 transformed, 3 corrected, 4 tapered
+    std::string err;
+    int64_t n_launches;
+
+    // tables
+    void* twiddle;           // [N] complex of grid_prec: e^{+2 pi i k/N}
+    double* taper;           // [N] c((p-N/2)/N)
+    double* kb_coef;         // [kb_terms] series coefficients of g in y = 1-(2t/S)^2
+    int kb_terms;
+
+    // resident buffers
+    void* stack;             // [batch][N][N] complex of grid_prec
+    size_t plane_bytes;
+    double* image;           // [N][N]
+
+    // per-call visibility scratch (grows)
+    int64_t cap_vis;
+    uint32_t *keys, *keys_a, *keys_b, *perm_a, *perm_b;
+    uint32_t* hist; size_t hist_cap;
+    uint32_t* scan_tmp; size_t scan_cap;
+    uint32_t *sorted_keys, *sorted_perm;   // point into keys_a/b, perm_a/b after the sort
+    int64_t* plane_start;    // [n_planes_total + 1] offsets into the sorted order
+    int64_t plane_start_cap;
+    double* chan_scale;      // [C] device, s_c = f_c / c0
+    WRange* wrange;          // [n_img] device
+    int chan_cap;
+    double* h_scale;         // pinned host staging of s_c (RICK_MAX_CHAN)
+    cudaEvent_t ev_scale;    // completion of the last upload from h_scale
+    std::vector<double> last_freq;
+    DevCounters* counters;   // device
+    int64_t M; int32_t C; int64_t R; int n_img;
+
+    // host-buffer staging for rick_image_host
+    void* st_vis; size_t st_vis_cap;
+    double* st_uvw; size_t st_uvw_cap;
+    float* st_wgt; size_t st_wgt_cap;
+    double* st_img; size_t st_img_cap;
+};
+
+#define RICK_CUDA(p, call)                                                             \
+    do {                                                                               \
+        cudaError_t e__ = (call);                                                      \
+        if (e__ != cudaSuccess) {                                                      \
+            (p)->err = std::string(#call) + ": " + cudaGetErrorString(e__);            \
+            return e__ == cudaErrorMemoryAllocation ? RICK_ERR_OOM : RICK_ERR_CUDA;    \
+        }                                                                              \
+    } while (0)
+
+#define RICK_LAUNCHED(p)                                                               \
+    do {                                                                               \
+        (p)->n_launches++;                                                             \
+        cudaError_t e__ = cudaGetLastError();                                          \
+        if (e__ != cudaSuccess) {                                                      \
+            (p)->err = std::string("kernel launch: ") + cudaGetErrorString(e__);       \
+            return RICK_ERR_CUDA;                                                      \
+        }                                                                              \
+    } while (0)
+
+// stage entry points (each enqueues on p->stream)
+int rick_tables_build(rick_plan_t* p);                                   // tables.cu
+int rick_index_sort(rick_plan_t* p, const double* uvw_m, const float* weights);   // index_sort.cu
+int rick_zero_planes(rick_plan_t* p, int n_planes);                      // grid.cu
+int rick_grid_planes(rick_plan_t* p, const void* vis, int vis_dtype, const double* uvw_m,
+                     const float* weights, int plane_first, int n_planes);      // grid.cu
+int rick_fft_planes(rick_plan_t* p, int n_planes);                       // fft.cu
+int rick_wcorrect(rick_plan_t* p, int img, int z_first, int n_planes, double* image,
+                  int accumulate, int fuse_taper);                     // wcorrect.cu
+int rick_taper_divide(rick_plan_t* p, double* image);                    // wcorrect.cu
+
+// ordered (monotone) encoding of doubles for atomicMin/atomicMax on u64
+__host__ __device__ inline unsigned long long rick_ord_encode(double x)
+{
+#ifdef __CUDA_ARCH__
+    unsigned long long b = (unsigned long long)__double_as_longlong(x);
+#else
+    unsigned long long b;
+    memcpy(&b, &x, sizeof(b));
+#endif
+    return (b & 0x8000000000000000ull) ? ~b : (b | 0x8000000000000000ull);
+}
+__host__ __device__ inline double rick_ord_decode(unsigned long long e)
+{
+    unsigned long long b = (e & 0x8000000000000000ull) ? (e & 0x7FFFFFFFFFFFFFFFull) : ~e;
+#ifdef __CUDA_ARCH__
+    return __longlong_as_double((long long)b);
+#else
+    double x;
+    memcpy(&x, &b, sizeof(x));
+    return x;
+#endif
+}

@@ -1,0 +1,117 @@
+// fft.cu -- a4: centred, unnormalised, + sign 2-D complex FFT of every resident w-plane, in
+// place (PAPER.md:53 "each w-plane is Fourier transformed separately", :68):
+//   P_z[q][p] = sum_{j,i} G_z[j][i] exp(+2 pi i ((i-N/2)(p-N/2) + (j-N/2)(q-N/2)) / N)
+// Two passes over the stack (the HBM floor for a plane that does not fit L2: 4 * N^2 * E
+// bytes): k_fft_rows transforms the contiguous u axis, one row per CTA held in registers
+// (16 elements per thread) with shared-memory exchanges between radix-16 stages;
+// k_fft_cols transforms the strided v axis on column strips WC columns wide.
+// Centring = index rotation by N/2 = register renaming e -> (e+8) mod 16 (fft_core.cuh).
+#include "common.cuh"
+#include "fft_core.cuh"
+
+template <typename T, int LOG2N> struct RowCfg {
+    static constexpr int N = 1 << LOG2N, NT = N / 16;
+    static constexpr int THREADS = NT >= 256 ? NT : 256;
+    static constexpr int RPC = THREADS / NT;                       // rows per CTA
+    static constexpr size_t SMEM = (size_t)RPC * (N + N / 16) * 2 * sizeof(T);
+};
+
+template <typename T, int LOG2N>
+__global__ void __launch_bounds__(RowCfg<T, LOG2N>::THREADS)
+k_fft_rows(typename cplx_of<T>::type* __restrict__ stack,
+           const typename cplx_of<T>::type* __restrict__ tw)
+{
+    typedef typename cplx_of<T>::type C;
+    typedef RowCfg<T, LOG2N> K;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int rl = threadIdx.x / K::NT, t = threadIdx.x - rl * K::NT;
+    C* sm = reinterpret_cast<C*>(smem_raw) + (size_t)rl * (K::N + K::N / 16);
+    C* g = stack + ((size_t)blockIdx.x * K::RPC + rl) * K::N;
+    C v[16];
+#pragma unroll
+    for (int e = 0; e < 16; ++e) v[e] = g[t + K::NT * ((e + 8) & 15)];
+    fft_thread<T, LOG2N>(v, t, sm, 1, 0, tw);
+#pragma unroll
+    for (int e = 0; e < 16; ++e) g[t + K::NT * ((e + 8) & 15)] = v[e];
+}
+
+template <typename T, int LOG2N> struct ColCfg {
+    static constexpr int N = 1 << LOG2N, NT = N / 16;
+    static constexpr int MAXT = sizeof(T) == 8 ? 512 : 1024;       // register budget
+    static constexpr int WANT = 32 / (2 * (int)sizeof(T));          // one 32-byte sector
+    static constexpr int W0 = NT * WANT <= MAXT ? WANT : (MAXT / NT >= 1 ? MAXT / NT : 1);
+    static constexpr int WC = NT * W0 >= 256 ? W0 : 256 / NT;       // columns per CTA
+    static constexpr int THREADS = NT * WC;
+    static constexpr size_t SMEM = (size_t)WC * (N + N / 16) * 2 * sizeof(T);
+};
+
+template <typename T, int LOG2N>
+__global__ void __launch_bounds__(ColCfg<T, LOG2N>::THREADS)
+k_fft_cols(typename cplx_of<T>::type* __restrict__ stack,
+           const typename cplx_of<T>::type* __restrict__ tw)
+{
+    typedef typename cplx_of<T>::type C;
+    typedef ColCfg<T, LOG2N> K;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    C* sm = reinterpret_cast<C*>(smem_raw);
+    constexpr int STRIPS = K::N / K::WC;
+    const int plane = blockIdx.x / STRIPS, strip = blockIdx.x - plane * STRIPS;
+    const int c = threadIdx.x % K::WC, t = threadIdx.x / K::WC;
+    C* g = stack + (size_t)plane * K::N * K::N + (size_t)strip * K::WC + c;
+    C v[16];
+#pragma unroll
+    for (int e = 0; e < 16; ++e) v[e] = g[(size_t)(t + K::NT * ((e + 8) & 15)) * K::N];
+    fft_thread<T, LOG2N>(v, t, sm, K::WC, c, tw);
+#pragma unroll
+    for (int e = 0; e < 16; ++e) g[(size_t)(t + K::NT * ((e + 8) & 15)) * K::N] = v[e];
+}
+
+template <typename T, int LOG2N>
+static int launch_fft(rick_plan_t* p, int n_planes)
+{
+    typedef typename cplx_of<T>::type C;
+    typedef RowCfg<T, LOG2N> KR;
+    typedef ColCfg<T, LOG2N> KC;
+    RICK_CUDA(p, cudaFuncSetAttribute(k_fft_rows<T, LOG2N>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      (int)KR::SMEM));
+    RICK_CUDA(p, cudaFuncSetAttribute(k_fft_cols<T, LOG2N>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      (int)KC::SMEM));
+    const unsigned int row_blocks = (unsigned int)((size_t)n_planes * KR::N / KR::RPC);
+    k_fft_rows<T, LOG2N><<<row_blocks, KR::THREADS, KR::SMEM, p->stream>>>((C*)p->stack, (const C*)p->twiddle);
+    RICK_LAUNCHED(p);
+    const unsigned int col_blocks = (unsigned int)((size_t)n_planes * (KC::N / KC::WC));
+    k_fft_cols<T, LOG2N><<<col_blocks, KC::THREADS, KC::SMEM, p->stream>>>((C*)p->stack, (const C*)p->twiddle);
+    RICK_LAUNCHED(p);
+    return RICK_OK;
+}
+
+int rick_fft_planes(rick_plan_t* p, int n_planes)
+{
+    if (n_planes <= 0) return RICK_OK;
+    if (p->f32) {
+        switch (p->log2N) {
+            case 6: return launch_fft<float, 6>(p, n_planes);
+            case 7: return launch_fft<float, 7>(p, n_planes);
+            case 8: return launch_fft<float, 8>(p, n_planes);
+            case 9: return launch_fft<float, 9>(p, n_planes);
+            case 10: return launch_fft<float, 10>(p, n_planes);
+            case 11: return launch_fft<float, 11>(p, n_planes);
+            case 12: return launch_fft<float, 12>(p, n_planes);
+            case 13: return launch_fft<float, 13>(p, n_planes);
+            case 14: return launch_fft<float, 14>(p, n_planes);
+        }
+    } else {
+        switch (p->log2N) {
+            case 6: return launch_fft<double, 6>(p, n_planes);
+            case 7: return launch_fft<double, 7>(p, n_planes);
+            case 8: return launch_fft<double, 8>(p, n_planes);
+            case 9: return launch_fft<double, 9>(p, n_planes);
+            case 10: return launch_fft<double, 10>(p, n_planes);
+            case 11: return launch_fft<double, 11>(p, n_planes);
+            case 12: return launch_fft<double, 12>(p, n_planes);
+            case 13: return launch_fft<double, 13>(p, n_planes);
+        }
+    }
+    p->err = "grid edge not supported by the FFT at this precision";
+    return RICK_ERR_INVALID;
+}

@@ -1,0 +1,401 @@
+// index_sort.cu -- a0 (w range), a1 (cell / plane index + key), a2 (stable LSD radix sort).
+//
+// a0/a1 follow SURVEY.md 8(c) steps 1-4 / DESIGN.md "Index arithmetic": every floating-point
+// operation is individually rounded (__dmul_rn / __dadd_rn / __ddiv_rn, never contracted into
+// FMA) and done in the stated order, so cell, plane and key are BIT-EXACT against the oracle.
+//   s_c = f_c / c0 (host, IEEE division);  inv_du = N * dl
+//   x_u = (u_m * s_c) * inv_du;  i_u = floor(x_u + (N/2 + 0.5))       (nearest cell, ties up; R8)
+//   on-grid <=> i_u-h >= 0, i_u+h <= N-1 (same in v)                   (Eq. 5; R10)
+//   w_l = w_m * s_c;  dw = (w_max - w_min)/N_w;  i_p = min(N_w-1, floor((w_l - w_min) * (1/dw)))
+//                                                                     ("closest w-plane", :48; R4)
+//   key = ((img*N_w + i_p)*T + i_v/B)*T + i_u/B;  dropped -> 0xFFFFFFFF
+// a2: the single-GPU analogue of the paper's bucket sort: a stable
+// least-significant-digit radix sort of (key, visibility index) pairs, which equals the
+// oracle's sort by (key, index).
+#include "common.cuh"
+
+// ------------------------------------------------------------------------------------------
+// a0: w range.  min/max over rows of w [m]; multiplication by s_c > 0 is monotone under
+// round-to-nearest, so min_{r} fl(w_r s_c) = fl((min_r w_r) s_c) exactly.
+// ------------------------------------------------------------------------------------------
+__global__ void k_counters_reset(DevCounters* c)
+{
+    c->wmin_bits = 0xFFFFFFFFFFFFFFFFull;
+    c->wmax_bits = 0ull;
+    c->n_gridded = 0ull;
+    c->n_dropped = 0ull;
+    c->sum_w = 0.0;
+    c->grid_chunk = 0u;
+    c->pad = 0u;
+}
+
+__global__ void k_wrange_rows(const double* __restrict__ uvw, long long R, DevCounters* c)
+{
+    unsigned long long lo = 0xFFFFFFFFFFFFFFFFull, hi = 0ull;
+    for (long long r = blockIdx.x * (long long)blockDim.x + threadIdx.x; r < R;
+         r += (long long)gridDim.x * blockDim.x) {
+        unsigned long long e = rick_ord_encode(uvw[3 * r + 2]);
+        lo = e < lo ? e : lo;
+        hi = e > hi ? e : hi;
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+        unsigned long long l2 = __shfl_xor_sync(0xffffffffu, lo, o);
+        unsigned long long h2 = __shfl_xor_sync(0xffffffffu, hi, o);
+        lo = l2 < lo ? l2 : lo;
+        hi = h2 > hi ? h2 : hi;
+    }
+    if ((threadIdx.x & 31) == 0) {
+        atomicMin(&c->wmin_bits, lo);
+        atomicMax(&c->wmax_bits, hi);
+    }
+}
+
+__global__ void k_wrange_finish(const DevCounters* c, const double* __restrict__ chan_scale, int C,
+                                int cube, int Nw, double w_min_given, double w_max_given,
+                                long long R, WRange* __restrict__ out)
+{
+    const int g = blockIdx.x * blockDim.x + threadIdx.x;
+    const int n_img = cube ? C : 1;
+    if (g >= n_img) return;
+    double lo, hi;
+    if (R == 0) {
+        lo = 0.0;
+        hi = 0.0;
+    } else {
+        const double wlo_m = rick_ord_decode(c->wmin_bits), whi_m = rick_ord_decode(c->wmax_bits);
+        if (cube) {
+            const double s = chan_scale[g];
+            lo = __dmul_rn(wlo_m, s);
+            hi = __dmul_rn(whi_m, s);
+        } else {
+            lo = INFINITY;
+            hi = -INFINITY;
+            for (int ch = 0; ch < C; ++ch) {
+                const double s = chan_scale[ch];
+                lo = fmin(lo, __dmul_rn(wlo_m, s));
+                hi = fmax(hi, __dmul_rn(whi_m, s));
+            }
+        }
+    }
+    if (w_min_given == w_min_given) lo = w_min_given;
+    if (w_max_given == w_max_given) hi = w_max_given;
+    WRange w;
+    w.w_min = lo;
+    w.w_max = hi;
+    w.dw = __ddiv_rn(__dsub_rn(hi, lo), (double)Nw);
+    w.inv_dw = w.dw > 0.0 ? __ddiv_rn(1.0, w.dw) : 0.0;
+    out[g] = w;
+}
+
+// ------------------------------------------------------------------------------------------
+// a1: one thread per visibility k = r*C + c.
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+k_index_key(const double* __restrict__ uvw, const float* __restrict__ wgt,
+            const double* __restrict__ chan_scale, const WRange* __restrict__ wrange,
+            unsigned int M, unsigned int C, int N, int Nw, int h, int B, int T, int cube,
+            double inv_du, uint32_t* __restrict__ keys, DevCounters* cnt)
+{
+    const unsigned int k = blockIdx.x * blockDim.x + threadIdx.x;
+    unsigned int on = 0, off = 0;
+    double sw = 0.0;
+    if (k < M) {
+        const unsigned int r = k / C, c = k - r * C;
+        const double s = chan_scale[c];
+        const double um = uvw[3ull * r + 0], vm = uvw[3ull * r + 1], wm = uvw[3ull * r + 2];
+        const double shift = (double)(N / 2) + 0.5;
+        const double xu = __dmul_rn(__dmul_rn(um, s), inv_du);
+        const double xv = __dmul_rn(__dmul_rn(vm, s), inv_du);
+        const int iu = (int)floor(__dadd_rn(xu, shift));
+        const int iv = (int)floor(__dadd_rn(xv, shift));
+        const int img = cube ? (int)c : 0;
+        const WRange wr = wrange[img];
+        int ip = (int)floor(__dmul_rn(__dsub_rn(__dmul_rn(wm, s), wr.w_min), wr.inv_dw));
+        ip = ip > Nw - 1 ? Nw - 1 : ip;
+        ip = ip < 0 ? 0 : ip;
+        const bool ok = (iu - h >= 0) && (iu + h <= N - 1) && (iv - h >= 0) && (iv + h <= N - 1);
+        uint32_t key = RICK_KEY_DROPPED;
+        if (ok) {
+            unsigned long long kk = (unsigned long long)img * (unsigned)Nw + (unsigned)ip;
+            kk = (kk * (unsigned)T + (unsigned)(iv / B)) * (unsigned)T + (unsigned)(iu / B);
+            key = (uint32_t)kk;
+            on = 1;
+            sw = wgt ? (double)wgt[k] : 1.0;
+        } else {
+            off = 1;
+        }
+        keys[k] = key;
+    }
+    // warp-reduced statistics
+    const unsigned int b_on = __ballot_sync(0xffffffffu, on), b_off = __ballot_sync(0xffffffffu, off);
+    for (int o = 16; o > 0; o >>= 1) sw += __shfl_xor_sync(0xffffffffu, sw, o);
+    if ((threadIdx.x & 31) == 0) {
+        if (b_on) {
+            atomicAdd(&cnt->n_gridded, (unsigned long long)__popc(b_on));
+            atomicAdd(&cnt->sum_w, sw);
+        }
+        if (b_off) atomicAdd(&cnt->n_dropped, (unsigned long long)__popc(b_off));
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// a2: LSD radix sort, <= 8-bit digits, stable.
+// ------------------------------------------------------------------------------------------
+#define RS_THREADS 256
+#define RS_ITEMS 16
+#define RS_TILE (RS_THREADS * RS_ITEMS)
+
+__global__ void __launch_bounds__(RS_THREADS)
+k_radix_hist(const uint32_t* __restrict__ keys, unsigned int M, int shift, uint32_t mask, int nbins,
+             uint32_t* __restrict__ hist, unsigned int nblocks)
+{
+    __shared__ uint32_t hs[256];
+    hs[threadIdx.x] = 0;
+    __syncthreads();
+    const unsigned long long base = (unsigned long long)blockIdx.x * RS_TILE;
+#pragma unroll
+    for (int i = 0; i < RS_ITEMS; ++i) {
+        const unsigned long long idx = base + (unsigned)i * RS_THREADS + threadIdx.x;
+        const bool valid = idx < M;
+        const uint32_t d = valid ? ((keys[idx] >> shift) & mask) : 0xFFFFu;
+        const unsigned int m = __match_any_sync(0xffffffffu, d);
+        if (valid && (int)(threadIdx.x & 31) == __ffs(m) - 1) atomicAdd(&hs[d], (uint32_t)__popc(m));
+    }
+    __syncthreads();
+    if ((int)threadIdx.x < nbins) hist[(size_t)threadIdx.x * nblocks + blockIdx.x] = hs[threadIdx.x];
+}
+
+__global__ void __launch_bounds__(RS_THREADS)
+k_radix_scatter(const uint32_t* __restrict__ kin, const uint32_t* __restrict__ vin,
+                uint32_t* __restrict__ kout, uint32_t* __restrict__ vout, unsigned int M, int shift,
+                uint32_t mask, int nbins, const uint32_t* __restrict__ hist_scanned,
+                unsigned int nblocks)
+{
+    __shared__ uint32_t cnt[RS_THREADS / 32][256];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    for (int i = threadIdx.x; i < (RS_THREADS / 32) * 256; i += RS_THREADS) (&cnt[0][0])[i] = 0;
+    __syncthreads();
+    const unsigned long long base =
+        (unsigned long long)blockIdx.x * RS_TILE + (unsigned)warp * (32 * RS_ITEMS);
+    uint32_t key[RS_ITEMS];
+    uint32_t rank[RS_ITEMS];
+#pragma unroll
+    for (int i = 0; i < RS_ITEMS; ++i) {
+        const unsigned long long idx = base + (unsigned)i * 32 + lane;
+        const bool valid = idx < M;
+        key[i] = valid ? kin[idx] : 0xFFFFFFFFu;
+        const uint32_t d = (key[i] >> shift) & mask;
+        const unsigned int m = __match_any_sync(0xffffffffu, valid ? d : 0xFFFFu);
+        const int leader = __ffs(m) - 1;
+        uint32_t old = 0;
+        if (valid && lane == leader) {
+            old = cnt[warp][d];
+            cnt[warp][d] = old + (uint32_t)__popc(m);
+        }
+        old = __shfl_sync(0xffffffffu, old, leader);
+        rank[i] = old + (uint32_t)__popc(m & ((1u << lane) - 1u));
+        __syncwarp();
+    }
+    __syncthreads();
+    if ((int)threadIdx.x < nbins) {
+        uint32_t run = hist_scanned[(size_t)threadIdx.x * nblocks + blockIdx.x];
+#pragma unroll
+        for (int w = 0; w < RS_THREADS / 32; ++w) {
+            const uint32_t t = cnt[w][threadIdx.x];
+            cnt[w][threadIdx.x] = run;
+            run += t;
+        }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int i = 0; i < RS_ITEMS; ++i) {
+        const unsigned long long idx = base + (unsigned)i * 32 + lane;
+        if (idx < M) {
+            const uint32_t d = (key[i] >> shift) & mask;
+            const uint32_t pos = cnt[warp][d] + rank[i];
+            kout[pos] = key[i];
+            vout[pos] = vin ? vin[idx] : (uint32_t)idx;
+        }
+    }
+}
+
+// exclusive scan of a u32 array: (1) per-block sums, (2) scan of the sums, (3) apply
+#define SC_THREADS 1024
+#define SC_ITEMS 4
+#define SC_TILE (SC_THREADS * SC_ITEMS)
+
+__device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t* total)
+{
+    __shared__ uint32_t ws[32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    uint32_t x = v;
+    for (int o = 1; o < 32; o <<= 1) {
+        uint32_t y = __shfl_up_sync(0xffffffffu, x, o);
+        if (lane >= o) x += y;
+    }
+    if (lane == 31) ws[warp] = x;
+    __syncthreads();
+    if (warp == 0) {
+        uint32_t s = ws[lane];
+        for (int o = 1; o < 32; o <<= 1) {
+            uint32_t y = __shfl_up_sync(0xffffffffu, s, o);
+            if (lane >= o) s += y;
+        }
+        ws[lane] = s;
+    }
+    __syncthreads();
+    const uint32_t warp_off = warp ? ws[warp - 1] : 0;
+    *total = ws[31];
+    const uint32_t r = warp_off + x - v;
+    __syncthreads();
+    return r;
+}
+
+__global__ void __launch_bounds__(SC_THREADS)
+k_scan_reduce(const uint32_t* __restrict__ a, size_t n, uint32_t* __restrict__ sums)
+{
+    const size_t base = (size_t)blockIdx.x * SC_TILE + (size_t)threadIdx.x * SC_ITEMS;
+    uint32_t s = 0;
+#pragma unroll
+    for (int i = 0; i < SC_ITEMS; ++i)
+        if (base + i < n) s += a[base + i];
+    uint32_t tot;
+    block_exclusive_scan(s, &tot);
+    if (threadIdx.x == 0) sums[blockIdx.x] = tot;
+}
+
+__global__ void __launch_bounds__(SC_THREADS) k_scan_top(uint32_t* __restrict__ sums, unsigned int nb)
+{
+    uint32_t carry = 0;
+    for (unsigned int b0 = 0; b0 < nb; b0 += SC_THREADS) {
+        const unsigned int i = b0 + threadIdx.x;
+        const uint32_t v = i < nb ? sums[i] : 0;
+        uint32_t tot;
+        const uint32_t e = block_exclusive_scan(v, &tot);
+        if (i < nb) sums[i] = carry + e;
+        carry += tot;
+    }
+}
+
+__global__ void __launch_bounds__(SC_THREADS)
+k_scan_apply(uint32_t* __restrict__ a, size_t n, const uint32_t* __restrict__ sums)
+{
+    const size_t base = (size_t)blockIdx.x * SC_TILE + (size_t)threadIdx.x * SC_ITEMS;
+    uint32_t v[SC_ITEMS], s = 0;
+#pragma unroll
+    for (int i = 0; i < SC_ITEMS; ++i) {
+        v[i] = base + i < n ? a[base + i] : 0;
+        s += v[i];
+    }
+    uint32_t tot;
+    uint32_t e = block_exclusive_scan(s, &tot) + sums[blockIdx.x];
+#pragma unroll
+    for (int i = 0; i < SC_ITEMS; ++i) {
+        if (base + i < n) a[base + i] = e;
+        e += v[i];
+    }
+}
+
+// plane_start[z] = first sorted position whose key >= z*T*T  (z = 0..n_planes_total)
+__global__ void k_plane_starts(const uint32_t* __restrict__ skeys, unsigned int M, unsigned long long TT,
+                               int n_planes_total, long long* __restrict__ plane_start)
+{
+    const int z = blockIdx.x * blockDim.x + threadIdx.x;
+    if (z > n_planes_total) return;
+    const unsigned long long target = (unsigned long long)z * TT;
+    unsigned int lo = 0, hi = M;
+    while (lo < hi) {
+        const unsigned int mid = lo + (hi - lo) / 2;
+        if ((unsigned long long)skeys[mid] < target) lo = mid + 1; else hi = mid;
+    }
+    plane_start[z] = (long long)lo;
+}
+
+// ------------------------------------------------------------------------------------------
+static int ensure_u32(rick_plan_t* p, uint32_t** buf, size_t* cap, size_t need)
+{
+    if (*cap >= need) return RICK_OK;
+    if (*buf) cudaFree(*buf);
+    *buf = nullptr;
+    *cap = 0;
+    RICK_CUDA(p, cudaMalloc(buf, sizeof(uint32_t) * need));
+    *cap = need;
+    return RICK_OK;
+}
+
+int rick_index_sort(rick_plan_t* p, const double* uvw_m, const float* weights)
+{
+    cudaStream_t st = p->stream;
+    const unsigned int M = (unsigned int)p->M;
+    const int n_planes_total = p->n_img * p->Nw;
+
+    k_counters_reset<<<1, 1, 0, st>>>(p->counters);
+    RICK_LAUNCHED(p);
+    if (p->R > 0) {
+        int nb = (int)((p->R + 255) / 256);
+        if (nb > p->n_sm * 8) nb = p->n_sm * 8;
+        k_wrange_rows<<<nb, 256, 0, st>>>(uvw_m, (long long)p->R, p->counters);
+        RICK_LAUNCHED(p);
+    }
+    k_wrange_finish<<<(p->n_img + 127) / 128, 128, 0, st>>>(p->counters, p->chan_scale, p->C, p->d.cube,
+                                                          p->Nw, p->d.w_min, p->d.w_max,
+                                                          (long long)p->R, p->wrange);
+    RICK_LAUNCHED(p);
+
+    p->sorted_keys = p->keys;
+    p->sorted_perm = p->perm_a;
+    if (M > 0) {
+        k_index_key<<<(M + 255) / 256, 256, 0, st>>>(uvw_m, weights, p->chan_scale, p->wrange, M,
+                                                    (unsigned)p->C, p->N, p->Nw, p->h, p->B, p->T,
+                                                    p->d.cube, p->inv_du, p->keys, p->counters);
+        RICK_LAUNCHED(p);
+
+        // key bits: the all-ones pattern of the sorted bit range is reserved for the sentinel
+        const unsigned long long nkeys = (unsigned long long)n_planes_total * p->T * p->T;
+        int bits = 1;
+        while (((1ull << bits) - 1ull) < nkeys) ++bits;
+        const int npass = (bits + 7) / 8;
+        const unsigned int nblocks = (M + RS_TILE - 1) / RS_TILE;
+        int rc = ensure_u32(p, &p->hist, &p->hist_cap, (size_t)256 * nblocks);
+        if (rc) return rc;
+        const size_t n_hist_max = (size_t)256 * nblocks;
+        const unsigned int nsb_max = (unsigned int)((n_hist_max + SC_TILE - 1) / SC_TILE);
+        rc = ensure_u32(p, &p->scan_tmp, &p->scan_cap, nsb_max);
+        if (rc) return rc;
+
+        const uint32_t* kin = p->keys;
+        const uint32_t* vin = nullptr;
+        uint32_t* kbuf[2] = {p->keys_a, p->keys_b};
+        uint32_t* vbuf[2] = {p->perm_a, p->perm_b};
+        int shift = 0;
+        for (int pass = 0; pass < npass; ++pass) {
+            const int nb_bits = (bits - shift + (npass - pass) - 1) / (npass - pass);
+            const int nbins = 1 << nb_bits;
+            const uint32_t mask = (uint32_t)(nbins - 1);
+            k_radix_hist<<<nblocks, RS_THREADS, 0, st>>>(kin, M, shift, mask, nbins, p->hist, nblocks);
+            RICK_LAUNCHED(p);
+            const size_t n_hist = (size_t)nbins * nblocks;
+            const unsigned int nsb = (unsigned int)((n_hist + SC_TILE - 1) / SC_TILE);
+            k_scan_reduce<<<nsb, SC_THREADS, 0, st>>>(p->hist, n_hist, p->scan_tmp);
+            RICK_LAUNCHED(p);
+            k_scan_top<<<1, SC_THREADS, 0, st>>>(p->scan_tmp, nsb);
+            RICK_LAUNCHED(p);
+            k_scan_apply<<<nsb, SC_THREADS, 0, st>>>(p->hist, n_hist, p->scan_tmp);
+            RICK_LAUNCHED(p);
+            uint32_t* ko = kbuf[pass & 1];
+            uint32_t* vo = vbuf[pass & 1];
+            k_radix_scatter<<<nblocks, RS_THREADS, 0, st>>>(kin, vin, ko, vo, M, shift, mask, nbins,
+                                                          p->hist, nblocks);
+            RICK_LAUNCHED(p);
+            kin = ko;
+            vin = vo;
+            shift += nb_bits;
+        }
+        p->sorted_keys = (uint32_t*)kin;
+        p->sorted_perm = (uint32_t*)vin;
+    }
+    k_plane_starts<<<(n_planes_total + 1 + 127) / 128, 128, 0, st>>>(
+        p->sorted_keys, M, (unsigned long long)p->T * p->T, n_planes_total, (long long*)p->plane_start);
+    RICK_LAUNCHED(p);
+    return RICK_OK;
+}

@@ -1,0 +1,331 @@
+// plan.cu -- the C ABI of librick_b200 (include/rick.h): plan lifetime, argument checks,
+// the state machine and the host-side sequencing of a0..a6.  All arithmetic of the path runs
+// in the kernels of index_sort.cu / grid.cu / fft.cu / wcorrect.cu.
+#include "common.cuh"
+
+#include <math.h>
+#include <new>
+#include <vector>
+
+static bool is_pow2(int x) { return x > 0 && (x & (x - 1)) == 0; }
+
+static void free_dev(void* q)
+{
+    if (q) cudaFree(q);
+}
+
+extern "C" const char* rick_version(void) { return "librick_b200 0.1 sm_100a"; }
+
+extern "C" const char* rick_last_error(const rick_plan_t* p) { return p ? p->err.c_str() : "null plan"; }
+
+extern "C" int rick_plan_destroy(rick_plan_t* p)
+{
+    if (!p) return RICK_OK;
+    cudaStreamSynchronize(p->stream);
+    free_dev(p->twiddle); free_dev(p->taper); free_dev(p->kb_coef); free_dev(p->stack); free_dev(p->image);
+    free_dev(p->keys); free_dev(p->keys_a); free_dev(p->keys_b); free_dev(p->perm_a); free_dev(p->perm_b);
+    free_dev(p->hist); free_dev(p->scan_tmp); free_dev(p->plane_start); free_dev(p->chan_scale);
+    free_dev(p->wrange); free_dev(p->counters);
+    free_dev(p->st_vis); free_dev(p->st_uvw); free_dev(p->st_wgt); free_dev(p->st_img);
+    if (p->h_scale) cudaFreeHost(p->h_scale);
+    if (p->ev_scale) cudaEventDestroy(p->ev_scale);
+    delete p;
+    return RICK_OK;
+}
+
+static int plan_init(rick_plan_t* p)
+{
+    int dev = 0;
+    RICK_CUDA(p, cudaGetDevice(&dev));
+    RICK_CUDA(p, cudaDeviceGetAttribute(&p->n_sm, cudaDevAttrMultiProcessorCount, dev));
+    const size_t cell = p->f32 ? 8 : 16;
+    p->plane_bytes = (size_t)p->N * p->N * cell;
+    RICK_CUDA(p, cudaMalloc(&p->stack, p->plane_bytes * (size_t)p->batch));
+    RICK_CUDA(p, cudaMalloc(&p->image, sizeof(double) * (size_t)p->N * p->N));
+    RICK_CUDA(p, cudaMallocHost(&p->h_scale, sizeof(double) * RICK_MAX_CHAN));
+    RICK_CUDA(p, cudaEventCreateWithFlags(&p->ev_scale, cudaEventDisableTiming));
+    RICK_CUDA(p, cudaMalloc(&p->counters, sizeof(DevCounters)));
+    RICK_CUDA(p, cudaMemsetAsync(p->counters, 0, sizeof(DevCounters), p->stream));
+    return rick_tables_build(p);
+}
+
+extern "C" int rick_plan(rick_plan_t** out, const rick_plan_desc* d, void* cuda_stream)
+{
+    if (!out) return RICK_ERR_INVALID;
+    *out = nullptr;
+    if (!d) return RICK_ERR_INVALID;
+    if (!is_pow2(d->n) || d->n < 64 || d->n > 16384) return RICK_ERR_INVALID;
+    if (d->n_wplanes < 1 || d->n_wplanes > 65536) return RICK_ERR_INVALID;
+    if (d->support < 3 || d->support > 15 || (d->support & 1) == 0) return RICK_ERR_INVALID;
+    if (!(d->pixel_rad > 0.0) || !isfinite(d->pixel_rad)) return RICK_ERR_INVALID;
+    if (d->grid_prec != RICK_GRID_F64 && d->grid_prec != RICK_GRID_F32) return RICK_ERR_INVALID;
+    if (d->grid_prec == RICK_GRID_F64 && d->n > 8192) return RICK_ERR_INVALID;
+    const int B = d->tile ? d->tile : 16;
+    if (!is_pow2(B) || B < 8 || B > 32 || B > d->n) return RICK_ERR_INVALID;
+    if (d->plane_batch < 0 || d->plane_batch > d->n_wplanes) return RICK_ERR_INVALID;
+    if (d->cube != 0 && d->cube != 1) return RICK_ERR_INVALID;
+    if (d->reserved != 0) return RICK_ERR_INVALID;
+    if (isinf(d->w_min) || isinf(d->w_max)) return RICK_ERR_INVALID;
+    if (d->w_min == d->w_min && d->w_max == d->w_max && d->w_max < d->w_min) return RICK_ERR_INVALID;
+    if (d->kb_beta == d->kb_beta && d->kb_beta > 60.0) return RICK_ERR_INVALID;
+
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return RICK_ERR_CUDA;   // no CPU fallback
+
+    rick_plan_t* p = new (std::nothrow) rick_plan_s();
+    if (!p) return RICK_ERR_OOM;
+    p->d = *d;
+    p->N = d->n;
+    p->Nw = d->n_wplanes;
+    p->S = d->support;
+    p->h = (d->support - 1) / 2;
+    p->B = B;
+    p->T = d->n / B;
+    p->log2N = 0;
+    while ((1 << p->log2N) < d->n) p->log2N++;
+    p->f32 = d->grid_prec == RICK_GRID_F32;
+    p->batch = d->plane_batch ? d->plane_batch : d->n_wplanes;
+    p->beta = d->kb_beta > 0.0 ? d->kb_beta : 2.34 * (double)d->support;
+    p->dl = d->pixel_rad;
+    p->inv_du = (double)d->n * d->pixel_rad;
+    p->stream = (cudaStream_t)cuda_stream;
+    const int rc = plan_init(p);
+    if (rc != RICK_OK) {
+        rick_plan_destroy(p);
+        return rc;
+    }
+    *out = p;
+    return RICK_OK;
+}
+
+// ---------------------------------------------------------------------------------------
+static int check_inputs(rick_plan_t* p, const void* vis, int32_t vis_dtype, const double* uvw_m,
+                        const double* chan_freq_hz, int32_t n_chan, int64_t n_rows)
+{
+    if (vis_dtype != RICK_VIS_C64 && vis_dtype != RICK_VIS_C128) { p->err = "bad vis_dtype"; return RICK_ERR_INVALID; }
+    if (n_chan < 1 || n_chan > RICK_MAX_CHAN || !chan_freq_hz) { p->err = "bad channels"; return RICK_ERR_INVALID; }
+    if (n_rows < 0) { p->err = "negative n_rows"; return RICK_ERR_INVALID; }
+    if (n_rows > 0 && (!vis || !uvw_m)) { p->err = "null input"; return RICK_ERR_INVALID; }
+    for (int c = 0; c < n_chan; ++c)
+        if (!(chan_freq_hz[c] > 0.0) || !isfinite(chan_freq_hz[c])) { p->err = "bad frequency"; return RICK_ERR_INVALID; }
+    const unsigned long long M = (unsigned long long)n_rows * (unsigned long long)n_chan;
+    if (M >= 0xFFFFFFFFull) { p->err = "too many visibilities for 32-bit indices"; return RICK_ERR_INVALID; }
+    const unsigned long long n_img = p->d.cube ? (unsigned long long)n_chan : 1ull;
+    const unsigned long long nkeys = n_img * (unsigned long long)p->Nw * (unsigned long long)p->T * p->T;
+    if (nkeys >= 0xFFFFFFFFull) { p->err = "key space exceeds 32 bits (use a larger tile)"; return RICK_ERR_INVALID; }
+    return RICK_OK;
+}
+
+template <typename Tp> static int grow(rick_plan_t* p, Tp** buf, size_t n)
+{
+    free_dev(*buf);
+    *buf = nullptr;
+    RICK_CUDA(p, cudaMalloc(buf, sizeof(Tp) * (n ? n : 1)));
+    return RICK_OK;
+}
+
+static int prepare(rick_plan_t* p, const double* chan_freq_hz, int32_t n_chan, int64_t n_rows)
+{
+    p->C = n_chan;
+    p->R = n_rows;
+    p->M = n_rows * (int64_t)n_chan;
+    p->n_img = p->d.cube ? n_chan : 1;
+    int rc;
+    if (p->M > p->cap_vis) {
+        p->cap_vis = 0;
+        if ((rc = grow(p, &p->keys, (size_t)p->M))) return rc;
+        if ((rc = grow(p, &p->keys_a, (size_t)p->M))) return rc;
+        if ((rc = grow(p, &p->keys_b, (size_t)p->M))) return rc;
+        if ((rc = grow(p, &p->perm_a, (size_t)p->M))) return rc;
+        if ((rc = grow(p, &p->perm_b, (size_t)p->M))) return rc;
+        p->cap_vis = p->M;
+    }
+    if (!p->keys) {   // M == 0 on a fresh plan: keep the pointers valid
+        if ((rc = grow(p, &p->keys, 1))) return rc;
+        if ((rc = grow(p, &p->keys_a, 1))) return rc;
+        if ((rc = grow(p, &p->keys_b, 1))) return rc;
+        if ((rc = grow(p, &p->perm_a, 1))) return rc;
+        if ((rc = grow(p, &p->perm_b, 1))) return rc;
+    }
+    const int64_t n_pl = (int64_t)p->n_img * p->Nw + 1;
+    if (n_pl > p->plane_start_cap) {
+        if ((rc = grow(p, &p->plane_start, (size_t)n_pl))) return rc;
+        p->plane_start_cap = n_pl;
+    }
+    if (n_chan > p->chan_cap) {
+        if ((rc = grow(p, &p->chan_scale, (size_t)n_chan))) return rc;
+        if ((rc = grow(p, &p->wrange, (size_t)n_chan))) return rc;
+        p->chan_cap = n_chan;
+    }
+    const bool same = (int)p->last_freq.size() == n_chan &&
+                      memcmp(p->last_freq.data(), chan_freq_hz, sizeof(double) * (size_t)n_chan) == 0;
+    if (!same) {
+        // pinned staging; wait for the previous upload before overwriting it (normally done long ago)
+        RICK_CUDA(p, cudaEventSynchronize(p->ev_scale));
+        for (int c = 0; c < n_chan; ++c) p->h_scale[c] = chan_freq_hz[c] / RICK_C0;   // s_c = f_c / c0
+        RICK_CUDA(p, cudaMemcpyAsync(p->chan_scale, p->h_scale, sizeof(double) * (size_t)n_chan,
+                                     cudaMemcpyHostToDevice, p->stream));
+        RICK_CUDA(p, cudaEventRecord(p->ev_scale, p->stream));
+        p->last_freq.assign(chan_freq_hz, chan_freq_hz + n_chan);
+    }
+    return RICK_OK;
+}
+
+extern "C" int rick_grid(rick_plan_t* p, const void* vis, int32_t vis_dtype, const double* uvw_m,
+                         const float* weights, const double* chan_freq_hz, int32_t n_chan, int64_t n_rows)
+{
+    if (!p) return RICK_ERR_INVALID;
+    p->err.clear();
+    if (p->batch != p->Nw || p->d.cube) { p->err = "staged calls need the whole stack resident and cube = 0"; return RICK_ERR_STATE; }
+    int rc = check_inputs(p, vis, vis_dtype, uvw_m, chan_freq_hz, n_chan, n_rows);
+    if (rc) return rc;
+    p->state = 0;
+    if ((rc = prepare(p, chan_freq_hz, n_chan, n_rows))) return rc;
+    if ((rc = rick_index_sort(p, uvw_m, weights))) return rc;
+    if ((rc = rick_zero_planes(p, p->Nw))) return rc;
+    if ((rc = rick_grid_planes(p, vis, vis_dtype, uvw_m, weights, 0, p->Nw))) return rc;
+    p->state = 1;
+    return RICK_OK;
+}
+
+extern "C" int rick_fft_wplanes(rick_plan_t* p)
+{
+    if (!p) return RICK_ERR_INVALID;
+    p->err.clear();
+    if (p->state != 1) { p->err = "rick_fft_wplanes needs a gridded stack"; return RICK_ERR_STATE; }
+    const int rc = rick_fft_planes(p, p->Nw);
+    if (rc) return rc;
+    p->state = 2;
+    return RICK_OK;
+}
+
+extern "C" int rick_wcorrect_accumulate(rick_plan_t* p)
+{
+    if (!p) return RICK_ERR_INVALID;
+    p->err.clear();
+    if (p->state != 2) { p->err = "rick_wcorrect_accumulate needs a transformed stack"; return RICK_ERR_STATE; }
+    const int rc = rick_wcorrect(p, 0, 0, p->Nw, p->image, 0, 0);
+    if (rc) return rc;
+    p->state = 3;
+    return RICK_OK;
+}
+
+extern "C" int rick_gridcorrect(rick_plan_t* p)
+{
+    if (!p) return RICK_ERR_INVALID;
+    p->err.clear();
+    if (p->state != 3) { p->err = "rick_gridcorrect needs a w-corrected image"; return RICK_ERR_STATE; }
+    const int rc = rick_taper_divide(p, p->image);
+    if (rc) return rc;
+    p->state = 4;
+    return RICK_OK;
+}
+
+extern "C" int rick_image(rick_plan_t* p, const void* vis, int32_t vis_dtype, const double* uvw_m,
+                          const float* weights, const double* chan_freq_hz, int32_t n_chan,
+                          int64_t n_rows, double* image_out)
+{
+    if (!p) return RICK_ERR_INVALID;
+    p->err.clear();
+    int rc = check_inputs(p, vis, vis_dtype, uvw_m, chan_freq_hz, n_chan, n_rows);
+    if (rc) return rc;
+    if (p->d.cube && !image_out) { p->err = "cube mode needs image_out"; return RICK_ERR_INVALID; }
+    p->state = 0;
+    if ((rc = prepare(p, chan_freq_hz, n_chan, n_rows))) return rc;
+    if ((rc = rick_index_sort(p, uvw_m, weights))) return rc;
+    const size_t NN = (size_t)p->N * p->N;
+    for (int img = 0; img < p->n_img; ++img) {
+        double* dst = p->d.cube ? image_out + (size_t)img * NN : p->image;
+        for (int z0 = 0; z0 < p->Nw; z0 += p->batch) {
+            const int nb = p->Nw - z0 < p->batch ? p->Nw - z0 : p->batch;
+            const int last = z0 + nb >= p->Nw;
+            if ((rc = rick_zero_planes(p, nb))) return rc;
+            if ((rc = rick_grid_planes(p, vis, vis_dtype, uvw_m, weights, img * p->Nw + z0, nb))) return rc;
+            if ((rc = rick_fft_planes(p, nb))) return rc;
+            if ((rc = rick_wcorrect(p, img, z0, nb, dst, z0 > 0, last))) return rc;
+        }
+    }
+    if (!p->d.cube) {
+        if (image_out)
+            RICK_CUDA(p, cudaMemcpyAsync(image_out, p->image, sizeof(double) * NN, cudaMemcpyDeviceToDevice, p->stream));
+        // the staged state machine may continue only if the whole stack is what is resident
+        p->state = 4;
+    }
+    return RICK_OK;
+}
+
+template <typename Tp> static int ensure_bytes(rick_plan_t* p, Tp** buf, size_t* cap, size_t bytes)
+{
+    if (*cap >= bytes) return RICK_OK;
+    free_dev(*buf);
+    *buf = nullptr;
+    *cap = 0;
+    RICK_CUDA(p, cudaMalloc(buf, bytes ? bytes : 16));
+    *cap = bytes;
+    return RICK_OK;
+}
+
+extern "C" int rick_image_host(rick_plan_t* p, const void* vis_host, int32_t vis_dtype, const double* uvw_m_host,
+                               const float* weights_host, const double* chan_freq_hz, int32_t n_chan,
+                               int64_t n_rows, double* image_out_host)
+{
+    if (!p) return RICK_ERR_INVALID;
+    p->err.clear();
+    if (!image_out_host) { p->err = "null image_out_host"; return RICK_ERR_INVALID; }
+    int rc = check_inputs(p, vis_host, vis_dtype, uvw_m_host, chan_freq_hz, n_chan, n_rows);
+    if (rc) return rc;
+    const size_t M = (size_t)n_rows * (size_t)n_chan;
+    const size_t vis_bytes = M * (vis_dtype == RICK_VIS_C128 ? 16 : 8);
+    const size_t NN = (size_t)p->N * p->N;
+    const size_t n_img = p->d.cube ? (size_t)n_chan : 1;
+    if ((rc = ensure_bytes(p, &p->st_vis, &p->st_vis_cap, vis_bytes))) return rc;
+    if ((rc = ensure_bytes(p, &p->st_uvw, &p->st_uvw_cap, sizeof(double) * 3 * (size_t)n_rows))) return rc;
+    if (weights_host && (rc = ensure_bytes(p, &p->st_wgt, &p->st_wgt_cap, sizeof(float) * M))) return rc;
+    if ((rc = ensure_bytes(p, &p->st_img, &p->st_img_cap, sizeof(double) * NN * n_img))) return rc;
+    if (M) {
+        RICK_CUDA(p, cudaMemcpyAsync(p->st_vis, vis_host, vis_bytes, cudaMemcpyHostToDevice, p->stream));
+        RICK_CUDA(p, cudaMemcpyAsync(p->st_uvw, uvw_m_host, sizeof(double) * 3 * (size_t)n_rows, cudaMemcpyHostToDevice, p->stream));
+        if (weights_host)
+            RICK_CUDA(p, cudaMemcpyAsync(p->st_wgt, weights_host, sizeof(float) * M, cudaMemcpyHostToDevice, p->stream));
+    }
+    rc = rick_image(p, p->st_vis, vis_dtype, p->st_uvw, weights_host ? p->st_wgt : nullptr, chan_freq_hz,
+                    n_chan, n_rows, p->st_img);
+    if (rc) return rc;
+    RICK_CUDA(p, cudaMemcpyAsync(image_out_host, p->st_img, sizeof(double) * NN * n_img, cudaMemcpyDeviceToHost, p->stream));
+    RICK_CUDA(p, cudaStreamSynchronize(p->stream));
+    return RICK_OK;
+}
+
+extern "C" int rick_get_image(rick_plan_t* p, double* dst_device)
+{
+    if (!p || !dst_device) return RICK_ERR_INVALID;
+    p->err.clear();
+    if (p->d.cube) { p->err = "rick_get_image: cube plans return their images through image_out"; return RICK_ERR_STATE; }
+    if (p->state < 3) { p->err = "no image yet"; return RICK_ERR_STATE; }
+    RICK_CUDA(p, cudaMemcpyAsync(dst_device, p->image, sizeof(double) * (size_t)p->N * p->N, cudaMemcpyDeviceToDevice, p->stream));
+    return RICK_OK;
+}
+
+extern "C" int rick_get_stats(rick_plan_t* p, rick_stats* out)
+{
+    if (!p || !out) return RICK_ERR_INVALID;
+    p->err.clear();
+    DevCounters c;
+    WRange w;
+    memset(&w, 0, sizeof(w));
+    RICK_CUDA(p, cudaStreamSynchronize(p->stream));
+    RICK_CUDA(p, cudaMemcpy(&c, p->counters, sizeof(c), cudaMemcpyDeviceToHost));
+    if (p->wrange) RICK_CUDA(p, cudaMemcpy(&w, p->wrange, sizeof(w), cudaMemcpyDeviceToHost));
+    out->n_vis = p->M;
+    out->n_gridded = (int64_t)c.n_gridded;
+    out->n_dropped = (int64_t)c.n_dropped;
+    out->sum_w = c.sum_w;
+    out->w_min = w.w_min;
+    out->w_max = w.w_max;
+    out->n_launches = p->n_launches;
+    return RICK_OK;
+}
+
+extern "C" const uint32_t* rick_debug_keys(rick_plan_t* p) { return (p && p->cap_vis >= 0 && p->keys) ? p->keys : nullptr; }
+extern "C" const uint32_t* rick_debug_perm(rick_plan_t* p) { return p ? p->sorted_perm : nullptr; }
+extern "C" void* rick_debug_planes(rick_plan_t* p) { return (p && p->state >= 1) ? p->stack : nullptr; }

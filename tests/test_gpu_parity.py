@@ -1,0 +1,264 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element on
+the same seeded inputs.  Bars (BASELINE.json north_star): keys / permutation / counts
+bit-exact; planes and images relative L2 <= 1e-10 (fp64 grid) / <= 1e-4 (fp32 grid)."""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_2601_19714_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+TOL64, TOL32 = 1e-10, 1e-4
+
+
+def _rel(a, b):
+    a = np.asarray(a)
+    b = np.asarray(b)
+    nb = np.linalg.norm(b.ravel())
+    return np.linalg.norm((a - b).ravel()) / (nb if nb > 0 else 1.0)
+
+
+def _rick():
+    import torch
+    assert torch.cuda.is_available(), "these tests need the B200"
+    from paper_2601_19714_b200 import rick
+    return rick
+
+
+def _oracle(wl, **kw):
+    return oracle.image(wl.uvw_m, wl.freq_hz, wl.vis, wl.weights, wl.n, wl.n_wplanes, wl.support,
+                        wl.pixel_rad, cube=wl.cube, **kw)
+
+
+def _staged(wl, tile=0):
+    rick = _rick()
+    plan = rick.plan_from_workload(wl, tile=tile, plane_batch=0)
+    vis, uvw, wgt = rick.to_device(wl)
+    out = {}
+    plan.rick_grid(vis, uvw, wgt, wl.freq_hz)
+    out["keys"] = plan.debug_keys().cpu().numpy().view(np.uint32)
+    out["perm"] = plan.debug_perm().cpu().numpy().view(np.uint32)
+    out["grid"] = plan.debug_planes().cpu().numpy()
+    plan.rick_fft_wplanes()
+    out["fft"] = plan.debug_planes().cpu().numpy()
+    plan.rick_wcorrect_accumulate()
+    out["raw"] = plan.rick_get_image().cpu().numpy()
+    plan.rick_gridcorrect()
+    out["image"] = plan.rick_get_image().cpu().numpy()
+    out["stats"] = plan.rick_get_stats()
+    plan.destroy()
+    return out
+
+
+def _check_staged(wl, tol, tile=0):
+    B = tile or 16
+    g = _staged(wl, tile=tile)
+    o = _oracle(wl, B=B, want_stacks=True, want_raw=True)
+    idx = oracle.index(wl.uvw_m, wl.freq_hz, wl.n, wl.n_wplanes, wl.support, wl.pixel_rad, B)
+    assert np.array_equal(g["keys"], idx["key"])                       # bit-exact
+    assert np.array_equal(g["perm"], oracle.sort(idx["key"]))          # bit-exact, stable
+    st = g["stats"]
+    assert st["n_vis"] == o["stats"]["n_vis"] and st["n_gridded"] == o["stats"]["n_gridded"]
+    assert st["n_dropped"] == o["stats"]["n_dropped"]
+    assert st["w_min"] == o["stats"]["w_min"] and st["w_max"] == o["stats"]["w_max"]
+    assert abs(st["sum_w"] - o["stats"]["sum_w"]) <= 1e-9 * max(1.0, o["stats"]["sum_w"])
+    errs = dict(grid=_rel(g["grid"], o["stack_grid"]), fft=_rel(g["fft"], o["stack_fft"]),
+                raw=_rel(g["raw"], o["raw_image"]), image=_rel(g["image"], o["image"]))
+    pk = np.unravel_index(np.argmax(np.abs(o["image"])), o["image"].shape)
+    print(wl.name, "rel L2:", {k: f"{v:.2e}" for k, v in errs.items()},
+          "peak pixel", pk, "oracle", o["image"][pk], "gpu", g["image"][pk])
+    for k, v in errs.items():
+        assert v <= tol, (k, v)
+    assert abs(g["image"][pk] - o["image"][pk]) <= 10 * tol * abs(o["image"][pk])
+    return g, o
+
+
+def test_cfg1_stagewise(cfg1):
+    _check_staged(cfg1, TOL64)
+
+
+def test_cfg1_tile_sizes(cfg1):
+    for tile in (8, 32):
+        _check_staged(cfg1, TOL64, tile=tile)
+
+
+def test_cfg1_rick_image_equals_staged(cfg1):
+    rick = _rick()
+    wl = cfg1
+    plan = rick.plan_from_workload(wl)
+    vis, uvw, wgt = rick.to_device(wl)
+    img = plan.rick_image(vis, uvw, wgt, wl.freq_hz).cpu().numpy()
+    o = _oracle(wl)
+    assert _rel(img, o["image"]) <= TOL64
+    assert _rel(plan.rick_get_image().cpu().numpy(), o["image"]) <= TOL64
+    # repeated calls on the same plan give the same answer (scratch reuse, counters reset)
+    img2 = plan.rick_image(vis, uvw, wgt, wl.freq_hz).cpu().numpy()
+    assert _rel(img2, o["image"]) <= TOL64
+    assert plan.rick_get_stats()["n_gridded"] == o["stats"]["n_gridded"]
+    plan.destroy()
+
+
+def test_cfg2_midsize_weights_ragged():
+    # MeerKAT-shaped, several tiles / chunks / radix tiles with ragged tails, weighted
+    wl = synth.make_config(2, n_times=13, n=1024, n_wplanes=5, n_src=20, with_weights=True)
+    assert wl.n_vis % 4096 != 0 and wl.n_vis % 128 != 0
+    _check_staged(wl, TOL64)
+
+
+def test_cfg3_midsize_lofar_shape():
+    wl = synth.make_config(3, n_times=24, n=2048, n_wplanes=6, n_src=30)
+    g, o = _check_staged(wl, TOL64)
+    assert o["stats"]["n_dropped"] > 0
+
+
+def test_support_and_beta_variants():
+    wl = synth.make_config(1, n_times=8)
+    rick = _rick()
+    vis, uvw, wgt = rick.to_device(wl)
+    for S, beta in [(3, 0.0), (5, 9.0), (9, 0.0), (15, 0.0)]:
+        plan = rick.Plan(wl.n, wl.n_wplanes, S, wl.pixel_rad, kb_beta=beta)
+        img = plan.rick_image(vis, uvw, wgt, wl.freq_hz).cpu().numpy()
+        plan.destroy()
+        o = oracle.image(wl.uvw_m, wl.freq_hz, wl.vis, None, wl.n, wl.n_wplanes, S, wl.pixel_rad, beta=beta)
+        assert _rel(img, o["image"]) <= TOL64, (S, beta)
+
+
+def test_fp32_grid_plane_batches():
+    # config-4-shaped: fp32 grid, planes streamed in ragged batches into one image
+    wl = synth.make_config(4, n_times=24, n=1024, n_wplanes=8, n_src=20)
+    rick = _rick()
+    vis, uvw, wgt = rick.to_device(wl)
+    o = _oracle(wl)
+    for pb in (3, 8, 1):
+        plan = rick.plan_from_workload(wl, plane_batch=pb)
+        img = plan.rick_image(vis, uvw, wgt, wl.freq_hz).cpu().numpy()
+        plan.destroy()
+        e = _rel(img, o["image"])
+        N = wl.n
+        inner = slice(N // 4, 3 * N // 4)
+        pk = np.unravel_index(np.argmax(np.abs(o["image"])), o["image"].shape)
+        print(f"fp32 batch {pb}: rel L2 {e:.2e}, inner half {_rel(img[inner, inner], o['image'][inner, inner]):.2e},"
+              f" peak {pk} oracle {o['image'][pk]:.6e} gpu {img[pk]:.6e}")
+        assert e <= TOL32
+
+
+def test_fp64_plane_batches_equal_resident():
+    wl = synth.make_config(2, n_times=6, n=512, n_wplanes=7, n_src=10)
+    rick = _rick()
+    vis, uvw, wgt = rick.to_device(wl)
+    o = _oracle(wl)
+    for pb in (0, 2, 7):
+        plan = rick.plan_from_workload(wl, plane_batch=pb)
+        img = plan.rick_image(vis, uvw, wgt, wl.freq_hz).cpu().numpy()
+        plan.destroy()
+        assert _rel(img, o["image"]) <= TOL64
+
+
+def test_cube_mode():
+    wl = synth.make_config(5, n_times=6, n=256, n_chan=5, n_wplanes=4, n_src=10)
+    rick = _rick()
+    vis, uvw, wgt = rick.to_device(wl)
+    plan = rick.plan_from_workload(wl)
+    cube = plan.rick_image(vis, uvw, wgt, wl.freq_hz).cpu().numpy()
+    keys = plan.debug_keys().cpu().numpy().view(np.uint32)
+    perm = plan.debug_perm().cpu().numpy().view(np.uint32)
+    plan.destroy()
+    o = _oracle(wl)
+    assert cube.shape == (5, wl.n, wl.n)
+    idx = oracle.index(wl.uvw_m, wl.freq_hz, wl.n, wl.n_wplanes, wl.support, wl.pixel_rad, 16, cube=1)
+    assert np.array_equal(keys, idx["key"]) and np.array_equal(perm, oracle.sort(idx["key"]))
+    for c in range(5):
+        assert _rel(cube[c], o["image"][c]) <= TOL64, c
+
+
+def test_given_w_range():
+    wl = synth.make_config(1, n_times=8)
+    rick = _rick()
+    vis, uvw, wgt = rick.to_device(wl)
+    plan = rick.plan_from_workload(wl, w_min=-5000.0, w_max=6000.0)
+    img = plan.rick_image(vis, uvw, wgt, wl.freq_hz).cpu().numpy()
+    st = plan.rick_get_stats()
+    plan.destroy()
+    o = oracle.image(wl.uvw_m, wl.freq_hz, wl.vis, None, wl.n, wl.n_wplanes, wl.support, wl.pixel_rad,
+                     w_min=-5000.0, w_max=6000.0)
+    assert st["w_min"] == -5000.0 and st["w_max"] == 6000.0
+    assert _rel(img, o["image"]) <= TOL64
+
+
+def test_edge_cases_empty_dropped_single():
+    import torch
+    rick = _rick()
+    N, dl = 256, 1e-4
+    freq = np.array([synth.C0])
+    plan = rick.Plan(N, 4, 7, dl)
+    # empty input -> zero image
+    img = plan.rick_image(torch.zeros((0, 1), dtype=torch.complex64, device="cuda"),
+                          torch.zeros((0, 3), dtype=torch.float64, device="cuda"), None, freq)
+    assert float(img.abs().max()) == 0.0 and plan.rick_get_stats()["n_vis"] == 0
+    # every visibility off the grid -> zero image, all dropped
+    du = 1.0 / (N * dl)
+    uvw = torch.tensor([[200.0 * du, 0.0, 1.0], [0.0, -126.0 * du, 2.0]], dtype=torch.float64, device="cuda")
+    vis = torch.ones((2, 1), dtype=torch.complex128, device="cuda")
+    img = plan.rick_image(vis, uvw, None, freq)
+    st = plan.rick_get_stats()
+    assert float(img.abs().max()) == 0.0 and st["n_dropped"] == 2 and st["n_gridded"] == 0
+    # a single visibility, all w equal (dw = 0 -> plane 0)
+    uvw = torch.tensor([[3.3 * du, -7.45 * du, 5.0]], dtype=torch.float64, device="cuda")
+    vis = torch.tensor([[1.5 - 0.25j]], dtype=torch.complex128, device="cuda")
+    img = plan.rick_image(vis, uvw, None, freq).cpu().numpy()
+    o = oracle.image(uvw.cpu().numpy(), freq, vis.cpu().numpy(), None, N, 4, 7, dl)
+    assert _rel(img, o["image"]) <= TOL64
+    # footprint touching cell 0 / N-1 is kept
+    uvw = torch.tensor([[(3 - N // 2) * du, (N - 4 - N // 2) * du, 0.0]], dtype=torch.float64, device="cuda")
+    img = plan.rick_image(vis, uvw, None, freq).cpu().numpy()
+    o = oracle.image(uvw.cpu().numpy(), freq, vis.cpu().numpy(), None, N, 4, 7, dl)
+    assert plan.rick_get_stats()["n_gridded"] == 1 and _rel(img, o["image"]) <= TOL64
+    plan.destroy()
+
+
+def test_state_machine_and_argument_errors(cfg1):
+    import torch
+    rick = _rick()
+    wl = cfg1
+    plan = rick.plan_from_workload(wl)
+    with pytest.raises(rick.RickError) as e:
+        plan.rick_fft_wplanes()
+    assert e.value.code == rick.RICK_ERR_STATE
+    vis, uvw, wgt = rick.to_device(wl)
+    plan.rick_grid(vis, uvw, wgt, wl.freq_hz)
+    with pytest.raises(rick.RickError):
+        plan.rick_gridcorrect()
+    with pytest.raises(rick.RickError) as e:
+        plan.rick_grid(vis, uvw, wgt, np.array([-1.0]))
+    assert e.value.code == rick.RICK_ERR_INVALID
+    plan.destroy()
+    for bad in [dict(n=100), dict(support=6), dict(support=17), dict(pixel_rad=0.0), dict(n_wplanes=0),
+                dict(tile=12), dict(plane_batch=99)]:
+        kw = dict(n=256, n_wplanes=8, support=7, pixel_rad=1e-4)
+        kw.update(bad)
+        with pytest.raises(rick.RickError) as e:
+            rick.Plan(**kw)
+        assert e.value.code == rick.RICK_ERR_INVALID
+    # staged calls are refused on batched / cube plans
+    p2 = rick.Plan(256, 8, 7, 1e-4, plane_batch=2)
+    with pytest.raises(rick.RickError) as e:
+        p2.rick_grid(vis, uvw, wgt, wl.freq_hz)
+    assert e.value.code == rick.RICK_ERR_STATE
+    p2.destroy()
+
+
+def test_host_buffer_entry(cfg1):
+    import torch
+    rick = _rick()
+    wl = cfg1
+    plan = rick.plan_from_workload(wl)
+    vis = torch.from_numpy(wl.vis).pin_memory()
+    uvw = torch.from_numpy(wl.uvw_m).pin_memory()
+    out = torch.empty((wl.n, wl.n), dtype=torch.float64).pin_memory()
+    plan.rick_image_host(vis, uvw, None, wl.freq_hz, out)
+    o = _oracle(wl)
+    assert _rel(out.numpy(), o["image"]) <= TOL64
+    plan.destroy()
