@@ -55,13 +55,13 @@ enum { RICK_GRID_F64 = 0, RICK_GRID_F32 = 1 };
 enum { RICK_VIS_C64 = 0, RICK_VIS_C128 = 1 };
 
 typedef struct {
-    int32_t n;           /* grid edge N: power of two, 64 <= N <= 32768                         */
+    int32_t n;           /* grid edge N: power of two, 64 <= N <= 16384 (8192 for F64)                        */
     int32_t n_wplanes;   /* N_w >= 1                                                            */
     int32_t support;     /* S, odd, 3..15 (Eq. 5: full kernel width in cells)                   */
     double  pixel_rad;   /* dl, radians per pixel, > 0                                          */
     double  kb_beta;     /* Kaiser-Bessel beta; <= 0 -> 2.34*S (reading R5)                     */
     int32_t grid_prec;   /* RICK_GRID_F64 (complex double mesh) | RICK_GRID_F32   */
-    int32_t tile;        /* sort-tile edge B in cells (power of two, 8..64); 0 -> 16            */
+    int32_t tile;        /* sort-tile edge B in cells (power of two, 8..32); 0 -> 16            */
     int32_t plane_batch; /* w-planes resident at once; 0 -> all N_w                             */
     int32_t cube;        /* 0: all channels into one image; 1: one image per channel (R16)      */
     int32_t reserved;    /* must be 0                                                           */
@@ -140,6 +140,16 @@ const char* rick_last_error(const rick_plan_t* p);
 const uint32_t* rick_debug_keys(rick_plan_t* p);   /* [M] keys in visibility order          */
 const uint32_t* rick_debug_perm(rick_plan_t* p);   /* [M] stable permutation (sorted order) */
 void*           rick_debug_planes(rick_plan_t* p); /* [N_w][N][N] complex of grid_prec      */
+
+/* Per-kernel timing with CUDA events on the plan's stream (for roofline reporting).
+ * rick_profile(p, 1) clears the records and brackets every later kernel launch with a
+ * pair of events; rick_profile(p, 0) stops.  Both SYNCHRONISE the stream.
+ * rick_profile_read SYNCHRONISES and returns, for one kernel class, the summed duration in
+ * milliseconds and the number of launches since profiling was enabled.
+ * rick_kernel_name(id): "grid", "fft_rows", "fft_cols", "wcorrect", ...; NULL past the end. */
+int rick_profile(rick_plan_t* p, int32_t enable);
+int rick_profile_read(rick_plan_t* p, int32_t kernel_id, double* total_ms, int64_t* launches);
+const char* rick_kernel_name(int32_t kernel_id);
 
 /* Library identification, e.g. "librick_b200 0.1 sm_100a". */
 const char* rick_version(void);

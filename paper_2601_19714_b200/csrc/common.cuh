@@ -69,6 +69,14 @@ struct rick_plan_s {
     DevCounters* counters;   // device
     int64_t M; int32_t C; int64_t R; int n_img;
 
+    // optional per-kernel CUDA-event timing (rick_profile)
+    int prof_on;
+    std::vector<cudaEvent_t> prof_ev;       // pool: 2 events per record
+    std::vector<int> prof_id;               // kernel class of each record
+    size_t prof_n;                          // records in use
+    double prof_ms[32];                     // aggregated by rick_profile_read
+    long long prof_cnt[32];
+
     // host-buffer staging for rick_image_host
     void* st_vis; size_t st_vis_cap;
     double* st_uvw; size_t st_uvw_cap;
@@ -83,6 +91,22 @@ struct rick_plan_s {
             (p)->err = std::string(#call) + ": " + cudaGetErrorString(e__);            \
             return e__ == cudaErrorMemoryAllocation ? RICK_ERR_OOM : RICK_ERR_CUDA;    \
         }                                                                              \
+    } while (0)
+
+// kernel classes for rick_profile_read / rick_kernel_name
+enum { RK_TABLES = 0, RK_RESET, RK_WRANGE, RK_INDEX_KEY, RK_RADIX_HIST, RK_SCAN, RK_RADIX_SCATTER,
+       RK_PLANE_STARTS, RK_ZERO, RK_GRID, RK_FFT_ROWS, RK_FFT_COLS, RK_WCORRECT, RK_TAPER, RK_NKERNELS };
+
+void rick_prof_begin(rick_plan_t* p, int id);   // plan.cu; no-ops unless profiling is on
+void rick_prof_end(rick_plan_t* p);
+
+// launch one kernel: optional CUDA-event bracket, launch counter, launch-error check
+#define RICK_KERNEL(p, id, ...)                                                        \
+    do {                                                                               \
+        rick_prof_begin((p), (id));                                                    \
+        __VA_ARGS__;                                                                   \
+        rick_prof_end((p));                                                            \
+        RICK_LAUNCHED(p);                                                              \
     } while (0)
 
 #define RICK_LAUNCHED(p)                                                               \

@@ -77,11 +77,9 @@ static int launch_fft(rick_plan_t* p, int n_planes)
     RICK_CUDA(p, cudaFuncSetAttribute(k_fft_cols<T, LOG2N>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                       (int)KC::SMEM));
     const unsigned int row_blocks = (unsigned int)((size_t)n_planes * KR::N / KR::RPC);
-    k_fft_rows<T, LOG2N><<<row_blocks, KR::THREADS, KR::SMEM, p->stream>>>((C*)p->stack, (const C*)p->twiddle);
-    RICK_LAUNCHED(p);
+    RICK_KERNEL(p, RK_FFT_ROWS, k_fft_rows<T, LOG2N><<<row_blocks, KR::THREADS, KR::SMEM, p->stream>>>((C*)p->stack, (const C*)p->twiddle));
     const unsigned int col_blocks = (unsigned int)((size_t)n_planes * (KC::N / KC::WC));
-    k_fft_cols<T, LOG2N><<<col_blocks, KC::THREADS, KC::SMEM, p->stream>>>((C*)p->stack, (const C*)p->twiddle);
-    RICK_LAUNCHED(p);
+    RICK_KERNEL(p, RK_FFT_COLS, k_fft_cols<T, LOG2N><<<col_blocks, KC::THREADS, KC::SMEM, p->stream>>>((C*)p->stack, (const C*)p->twiddle));
     return RICK_OK;
 }
 

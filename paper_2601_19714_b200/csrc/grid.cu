@@ -233,8 +233,7 @@ __global__ void __launch_bounds__(256) k_zero(uint4* __restrict__ dst, size_t n1
 int rick_zero_planes(rick_plan_t* p, int n_planes)
 {
     const size_t n16 = p->plane_bytes / 16 * (size_t)n_planes;
-    k_zero<<<p->n_sm * 8, 256, 0, p->stream>>>(reinterpret_cast<uint4*>(p->stack), n16);
-    RICK_LAUNCHED(p);
+    RICK_KERNEL(p, RK_ZERO, k_zero<<<p->n_sm * 8, 256, 0, p->stream>>>(reinterpret_cast<uint4*>(p->stack), n16));
     return RICK_OK;
 }
 
@@ -253,10 +252,8 @@ static int launch_grid(rick_plan_t* p, const GridParams& P)
     int per_sm = 1;
     RICK_CUDA(p, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_grid<GT, S>, GRID_WARPS * 32, smem));
     if (per_sm < 1) per_sm = 1;
-    k_chunk_reset<<<1, 1, 0, p->stream>>>(P.chunk_counter);
-    RICK_LAUNCHED(p);
-    k_grid<GT, S><<<p->n_sm * per_sm, GRID_WARPS * 32, smem, p->stream>>>(P);
-    RICK_LAUNCHED(p);
+    RICK_KERNEL(p, RK_RESET, k_chunk_reset<<<1, 1, 0, p->stream>>>(P.chunk_counter));
+    RICK_KERNEL(p, RK_GRID, k_grid<GT, S><<<p->n_sm * per_sm, GRID_WARPS * 32, smem, p->stream>>>(P));
     return RICK_OK;
 }
 

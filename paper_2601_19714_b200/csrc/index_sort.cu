@@ -329,26 +329,22 @@ int rick_index_sort(rick_plan_t* p, const double* uvw_m, const float* weights)
     const unsigned int M = (unsigned int)p->M;
     const int n_planes_total = p->n_img * p->Nw;
 
-    k_counters_reset<<<1, 1, 0, st>>>(p->counters);
-    RICK_LAUNCHED(p);
+    RICK_KERNEL(p, RK_RESET, k_counters_reset<<<1, 1, 0, st>>>(p->counters));
     if (p->R > 0) {
         int nb = (int)((p->R + 255) / 256);
         if (nb > p->n_sm * 8) nb = p->n_sm * 8;
-        k_wrange_rows<<<nb, 256, 0, st>>>(uvw_m, (long long)p->R, p->counters);
-        RICK_LAUNCHED(p);
+        RICK_KERNEL(p, RK_WRANGE, k_wrange_rows<<<nb, 256, 0, st>>>(uvw_m, (long long)p->R, p->counters));
     }
-    k_wrange_finish<<<(p->n_img + 127) / 128, 128, 0, st>>>(p->counters, p->chan_scale, p->C, p->d.cube,
+    RICK_KERNEL(p, RK_WRANGE, k_wrange_finish<<<(p->n_img + 127) / 128, 128, 0, st>>>(p->counters, p->chan_scale, p->C, p->d.cube,
                                                           p->Nw, p->d.w_min, p->d.w_max,
-                                                          (long long)p->R, p->wrange);
-    RICK_LAUNCHED(p);
+                                                          (long long)p->R, p->wrange));
 
     p->sorted_keys = p->keys;
     p->sorted_perm = p->perm_a;
     if (M > 0) {
-        k_index_key<<<(M + 255) / 256, 256, 0, st>>>(uvw_m, weights, p->chan_scale, p->wrange, M,
+        RICK_KERNEL(p, RK_INDEX_KEY, k_index_key<<<(M + 255) / 256, 256, 0, st>>>(uvw_m, weights, p->chan_scale, p->wrange, M,
                                                     (unsigned)p->C, p->N, p->Nw, p->h, p->B, p->T,
-                                                    p->d.cube, p->inv_du, p->keys, p->counters);
-        RICK_LAUNCHED(p);
+                                                    p->d.cube, p->inv_du, p->keys, p->counters));
 
         // key bits: the all-ones pattern of the sorted bit range is reserved for the sentinel
         const unsigned long long nkeys = (unsigned long long)n_planes_total * p->T * p->T;
@@ -372,21 +368,16 @@ int rick_index_sort(rick_plan_t* p, const double* uvw_m, const float* weights)
             const int nb_bits = (bits - shift + (npass - pass) - 1) / (npass - pass);
             const int nbins = 1 << nb_bits;
             const uint32_t mask = (uint32_t)(nbins - 1);
-            k_radix_hist<<<nblocks, RS_THREADS, 0, st>>>(kin, M, shift, mask, nbins, p->hist, nblocks);
-            RICK_LAUNCHED(p);
+            RICK_KERNEL(p, RK_RADIX_HIST, k_radix_hist<<<nblocks, RS_THREADS, 0, st>>>(kin, M, shift, mask, nbins, p->hist, nblocks));
             const size_t n_hist = (size_t)nbins * nblocks;
             const unsigned int nsb = (unsigned int)((n_hist + SC_TILE - 1) / SC_TILE);
-            k_scan_reduce<<<nsb, SC_THREADS, 0, st>>>(p->hist, n_hist, p->scan_tmp);
-            RICK_LAUNCHED(p);
-            k_scan_top<<<1, SC_THREADS, 0, st>>>(p->scan_tmp, nsb);
-            RICK_LAUNCHED(p);
-            k_scan_apply<<<nsb, SC_THREADS, 0, st>>>(p->hist, n_hist, p->scan_tmp);
-            RICK_LAUNCHED(p);
+            RICK_KERNEL(p, RK_SCAN, k_scan_reduce<<<nsb, SC_THREADS, 0, st>>>(p->hist, n_hist, p->scan_tmp));
+            RICK_KERNEL(p, RK_SCAN, k_scan_top<<<1, SC_THREADS, 0, st>>>(p->scan_tmp, nsb));
+            RICK_KERNEL(p, RK_SCAN, k_scan_apply<<<nsb, SC_THREADS, 0, st>>>(p->hist, n_hist, p->scan_tmp));
             uint32_t* ko = kbuf[pass & 1];
             uint32_t* vo = vbuf[pass & 1];
-            k_radix_scatter<<<nblocks, RS_THREADS, 0, st>>>(kin, vin, ko, vo, M, shift, mask, nbins,
-                                                          p->hist, nblocks);
-            RICK_LAUNCHED(p);
+            RICK_KERNEL(p, RK_RADIX_SCATTER, k_radix_scatter<<<nblocks, RS_THREADS, 0, st>>>(kin, vin, ko, vo, M, shift, mask, nbins,
+                                                          p->hist, nblocks));
             kin = ko;
             vin = vo;
             shift += nb_bits;
@@ -394,8 +385,7 @@ int rick_index_sort(rick_plan_t* p, const double* uvw_m, const float* weights)
         p->sorted_keys = (uint32_t*)kin;
         p->sorted_perm = (uint32_t*)vin;
     }
-    k_plane_starts<<<(n_planes_total + 1 + 127) / 128, 128, 0, st>>>(
-        p->sorted_keys, M, (unsigned long long)p->T * p->T, n_planes_total, (long long*)p->plane_start);
-    RICK_LAUNCHED(p);
+    RICK_KERNEL(p, RK_PLANE_STARTS, k_plane_starts<<<(n_planes_total + 1 + 127) / 128, 128, 0, st>>>(
+        p->sorted_keys, M, (unsigned long long)p->T * p->T, n_planes_total, (long long*)p->plane_start));
     return RICK_OK;
 }

@@ -14,6 +14,70 @@ static void free_dev(void* q)
     if (q) cudaFree(q);
 }
 
+// ---------------------------------------------------------------------------------------
+// per-kernel CUDA-event timing
+static const char* const k_names[RK_NKERNELS] = {
+    "tables", "reset", "wrange", "index_key", "radix_hist", "scan", "radix_scatter", "plane_starts",
+    "zero", "grid", "fft_rows", "fft_cols", "wcorrect", "taper"};
+
+void rick_prof_begin(rick_plan_t* p, int id)
+{
+    if (!p->prof_on) return;
+    if (p->prof_ev.size() < 2 * (p->prof_n + 1)) {
+        cudaEvent_t a = nullptr, b = nullptr;
+        if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) { p->prof_on = 0; return; }
+        p->prof_ev.push_back(a);
+        p->prof_ev.push_back(b);
+    }
+    if (p->prof_id.size() <= p->prof_n) p->prof_id.push_back(id); else p->prof_id[p->prof_n] = id;
+    cudaEventRecord(p->prof_ev[2 * p->prof_n], p->stream);
+}
+
+void rick_prof_end(rick_plan_t* p)
+{
+    if (!p->prof_on) return;
+    cudaEventRecord(p->prof_ev[2 * p->prof_n + 1], p->stream);
+    p->prof_n++;
+}
+
+static void prof_collect(rick_plan_t* p)
+{
+    cudaStreamSynchronize(p->stream);
+    for (size_t i = 0; i < p->prof_n; ++i) {
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, p->prof_ev[2 * i], p->prof_ev[2 * i + 1]) == cudaSuccess) {
+            p->prof_ms[p->prof_id[i]] += (double)ms;
+            p->prof_cnt[p->prof_id[i]]++;
+        }
+    }
+    p->prof_n = 0;
+}
+
+extern "C" int rick_profile(rick_plan_t* p, int32_t enable)
+{
+    if (!p) return RICK_ERR_INVALID;
+    prof_collect(p);
+    if (enable) {
+        for (int i = 0; i < 32; ++i) { p->prof_ms[i] = 0.0; p->prof_cnt[i] = 0; }
+    }
+    p->prof_on = enable ? 1 : 0;
+    return RICK_OK;
+}
+
+extern "C" int rick_profile_read(rick_plan_t* p, int32_t kernel_id, double* total_ms, int64_t* launches)
+{
+    if (!p || kernel_id < 0 || kernel_id >= RK_NKERNELS) return RICK_ERR_INVALID;
+    prof_collect(p);
+    if (total_ms) *total_ms = p->prof_ms[kernel_id];
+    if (launches) *launches = (int64_t)p->prof_cnt[kernel_id];
+    return RICK_OK;
+}
+
+extern "C" const char* rick_kernel_name(int32_t kernel_id)
+{
+    return (kernel_id >= 0 && kernel_id < RK_NKERNELS) ? k_names[kernel_id] : nullptr;
+}
+
 extern "C" const char* rick_version(void) { return "librick_b200 0.1 sm_100a"; }
 
 extern "C" const char* rick_last_error(const rick_plan_t* p) { return p ? p->err.c_str() : "null plan"; }
@@ -27,6 +91,7 @@ extern "C" int rick_plan_destroy(rick_plan_t* p)
     free_dev(p->hist); free_dev(p->scan_tmp); free_dev(p->plane_start); free_dev(p->chan_scale);
     free_dev(p->wrange); free_dev(p->counters);
     free_dev(p->st_vis); free_dev(p->st_uvw); free_dev(p->st_wgt); free_dev(p->st_img);
+    for (cudaEvent_t e : p->prof_ev) cudaEventDestroy(e);
     if (p->h_scale) cudaFreeHost(p->h_scale);
     if (p->ev_scale) cudaEventDestroy(p->ev_scale);
     delete p;

@@ -71,14 +71,13 @@ int rick_tables_build(rick_plan_t* p)
     RICK_CUDA(p, cudaStreamSynchronize(p->stream));   // cd is a local
 
     RICK_CUDA(p, cudaMalloc(&p->taper, sizeof(double) * N));
-    k_taper<<<(N + 255) / 256, 256, 0, p->stream>>>(p->taper, N, p->S, p->beta, (double)i0);
-    RICK_LAUNCHED(p);
+    RICK_KERNEL(p, RK_TABLES, k_taper<<<(N + 255) / 256, 256, 0, p->stream>>>(p->taper, N, p->S, p->beta, (double)i0));
 
     RICK_CUDA(p, cudaMalloc(&p->twiddle, (p->f32 ? sizeof(float2) : sizeof(double2)) * (size_t)N));
-    if (p->f32)
-        k_twiddle<float2><<<(N + 255) / 256, 256, 0, p->stream>>>((float2*)p->twiddle, N);
-    else
-        k_twiddle<double2><<<(N + 255) / 256, 256, 0, p->stream>>>((double2*)p->twiddle, N);
-    RICK_LAUNCHED(p);
+    if (p->f32) {
+        RICK_KERNEL(p, RK_TABLES, k_twiddle<float2><<<(N + 255) / 256, 256, 0, p->stream>>>((float2*)p->twiddle, N));
+    } else {
+        RICK_KERNEL(p, RK_TABLES, k_twiddle<double2><<<(N + 255) / 256, 256, 0, p->stream>>>((double2*)p->twiddle, N));
+    }
     return RICK_OK;
 }

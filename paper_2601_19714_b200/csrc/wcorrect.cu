@@ -75,22 +75,20 @@ int rick_wcorrect(rick_plan_t* p, int img, int z_first, int n_planes, double* im
 {
     const size_t NN = (size_t)p->N * p->N;
     const unsigned int blocks = (unsigned int)((NN + 255) / 256);
-    if (p->f32)
-        k_wcorrect<float2><<<blocks, 256, 0, p->stream>>>((const float2*)p->stack, n_planes, z_first, p->N,
-                                                        p->dl, p->wrange + img, image, accumulate,
-                                                        fuse_taper ? p->taper : nullptr);
-    else
-        k_wcorrect<double2><<<blocks, 256, 0, p->stream>>>((const double2*)p->stack, n_planes, z_first, p->N,
-                                                         p->dl, p->wrange + img, image, accumulate,
-                                                         fuse_taper ? p->taper : nullptr);
-    RICK_LAUNCHED(p);
+    const double* tp = fuse_taper ? p->taper : nullptr;
+    if (p->f32) {
+        RICK_KERNEL(p, RK_WCORRECT, k_wcorrect<float2><<<blocks, 256, 0, p->stream>>>(
+            (const float2*)p->stack, n_planes, z_first, p->N, p->dl, p->wrange + img, image, accumulate, tp));
+    } else {
+        RICK_KERNEL(p, RK_WCORRECT, k_wcorrect<double2><<<blocks, 256, 0, p->stream>>>(
+            (const double2*)p->stack, n_planes, z_first, p->N, p->dl, p->wrange + img, image, accumulate, tp));
+    }
     return RICK_OK;
 }
 
 int rick_taper_divide(rick_plan_t* p, double* image)
 {
     const size_t NN = (size_t)p->N * p->N;
-    k_taper_divide<<<(unsigned int)((NN + 255) / 256), 256, 0, p->stream>>>(image, p->N, p->taper);
-    RICK_LAUNCHED(p);
+    RICK_KERNEL(p, RK_TAPER, k_taper_divide<<<(unsigned int)((NN + 255) / 256), 256, 0, p->stream>>>(image, p->N, p->taper));
     return RICK_OK;
 }

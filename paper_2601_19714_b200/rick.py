@@ -24,7 +24,8 @@ RICK_VIS_C64, RICK_VIS_C128 = 0, 1
 EXPORTS = ["rick_plan", "rick_plan_destroy", "rick_grid", "rick_fft_wplanes",
            "rick_wcorrect_accumulate", "rick_gridcorrect", "rick_image", "rick_image_host",
            "rick_get_image", "rick_get_stats", "rick_last_error", "rick_debug_keys",
-           "rick_debug_perm", "rick_debug_planes", "rick_version"]
+           "rick_debug_perm", "rick_debug_planes", "rick_version", "rick_profile",
+           "rick_profile_read", "rick_kernel_name"]
 
 
 class PlanDesc(C.Structure):
@@ -78,6 +79,10 @@ def load_library():
     L.rick_debug_planes.argtypes = [vp]
     L.rick_debug_planes.restype = vp
     L.rick_version.restype = C.c_char_p
+    L.rick_profile.argtypes = [vp, i32]
+    L.rick_profile_read.argtypes = [vp, i32, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
+    L.rick_kernel_name.argtypes = [i32]
+    L.rick_kernel_name.restype = C.c_char_p
     for name in EXPORTS:
         getattr(L, name)
     _lib = L
@@ -183,6 +188,21 @@ class Plan:
         s = Stats()
         self._check(self._lib.rick_get_stats(self._h, C.byref(s)))
         return {k: getattr(s, k) for k, _ in Stats._fields_}
+
+    def rick_profile(self, enable: bool):
+        self._check(self._lib.rick_profile(self._h, 1 if enable else 0))
+
+    def rick_profile_read(self) -> dict:
+        """{kernel name: (total_ms, launches)} since profiling was enabled (synchronises)."""
+        out, i = {}, 0
+        while True:
+            name = self._lib.rick_kernel_name(i)
+            if name is None:
+                return out
+            ms, n = C.c_double(), C.c_int64()
+            self._check(self._lib.rick_profile_read(self._h, i, C.byref(ms), C.byref(n)))
+            out[name.decode()] = (ms.value, n.value)
+            i += 1
 
     # -- debug accessors (copies, synchronising) -------------------------------------------
     def _copy_from(self, ptr, nbytes, dtype, shape):

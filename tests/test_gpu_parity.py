@@ -103,7 +103,7 @@ def test_cfg1_rick_image_equals_staged(cfg1):
 
 def test_cfg2_midsize_weights_ragged():
     # MeerKAT-shaped, several tiles / chunks / radix tiles with ragged tails, weighted
-    wl = synth.make_config(2, n_times=13, n=1024, n_wplanes=5, n_src=20, with_weights=True)
+    wl = synth.make_config(2, n_times=13, n=1024, n_chan=13, n_wplanes=5, n_src=20, with_weights=True)
     assert wl.n_vis % 4096 != 0 and wl.n_vis % 128 != 0
     _check_staged(wl, TOL64)
 
