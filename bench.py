@@ -152,15 +152,19 @@ def main():
     # stage numbers (BASELINE.json's three-part metric), from the per-kernel events
     def ms_of(*names):
         return sum(prof[n][0] for n in names if n in prof) / args.steps
+    fused = ms_of("fft_cols_wcorrect") > 0
     t_sortgrid = ms_of("reset", "wrange", "index_key", "radix_hist", "scan", "radix_scatter", "plane_starts",
                        "zero", "grid")
     stages = {
         "grid_mvis_s_a0_a3": n_gridded / (t_sortgrid * 1e-3) / 1e6 if t_sortgrid else None,
         "grid_kernel_mvis_s": n_gridded / (ms_of("grid") * 1e-3) / 1e6 if ms_of("grid") else None,
-        "fft_gb_s": 4 * stack_bytes / (ms_of("fft_rows", "fft_cols") * 1e-3) / 1e9,
-        "wcorrect_gb_s": (stack_bytes + image_bytes) / (ms_of("wcorrect", "taper") * 1e-3) / 1e9,
-        "fft_plus_wcorrect_gb_s": (5 * stack_bytes + image_bytes) /
-                                  (ms_of("fft_rows", "fft_cols", "wcorrect", "taper") * 1e-3) / 1e9,
+        # a4 + a5 + a6 move 3 x stack + image when the column pass is fused with the correction
+        # (rows: read + write; columns+correction: read), else 5 x stack + image
+        "fft_rows_gb_s": 2 * stack_bytes / (ms_of("fft_rows") * 1e-3) / 1e9 if ms_of("fft_rows") else None,
+        "fft_plus_wcorrect_gb_s": ((3 if fused else 5) * stack_bytes + image_bytes) /
+                                  (ms_of("fft_rows", "fft_cols", "wcorrect", "taper", "fft_cols_wcorrect") * 1e-3) / 1e9,
+        "fft_plus_wcorrect_ms": ms_of("fft_rows", "fft_cols", "wcorrect", "taper", "fft_cols_wcorrect"),
+        "fused_cols_wcorrect": fused,
         "image_s": ms_per_step * 1e-3,
         "kernel_ms_per_step": {k: round(v[0] / args.steps, 4) for k, v in prof.items() if v[1]},
     }
@@ -168,7 +172,7 @@ def main():
     # roofline of the dominant kernel (algorithmic bytes per launch: DESIGN.md "Kernels")
     peaks = bu.measured_peaks(ROOT)
     alg_bytes = {"fft_rows": 2 * stack_bytes, "fft_cols": 2 * stack_bytes, "zero": stack_bytes,
-                 "wcorrect": stack_bytes + image_bytes}
+                 "wcorrect": stack_bytes + image_bytes, "fft_cols_wcorrect": stack_bytes + image_bytes}
     dom = max((k for k in prof if prof[k][1]), key=lambda k: prof[k][0])
     traffic_ncu = {"fft_rows": None, "fft_cols": None}      # filled from profiles/ when captured
     if dom in alg_bytes:

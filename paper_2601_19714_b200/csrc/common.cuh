@@ -77,6 +77,10 @@ struct rick_plan_s {
     double prof_ms[32];                     // aggregated by rick_profile_read
     long long prof_cnt[32];
 
+    // N = 4096 fp64 column kernels (fft_cols12.cu): TMA tensor map over the resident stack
+    int cols12_ok;
+    alignas(64) unsigned char cols12_tmap[128];
+
     // host-buffer staging for rick_image_host
     void* st_vis; size_t st_vis_cap;
     double* st_uvw; size_t st_uvw_cap;
@@ -95,7 +99,8 @@ struct rick_plan_s {
 
 // kernel classes for rick_profile_read / rick_kernel_name
 enum { RK_TABLES = 0, RK_RESET, RK_WRANGE, RK_INDEX_KEY, RK_RADIX_HIST, RK_SCAN, RK_RADIX_SCATTER,
-       RK_PLANE_STARTS, RK_ZERO, RK_GRID, RK_FFT_ROWS, RK_FFT_COLS, RK_WCORRECT, RK_TAPER, RK_NKERNELS };
+       RK_PLANE_STARTS, RK_ZERO, RK_GRID, RK_FFT_ROWS, RK_FFT_COLS, RK_WCORRECT, RK_TAPER, RK_COLS_WCORRECT,
+       RK_NKERNELS };
 
 void rick_prof_begin(rick_plan_t* p, int id);   // plan.cu; no-ops unless profiling is on
 void rick_prof_end(rick_plan_t* p);
@@ -125,7 +130,13 @@ int rick_index_sort(rick_plan_t* p, const double* uvw_m, const float* weights); 
 int rick_zero_planes(rick_plan_t* p, int n_planes);                      // grid.cu
 int rick_grid_planes(rick_plan_t* p, const void* vis, int vis_dtype, const double* uvw_m,
                      const float* weights, int plane_first, int n_planes);      // grid.cu
-int rick_fft_planes(rick_plan_t* p, int n_planes);                       // fft.cu
+int rick_fft_planes(rick_plan_t* p, int n_planes);                       // fft.cu: rows then columns
+int rick_fft_rows(rick_plan_t* p, int n_planes);                         // fft.cu
+int rick_fft_cols(rick_plan_t* p, int n_planes);                         // fft.cu (generic strided pass)
+int rick_cols12_init(rick_plan_t* p);                                    // fft_cols12.cu
+int rick_cols12_fft(rick_plan_t* p, int n_planes);                       // fft_cols12.cu
+int rick_cols12_wcorrect(rick_plan_t* p, int img, int z_first, int n_planes, double* image,
+                         int accumulate, int fuse_taper);                // fft_cols12.cu
 int rick_wcorrect(rick_plan_t* p, int img, int z_first, int n_planes, double* image,
                   int accumulate, int fuse_taper);                     // wcorrect.cu
 int rick_taper_divide(rick_plan_t* p, double* image);                    // wcorrect.cu

@@ -67,49 +67,58 @@ k_fft_cols(typename cplx_of<T>::type* __restrict__ stack,
 }
 
 template <typename T, int LOG2N>
-static int launch_fft(rick_plan_t* p, int n_planes)
+static int launch_fft(rick_plan_t* p, int n_planes, int which)   // which: 1 rows, 2 columns, 3 both
 {
     typedef typename cplx_of<T>::type C;
     typedef RowCfg<T, LOG2N> KR;
     typedef ColCfg<T, LOG2N> KC;
-    RICK_CUDA(p, cudaFuncSetAttribute(k_fft_rows<T, LOG2N>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      (int)KR::SMEM));
-    RICK_CUDA(p, cudaFuncSetAttribute(k_fft_cols<T, LOG2N>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      (int)KC::SMEM));
-    const unsigned int row_blocks = (unsigned int)((size_t)n_planes * KR::N / KR::RPC);
-    RICK_KERNEL(p, RK_FFT_ROWS, k_fft_rows<T, LOG2N><<<row_blocks, KR::THREADS, KR::SMEM, p->stream>>>((C*)p->stack, (const C*)p->twiddle));
-    const unsigned int col_blocks = (unsigned int)((size_t)n_planes * (KC::N / KC::WC));
-    RICK_KERNEL(p, RK_FFT_COLS, k_fft_cols<T, LOG2N><<<col_blocks, KC::THREADS, KC::SMEM, p->stream>>>((C*)p->stack, (const C*)p->twiddle));
+    if (which & 1) {
+        RICK_CUDA(p, cudaFuncSetAttribute(k_fft_rows<T, LOG2N>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                          (int)KR::SMEM));
+        const unsigned int row_blocks = (unsigned int)((size_t)n_planes * KR::N / KR::RPC);
+        RICK_KERNEL(p, RK_FFT_ROWS, k_fft_rows<T, LOG2N><<<row_blocks, KR::THREADS, KR::SMEM, p->stream>>>((C*)p->stack, (const C*)p->twiddle));
+    }
+    if (which & 2) {
+        if (!p->f32 && p->cols12_ok) return rick_cols12_fft(p, n_planes);
+        RICK_CUDA(p, cudaFuncSetAttribute(k_fft_cols<T, LOG2N>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                          (int)KC::SMEM));
+        const unsigned int col_blocks = (unsigned int)((size_t)n_planes * (KC::N / KC::WC));
+        RICK_KERNEL(p, RK_FFT_COLS, k_fft_cols<T, LOG2N><<<col_blocks, KC::THREADS, KC::SMEM, p->stream>>>((C*)p->stack, (const C*)p->twiddle));
+    }
     return RICK_OK;
 }
 
-int rick_fft_planes(rick_plan_t* p, int n_planes)
+static int fft_dispatch(rick_plan_t* p, int n_planes, int which)
 {
     if (n_planes <= 0) return RICK_OK;
     if (p->f32) {
         switch (p->log2N) {
-            case 6: return launch_fft<float, 6>(p, n_planes);
-            case 7: return launch_fft<float, 7>(p, n_planes);
-            case 8: return launch_fft<float, 8>(p, n_planes);
-            case 9: return launch_fft<float, 9>(p, n_planes);
-            case 10: return launch_fft<float, 10>(p, n_planes);
-            case 11: return launch_fft<float, 11>(p, n_planes);
-            case 12: return launch_fft<float, 12>(p, n_planes);
-            case 13: return launch_fft<float, 13>(p, n_planes);
-            case 14: return launch_fft<float, 14>(p, n_planes);
+            case 6: return launch_fft<float, 6>(p, n_planes, which);
+            case 7: return launch_fft<float, 7>(p, n_planes, which);
+            case 8: return launch_fft<float, 8>(p, n_planes, which);
+            case 9: return launch_fft<float, 9>(p, n_planes, which);
+            case 10: return launch_fft<float, 10>(p, n_planes, which);
+            case 11: return launch_fft<float, 11>(p, n_planes, which);
+            case 12: return launch_fft<float, 12>(p, n_planes, which);
+            case 13: return launch_fft<float, 13>(p, n_planes, which);
+            case 14: return launch_fft<float, 14>(p, n_planes, which);
         }
     } else {
         switch (p->log2N) {
-            case 6: return launch_fft<double, 6>(p, n_planes);
-            case 7: return launch_fft<double, 7>(p, n_planes);
-            case 8: return launch_fft<double, 8>(p, n_planes);
-            case 9: return launch_fft<double, 9>(p, n_planes);
-            case 10: return launch_fft<double, 10>(p, n_planes);
-            case 11: return launch_fft<double, 11>(p, n_planes);
-            case 12: return launch_fft<double, 12>(p, n_planes);
-            case 13: return launch_fft<double, 13>(p, n_planes);
+            case 6: return launch_fft<double, 6>(p, n_planes, which);
+            case 7: return launch_fft<double, 7>(p, n_planes, which);
+            case 8: return launch_fft<double, 8>(p, n_planes, which);
+            case 9: return launch_fft<double, 9>(p, n_planes, which);
+            case 10: return launch_fft<double, 10>(p, n_planes, which);
+            case 11: return launch_fft<double, 11>(p, n_planes, which);
+            case 12: return launch_fft<double, 12>(p, n_planes, which);
+            case 13: return launch_fft<double, 13>(p, n_planes, which);
         }
     }
     p->err = "grid edge not supported by the FFT at this precision";
     return RICK_ERR_INVALID;
 }
+
+int rick_fft_planes(rick_plan_t* p, int n_planes) { return fft_dispatch(p, n_planes, 3); }
+int rick_fft_rows(rick_plan_t* p, int n_planes) { return fft_dispatch(p, n_planes, 1); }
+int rick_fft_cols(rick_plan_t* p, int n_planes) { return fft_dispatch(p, n_planes, 2); }

@@ -1,0 +1,284 @@
+// fft_cols12.cu -- the column (v-axis) pass of a4 for the fp64 grid with N = 4096 = 16^3, and its
+// fusion with a5/a6 (PAPER.md:53, :68 FFT per w-plane; Eq. 2 :50 and :69 phase screen + plane sum;
+// reading R12 taper).
+//
+// Why a dedicated kernel.  A column of a 4096^2 complex128 plane is 64 KB, so one SM can hold a
+// strip of only two columns: the pass touches HBM in 32-byte pieces at a 64 KB stride.  Measured
+// on B200 (profiles/r1_colpass_probes.md): 32 B scattered reads run at ~4.7 TB/s through TMA but
+// only ~4 TB/s through LSU loads, 32 B scattered WRITES at ~2 TB/s; and the L1 tag stage pays one
+// cycle per 128 B line touched (16 lines per warp instruction).  Hence:
+//   * the strip is fetched by ONE TMA instruction per (strip, plane): a 5-D tensor map views the
+//     rows of a plane as digits row = w + 16 hh + 256 e and delivers the box in the order
+//     [e][w][hh][c] that the first radix-16 stage reads conflict-free.  The load of the next item is
+//     in flight while the current one is transformed (persistent CTA, one per SM, mbarrier).
+//   * k_cols12_wcorrect never writes the transformed plane: it keeps the CTA on one strip, walks
+//     the planes from the top down and sums them with Horner's rule in z,
+//         S <- P_z + step * S,   step = exp(2 pi i dw (n-1)),
+//     then I = Re(exp(2 pi i w_first (n-1)) S) [/ taper] once per strip.  Same mathematics as the
+//     geometric phase recurrence of wcorrect.cu, one complex FMA per pixel per plane, two sincospi
+//     per pixel per strip.
+//   * S and step (2 x 16 complex doubles per thread, 256 KB per SM) do not fit the register file
+//     next to the FFT; they live in TENSOR MEMORY, used here as a thread-private accumulator file
+//     (tcgen05.ld / tcgen05.st, shape 32x32b) -- the tensor cores themselves are not involved: no
+//     stage of this path is a dense contraction.
+// Shared memory: 128 KB TMA staging + 68 KB exchange buffer (real / imaginary halves in turn).
+#include "common.cuh"
+#include "fft_core.cuh"
+#include "sm100_ptx.cuh"
+
+namespace {
+
+constexpr int C12_LOG2N = 12, C12_N = 1 << C12_LOG2N, C12_NT = C12_N / 16, C12_WC = 2;
+constexpr int C12_THREADS = C12_NT * C12_WC, C12_STRIPS = C12_N / C12_WC;
+constexpr uint32_t C12_STAGE_BYTES = (uint32_t)C12_N * C12_WC * 16u;                        // 131072
+constexpr size_t C12_EX_BYTES = (size_t)C12_WC * (C12_N + C12_N / 16) * sizeof(double);     // 69632
+constexpr size_t C12_SMEM = C12_STAGE_BYTES + C12_EX_BYTES + 64;
+
+struct Roles {
+    int w, c, hh, t1, t2, t3;
+};
+__device__ __forceinline__ Roles roles()
+{
+    Roles r;
+    const int lane = threadIdx.x & 31;
+    r.w = threadIdx.x >> 5;
+    r.c = lane & 1;
+    r.hh = lane >> 1;
+    r.t1 = r.w + 16 * r.hh;      // stage 1: rows t1 + 256 e   (exchange 1 stays inside the warp)
+    r.t2 = 16 * r.w + r.hh;      // stage 2
+    r.t3 = r.t2;                 // stage 3: outputs X[t3 + 256 r]
+    return r;
+}
+
+// the 4096-point transform of the staged strip; on exit v[r] = X[t3 + 256 r] (uncentred index)
+__device__ __forceinline__ void strip_fft(double2 (&v)[16], const Roles& R, const double2* __restrict__ stg,
+                                          double* __restrict__ ex, const double2* __restrict__ tw,
+                                          unsigned long long* bar, uint32_t& parity, bool issue_next,
+                                          const CUtensorMap* tmap, int next_strip, int next_plane)
+{
+    mbar_wait(bar, parity);
+    parity ^= 1u;
+    // centring on input = rotation by N/2 = element e <- slot (e + 8) mod 16
+#pragma unroll
+    for (int e = 0; e < 16; ++e) v[e] = stg[(((e + 8) & 15) * 256 + R.w * 16 + R.hh) * 2 + R.c];
+    bfly16<double, C12_LOG2N, 0>(v, R.t1, tw);
+    __syncthreads();             // staging consumed by all; previous item's reads of `ex` are done
+    if (threadIdx.x == 0 && issue_next) {
+        mbar_arrive_expect_tx(bar, C12_STAGE_BYTES);
+        tma_load_5d(const_cast<double2*>(stg), tmap, bar, 4 * next_strip, 0, 0, 0, next_plane);
+    }
+    xchg16_warp(v, ex + (size_t)R.w * (16 * 17 * 2), R.hh, R.c);
+    bfly16<double, C12_LOG2N, 4>(v, R.t2, tw);
+    __syncthreads();             // every warp is done with its private region of `ex`
+    xchg16_cta(v, ex, R.t2, R.t3, R.c);
+    bfly16<double, C12_LOG2N, 8>(v, R.t3, tw);
+}
+
+// a4, column pass, in place (staged API).  Stores go straight from registers: 32 B pieces.
+__global__ void __launch_bounds__(C12_THREADS, 1)
+k_cols12_fft(const __grid_constant__ CUtensorMap tmap, double2* __restrict__ stack,
+             const double2* __restrict__ tw, int n_planes)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    double2* stg = reinterpret_cast<double2*>(smem_raw);
+    double* ex = reinterpret_cast<double*>(smem_raw + C12_STAGE_BYTES);
+    unsigned long long* bar = reinterpret_cast<unsigned long long*>(smem_raw + C12_STAGE_BYTES + C12_EX_BYTES);
+    const Roles R = roles();
+    if (threadIdx.x == 0) {
+        mbar_init(bar, 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    const int n_items = n_planes * C12_STRIPS;
+    int item = blockIdx.x;
+    if (threadIdx.x == 0 && item < n_items) {
+        mbar_arrive_expect_tx(bar, C12_STAGE_BYTES);
+        tma_load_5d(stg, &tmap, bar, 4 * (item % C12_STRIPS), 0, 0, 0, item / C12_STRIPS);
+    }
+    uint32_t parity = 0;
+    for (; item < n_items; item += gridDim.x) {
+        const int next = item + gridDim.x;
+        double2 v[16];
+        strip_fft(v, R, stg, ex, tw, bar, parity, next < n_items, &tmap, next % C12_STRIPS, next / C12_STRIPS);
+        const int plane = item / C12_STRIPS, strip = item - plane * C12_STRIPS;
+        double2* g = stack + (size_t)plane * C12_N * C12_N + (size_t)strip * C12_WC + R.c;
+#pragma unroll
+        for (int e = 0; e < 16; ++e) g[(size_t)(R.t3 + C12_NT * ((e + 8) & 15)) * C12_N] = v[e];
+    }
+}
+
+// a4 column pass fused with a5 (+ a6 when taper != nullptr).
+__global__ void __launch_bounds__(C12_THREADS, 1)
+k_cols12_wcorrect(const __grid_constant__ CUtensorMap tmap, const double2* __restrict__ tw, int n_planes,
+                  int z_first, double dl, const WRange* __restrict__ wr, double* __restrict__ image,
+                  int accumulate, const double* __restrict__ taper)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    double2* stg = reinterpret_cast<double2*>(smem_raw);
+    double* ex = reinterpret_cast<double*>(smem_raw + C12_STAGE_BYTES);
+    unsigned long long* bar = reinterpret_cast<unsigned long long*>(smem_raw + C12_STAGE_BYTES + C12_EX_BYTES);
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem_raw + C12_STAGE_BYTES + C12_EX_BYTES + 16);
+    const Roles R = roles();
+    if (threadIdx.x == 0) {
+        mbar_init(bar, 1);
+        mbar_fence_init();
+    }
+    if (R.w == 0) tmem_alloc_all(tmem_slot);
+    tmem_fence_before_sync();
+    __syncthreads();
+    tmem_fence_after_sync();
+    const uint32_t tbase = *tmem_slot;
+    // warps w, w+4, w+8, w+12 share the TMEM lanes 32 (w%4) ..; 128 columns each: S | step
+    const uint32_t tS = tbase + ((uint32_t)(32 * (R.w & 3)) << 16) + (uint32_t)((R.w >> 2) * 128);
+    const uint32_t tStep = tS + 64;
+
+    int strip = blockIdx.x;
+    if (threadIdx.x == 0 && strip < C12_STRIPS) {
+        mbar_arrive_expect_tx(bar, C12_STAGE_BYTES);
+        tma_load_5d(stg, &tmap, bar, 4 * strip, 0, 0, 0, n_planes - 1);
+    }
+    uint32_t parity = 0;
+    const double dw = wr->dw;
+    const double w_first = wr->w_min + ((double)z_first + 0.5) * dw;
+    for (; strip < C12_STRIPS; strip += gridDim.x) {
+        const int p = strip * C12_WC + R.c;
+        const double l = (double)(p - C12_N / 2) * dl;
+        // step = exp(2 pi i dw (n-1)) of this thread's 16 pixels (rows t3 + 256 ((e+8)&15)) -> TMEM
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            double2 st[4];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const int q = R.t3 + C12_NT * ((4 * k + i + 8) & 15);
+                const double m = (double)(q - C12_N / 2) * dl;
+                const double r2 = l * l + m * m;
+                double xs = 0.0;
+                if (r2 < 1.0) xs = dw * (-r2 / (1.0 + sqrt(1.0 - r2)));
+                xs -= rint(xs);
+                sincospi(2.0 * xs, &st[i].y, &st[i].x);
+            }
+            uint32_t r[16];
+            pack4(st, r);
+            tmem_st16(tStep + 16 * k, r);
+        }
+        tmem_wait_st();
+        for (int plane = n_planes - 1; plane >= 0; --plane) {
+            const bool more = plane > 0 || strip + (int)gridDim.x < C12_STRIPS;
+            double2 v[16];
+            strip_fft(v, R, stg, ex, tw, bar, parity, more, &tmap, plane > 0 ? strip : strip + (int)gridDim.x,
+                      plane > 0 ? plane - 1 : n_planes - 1);
+            // Horner in z: S <- P_z + step S
+            if (plane == n_planes - 1) {
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    const double2 s4[4] = {v[4 * k], v[4 * k + 1], v[4 * k + 2], v[4 * k + 3]};
+                    uint32_t r[16];
+                    pack4(s4, r);
+                    tmem_st16(tS + 16 * k, r);
+                }
+            } else {
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    uint32_t rs[16], rt[16];
+                    tmem_ld16(tS + 16 * k, rs);
+                    tmem_ld16(tStep + 16 * k, rt);
+                    tmem_wait_ld();
+                    double2 s4[4], st[4];
+                    unpack4(rs, s4);
+                    unpack4(rt, st);
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) {
+                        const double2 a = v[4 * k + i];
+                        double2 o;
+                        o.x = fma(st[i].x, s4[i].x, fma(-st[i].y, s4[i].y, a.x));
+                        o.y = fma(st[i].x, s4[i].y, fma(st[i].y, s4[i].x, a.y));
+                        s4[i] = o;
+                    }
+                    pack4(s4, rs);
+                    tmem_st16(tS + 16 * k, rs);
+                }
+            }
+            tmem_wait_st();
+        }
+        // I = Re(exp(2 pi i w_first (n-1)) S)  [+ previous batches]  [/ taper]
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            uint32_t rs[16];
+            tmem_ld16(tS + 16 * k, rs);
+            tmem_wait_ld();
+            double2 s4[4];
+            unpack4(rs, s4);
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const int q = R.t3 + C12_NT * ((4 * k + i + 8) & 15);
+                const double m = (double)(q - C12_N / 2) * dl;
+                const double r2 = l * l + m * m;
+                double val = 0.0;
+                if (r2 < 1.0) {
+                    double x0 = w_first * (-r2 / (1.0 + sqrt(1.0 - r2)));
+                    x0 -= rint(x0);
+                    double pr, pi;
+                    sincospi(2.0 * x0, &pi, &pr);
+                    val = pr * s4[i].x - pi * s4[i].y;
+                }
+                const size_t pix = (size_t)q * C12_N + p;
+                if (accumulate) val += image[pix];
+                if (taper) val /= (taper[p] * taper[q]);
+                image[pix] = val;
+            }
+        }
+    }
+    tmem_fence_before_sync();
+    __syncthreads();
+    if (R.w == 0) tmem_dealloc_all(tbase);
+}
+
+}   // namespace
+
+// Build the 5-D tensor map over the plan's resident stack (once, at plan creation).
+int rick_cols12_init(rick_plan_t* p)
+{
+    p->cols12_ok = 0;
+    if (p->f32 || p->N != C12_N) return RICK_OK;
+    rick_encode_tiled_fn enc = rick_get_encode_tiled();
+    if (!enc) {
+        p->err = "cuTensorMapEncodeTiled is not available from this driver";
+        return RICK_ERR_CUDA;
+    }
+    static_assert(sizeof(CUtensorMap) <= sizeof(p->cols12_tmap), "tensor map storage");
+    const cuuint64_t rowB = (cuuint64_t)C12_N * 16;
+    // dims: (re/im/column pair as doubles, hh, w, e, plane) with row = w + 16 hh + 256 e
+    const cuuint64_t dims[5] = {(cuuint64_t)2 * C12_N, 16, 16, 16, (cuuint64_t)p->batch};
+    const cuuint64_t strides[4] = {16 * rowB, rowB, 256 * rowB, (cuuint64_t)C12_N * rowB};
+    const cuuint32_t box[5] = {4, 16, 16, 16, 1};
+    const cuuint32_t es[5] = {1, 1, 1, 1, 1};
+    const CUresult r = enc(reinterpret_cast<CUtensorMap*>(p->cols12_tmap), CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 5, p->stack,
+                           dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                           CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        p->err = "cuTensorMapEncodeTiled failed";
+        return RICK_ERR_CUDA;
+    }
+    RICK_CUDA(p, cudaFuncSetAttribute(k_cols12_fft, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C12_SMEM));
+    RICK_CUDA(p, cudaFuncSetAttribute(k_cols12_wcorrect, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C12_SMEM));
+    p->cols12_ok = 1;
+    return RICK_OK;
+}
+
+int rick_cols12_fft(rick_plan_t* p, int n_planes)
+{
+    const CUtensorMap tm = *reinterpret_cast<const CUtensorMap*>(p->cols12_tmap);
+    RICK_KERNEL(p, RK_FFT_COLS, k_cols12_fft<<<p->n_sm, C12_THREADS, C12_SMEM, p->stream>>>(
+        tm, (double2*)p->stack, (const double2*)p->twiddle, n_planes));
+    return RICK_OK;
+}
+
+int rick_cols12_wcorrect(rick_plan_t* p, int img, int z_first, int n_planes, double* image, int accumulate,
+                         int fuse_taper)
+{
+    const CUtensorMap tm = *reinterpret_cast<const CUtensorMap*>(p->cols12_tmap);
+    RICK_KERNEL(p, RK_COLS_WCORRECT, k_cols12_wcorrect<<<p->n_sm, C12_THREADS, C12_SMEM, p->stream>>>(
+        tm, (const double2*)p->twiddle, n_planes, z_first, p->dl, p->wrange + img, image, accumulate,
+        fuse_taper ? p->taper : nullptr));
+    return RICK_OK;
+}

@@ -212,3 +212,96 @@ __device__ __forceinline__ void fft_thread(typename cplx_of<T>::type (&v)[16], c
         }
     }
 }
+
+// ------------------------------------------------------------------------------------------
+// Building blocks of the N = 4096 = 16^3 column kernels (fft_cols12.cu): one radix-16 stage on
+// the 16 registers of a thread, and the two inter-stage exchanges through a DOUBLE buffer
+// (real parts, then imaginary parts: half the shared memory of a complex exchange).
+// ------------------------------------------------------------------------------------------
+
+// twiddle (NS = 2^LOG2NS butterflies already combined) + radix-16 butterfly over v[e] = x[t + (N/16) e];
+// on exit v[r] = leg r in natural order.
+template <typename T, int LOG2N, int LOG2NS>
+__device__ __forceinline__ void bfly16(typename cplx_of<T>::type (&v)[16], const int t,
+                                       const typename cplx_of<T>::type* __restrict__ tw)
+{
+    typedef typename cplx_of<T>::type C;
+    constexpr int N = 1 << LOG2N, NS = 1 << LOG2NS;
+    if constexpr (LOG2NS > 0) {
+        const int jm = t & (NS - 1);
+        const C w1 = tw[jm * (N / (NS * 16))];
+        v[1] = cmul(v[1], w1);
+        const C w2 = cmul(w1, w1);
+        const C w3 = cmul(w2, w1);
+        v[2] = cmul(v[2], w2);
+        v[3] = cmul(v[3], w3);
+        const C w4 = cmul(w2, w2);
+        v[4] = cmul(v[4], w4);
+        v[5] = cmul(v[5], cmul(w4, w1));
+        v[6] = cmul(v[6], cmul(w4, w2));
+        const C w7 = cmul(w4, w3);
+        v[7] = cmul(v[7], w7);
+        const C w8 = cmul(w4, w4);
+        v[8] = cmul(v[8], w8);
+        v[9] = cmul(v[9], cmul(w8, w1));
+        v[10] = cmul(v[10], cmul(w8, w2));
+        v[11] = cmul(v[11], cmul(w8, w3));
+        const C w12 = cmul(w8, w4);
+        v[12] = cmul(v[12], w12);
+        v[13] = cmul(v[13], cmul(w12, w1));
+        v[14] = cmul(v[14], cmul(w12, w2));
+        v[15] = cmul(v[15], cmul(w8, w7));
+    }
+    fft16<T>(v);
+    C o[16];
+#pragma unroll
+    for (int r = 0; r < 16; ++r) o[r] = v[leg_reg<16>(r)];
+#pragma unroll
+    for (int r = 0; r < 16; ++r) v[r] = o[r];
+}
+
+// Exchange after stage 1 when a warp holds the roles t1 = w + 16 hh (hh = 0..15, two columns c
+// interleaved): the Stockham permutation closes inside the warp -- a 16 x 16 transpose per column,
+// writer hh leg r -> reader hh' = r element e = hh.  wb: this warp's 16*17*2 doubles.  No CTA barrier.
+__device__ __forceinline__ void xchg16_warp(double2 (&v)[16], double* __restrict__ wb, const int hh, const int c)
+{
+#pragma unroll
+    for (int r = 0; r < 16; ++r) wb[(hh * 17 + r) * 2 + c] = v[r].x;
+    __syncwarp();
+    double re[16];
+#pragma unroll
+    for (int e = 0; e < 16; ++e) re[e] = wb[(e * 17 + hh) * 2 + c];
+    __syncwarp();
+#pragma unroll
+    for (int r = 0; r < 16; ++r) wb[(hh * 17 + r) * 2 + c] = v[r].y;
+    __syncwarp();
+#pragma unroll
+    for (int e = 0; e < 16; ++e) {
+        v[e].y = wb[(e * 17 + hh) * 2 + c];
+        v[e].x = re[e];
+    }
+    __syncwarp();
+}
+
+// Exchange after stage 2 (NS = 16), CTA-wide: writer role t2 leg r -> position pos0 + 16 r;
+// reader role t3 element e <- position t3 + 256 e.  sm: 2 * (4096 + 256) doubles.
+__device__ __forceinline__ void xchg16_cta(double2 (&v)[16], double* __restrict__ sm, const int t2, const int t3,
+                                           const int c)
+{
+    const int pos0 = ((t2 >> 4) << 8) + (t2 & 15);
+#pragma unroll
+    for (int r = 0; r < 16; ++r) sm[fft_pad(pos0 + r * 16) * 2 + c] = v[r].x;
+    __syncthreads();
+    double re[16];
+#pragma unroll
+    for (int e = 0; e < 16; ++e) re[e] = sm[fft_pad(t3 + 256 * e) * 2 + c];
+    __syncthreads();
+#pragma unroll
+    for (int r = 0; r < 16; ++r) sm[fft_pad(pos0 + r * 16) * 2 + c] = v[r].y;
+    __syncthreads();
+#pragma unroll
+    for (int e = 0; e < 16; ++e) {
+        v[e].y = sm[fft_pad(t3 + 256 * e) * 2 + c];
+        v[e].x = re[e];
+    }
+}

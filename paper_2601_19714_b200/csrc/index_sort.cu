@@ -96,14 +96,17 @@ k_index_key(const double* __restrict__ uvw, const float* __restrict__ wgt,
             unsigned int M, unsigned int C, int N, int Nw, int h, int B, int T, int cube,
             double inv_du, uint32_t* __restrict__ keys, DevCounters* cnt)
 {
-    const unsigned int k = blockIdx.x * blockDim.x + threadIdx.x;
+    // grid-stride: statistics stay in registers, one set of atomics per block (same-address
+    // atomics per warp made this kernel atomic-bound)
     unsigned int on = 0, off = 0;
     double sw = 0.0;
-    if (k < M) {
+    const double shift = (double)(N / 2) + 0.5;
+    for (unsigned long long kk0 = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; kk0 < M;
+         kk0 += (unsigned long long)gridDim.x * blockDim.x) {
+        const unsigned int k = (unsigned int)kk0;
         const unsigned int r = k / C, c = k - r * C;
         const double s = chan_scale[c];
         const double um = uvw[3ull * r + 0], vm = uvw[3ull * r + 1], wm = uvw[3ull * r + 2];
-        const double shift = (double)(N / 2) + 0.5;
         const double xu = __dmul_rn(__dmul_rn(um, s), inv_du);
         const double xv = __dmul_rn(__dmul_rn(vm, s), inv_du);
         const int iu = (int)floor(__dadd_rn(xu, shift));
@@ -119,22 +122,40 @@ k_index_key(const double* __restrict__ uvw, const float* __restrict__ wgt,
             unsigned long long kk = (unsigned long long)img * (unsigned)Nw + (unsigned)ip;
             kk = (kk * (unsigned)T + (unsigned)(iv / B)) * (unsigned)T + (unsigned)(iu / B);
             key = (uint32_t)kk;
-            on = 1;
-            sw = wgt ? (double)wgt[k] : 1.0;
+            on++;
+            sw += wgt ? (double)wgt[k] : 1.0;
         } else {
-            off = 1;
+            off++;
         }
         keys[k] = key;
     }
-    // warp-reduced statistics
-    const unsigned int b_on = __ballot_sync(0xffffffffu, on), b_off = __ballot_sync(0xffffffffu, off);
-    for (int o = 16; o > 0; o >>= 1) sw += __shfl_xor_sync(0xffffffffu, sw, o);
+    // block-reduced statistics
+    __shared__ unsigned int s_on[8], s_off[8];
+    __shared__ double s_sw[8];
+    for (int o = 16; o > 0; o >>= 1) {
+        on += __shfl_xor_sync(0xffffffffu, on, o);
+        off += __shfl_xor_sync(0xffffffffu, off, o);
+        sw += __shfl_xor_sync(0xffffffffu, sw, o);
+    }
     if ((threadIdx.x & 31) == 0) {
-        if (b_on) {
-            atomicAdd(&cnt->n_gridded, (unsigned long long)__popc(b_on));
-            atomicAdd(&cnt->sum_w, sw);
+        s_on[threadIdx.x >> 5] = on;
+        s_off[threadIdx.x >> 5] = off;
+        s_sw[threadIdx.x >> 5] = sw;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        unsigned long long t_on = 0, t_off = 0;
+        double t_sw = 0.0;
+        for (int w = 0; w < (int)(blockDim.x >> 5); ++w) {
+            t_on += s_on[w];
+            t_off += s_off[w];
+            t_sw += s_sw[w];
         }
-        if (b_off) atomicAdd(&cnt->n_dropped, (unsigned long long)__popc(b_off));
+        if (t_on) {
+            atomicAdd(&cnt->n_gridded, t_on);
+            atomicAdd(&cnt->sum_w, t_sw);
+        }
+        if (t_off) atomicAdd(&cnt->n_dropped, t_off);
     }
 }
 
@@ -342,9 +363,13 @@ int rick_index_sort(rick_plan_t* p, const double* uvw_m, const float* weights)
     p->sorted_keys = p->keys;
     p->sorted_perm = p->perm_a;
     if (M > 0) {
-        RICK_KERNEL(p, RK_INDEX_KEY, k_index_key<<<(M + 255) / 256, 256, 0, st>>>(uvw_m, weights, p->chan_scale, p->wrange, M,
+        {
+            unsigned int nb = (M + 255) / 256;
+            if (nb > (unsigned)p->n_sm * 8u) nb = (unsigned)p->n_sm * 8u;
+            RICK_KERNEL(p, RK_INDEX_KEY, k_index_key<<<nb, 256, 0, st>>>(uvw_m, weights, p->chan_scale, p->wrange, M,
                                                     (unsigned)p->C, p->N, p->Nw, p->h, p->B, p->T,
                                                     p->d.cube, p->inv_du, p->keys, p->counters));
+        }
 
         // key bits: the all-ones pattern of the sorted bit range is reserved for the sentinel
         const unsigned long long nkeys = (unsigned long long)n_planes_total * p->T * p->T;

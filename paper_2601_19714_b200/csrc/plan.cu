@@ -18,7 +18,7 @@ static void free_dev(void* q)
 // per-kernel CUDA-event timing
 static const char* const k_names[RK_NKERNELS] = {
     "tables", "reset", "wrange", "index_key", "radix_hist", "scan", "radix_scatter", "plane_starts",
-    "zero", "grid", "fft_rows", "fft_cols", "wcorrect", "taper"};
+    "zero", "grid", "fft_rows", "fft_cols", "wcorrect", "taper", "fft_cols_wcorrect"};
 
 void rick_prof_begin(rick_plan_t* p, int id)
 {
@@ -111,7 +111,9 @@ static int plan_init(rick_plan_t* p)
     RICK_CUDA(p, cudaEventCreateWithFlags(&p->ev_scale, cudaEventDisableTiming));
     RICK_CUDA(p, cudaMalloc(&p->counters, sizeof(DevCounters)));
     RICK_CUDA(p, cudaMemsetAsync(p->counters, 0, sizeof(DevCounters), p->stream));
-    return rick_tables_build(p);
+    const int rc = rick_tables_build(p);
+    if (rc) return rc;
+    return rick_cols12_init(p);
 }
 
 extern "C" int rick_plan(rick_plan_t** out, const rick_plan_desc* d, void* cuda_stream)
@@ -306,8 +308,13 @@ extern "C" int rick_image(rick_plan_t* p, const void* vis, int32_t vis_dtype, co
             const int last = z0 + nb >= p->Nw;
             if ((rc = rick_zero_planes(p, nb))) return rc;
             if ((rc = rick_grid_planes(p, vis, vis_dtype, uvw_m, weights, img * p->Nw + z0, nb))) return rc;
-            if ((rc = rick_fft_planes(p, nb))) return rc;
-            if ((rc = rick_wcorrect(p, img, z0, nb, dst, z0 > 0, last))) return rc;
+            if (p->cols12_ok) {   // column pass fused with the w-correction: the transformed planes are never written
+                if ((rc = rick_fft_rows(p, nb))) return rc;
+                if ((rc = rick_cols12_wcorrect(p, img, z0, nb, dst, z0 > 0, last))) return rc;
+            } else {
+                if ((rc = rick_fft_planes(p, nb))) return rc;
+                if ((rc = rick_wcorrect(p, img, z0, nb, dst, z0 > 0, last))) return rc;
+            }
         }
     }
     if (!p->d.cube) {

@@ -114,6 +114,31 @@ def test_cfg3_midsize_lofar_shape():
     assert o["stats"]["n_dropped"] > 0
 
 
+def test_n4096_tma_tmem_column_kernels():
+    # N = 4096 fp64 takes the dedicated column kernels (fft_cols12.cu): TMA-fed in-place pass in the
+    # staged API, column pass fused with the w-correction (Horner over planes in TMEM) in rick_image.
+    wl = synth.make_config(2, n_times=4, n_wplanes=5, n_src=8)
+    assert wl.n == 4096
+    g, o = _check_staged(wl, TOL64)
+    rick = _rick()
+    vis, uvw, wgt = rick.to_device(wl)
+    for pb in (0, 2):                      # all planes resident; ragged batches 2+2+1 (accumulate path)
+        plan = rick.plan_from_workload(wl, plane_batch=pb)
+        img = plan.rick_image(vis, uvw, wgt, wl.freq_hz).cpu().numpy()
+        img2 = plan.rick_image(vis, uvw, wgt, wl.freq_hz).cpu().numpy()      # TMEM re-allocation on reuse
+        plan.destroy()
+        e = _rel(img, o["image"])
+        print(f"N=4096 fused rick_image plane_batch={pb}: rel L2 {e:.2e}")
+        assert e <= TOL64 and _rel(img2, o["image"]) <= TOL64
+    # one plane only (Horner degenerates to S = P_0)
+    wl1 = synth.make_config(2, n_times=2, n_wplanes=1, n_src=4)
+    plan = rick.plan_from_workload(wl1)
+    v1, u1, w1 = rick.to_device(wl1)
+    img = plan.rick_image(v1, u1, w1, wl1.freq_hz).cpu().numpy()
+    plan.destroy()
+    assert _rel(img, _oracle(wl1)["image"]) <= TOL64
+
+
 def test_support_and_beta_variants():
     wl = synth.make_config(1, n_times=8)
     rick = _rick()
