@@ -11,7 +11,7 @@
 #define RICK_C0 299792458.0
 #define RICK_MAX_CHAN 4096
 #define RICK_KEY_DROPPED 0xFFFFFFFFu
-#define RICK_MAX_KB_TERMS 96
+#define RICK_KB_DEG 18          // degree of the per-tap polynomial of the Kaiser-Bessel kernel
 
 // Per-image w-plane geometry, computed on the device by k_wrange_finish (a0).
 struct WRange {
@@ -44,8 +44,7 @@ struct rick_plan_s {
     // tables
     void* twiddle;           // [N] complex of grid_prec: e^{+2 pi i k/N}
     double* taper;           // [N] c((p-N/2)/N)
-    double* kb_coef;         // [kb_terms] series coefficients of g in y = 1-(2t/S)^2
-    int kb_terms;
+    double kb_poly[15 * (RICK_KB_DEG + 1)];   // host: [S][DEG+1], tap a on d = (a-h) - s/2, s in [-1,1]
 
     // resident buffers
     void* stack;             // [batch][N][N] complex of grid_prec

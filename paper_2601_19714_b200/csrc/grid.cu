@@ -9,14 +9,21 @@
 // balance in visibilities, whatever the skew of the uv coverage) and owns a PRIVATE
 // shared-memory accumulation tile of (B+S-1)^2 cells -- the tile plus the kernel halo, the
 // single-GPU analogue of the paper's ghost region.  Per batch of 32 visibilities every lane
-// evaluates the 2S kernel values of its own visibility (Horner on the I0 power series in
-// y = 1-(2t/S)^2, all lanes busy), stages them in shared memory, then the warp walks the 32
-// visibilities one by one with its lanes spread over the S*S footprint cells: plain
-// read-modify-write, no shared-memory atomics (cells of one footprint are distinct, and
-// successive visibilities are ordered by __syncwarp).  When the tile key changes, the tile is
-// flushed to HBM with fire-and-forget RED atomics (non-zero cells only) and re-zeroed.
-// The tile row pitch is padded so that pitch == S (mod 8 | 16): consecutive lanes then hit
-// consecutive 16-byte (8-byte) bank groups -> conflict-free.
+// evaluates the 2S kernel values of its own visibility, stages them in shared memory, then the
+// warp walks the 32 visibilities one by one with its lanes spread over the footprint, each lane
+// owning two horizontally adjacent cells: plain read-modify-write, no shared-memory atomics
+// (cells of one footprint are distinct, and successive visibilities are ordered by __syncwarp).
+// When the tile key changes, the tile is flushed to HBM with fire-and-forget RED atomics
+// (non-zero cells only) and re-zeroed.
+//
+// Kernel values.  d_a = (a-h) - delta with delta = x_u - (i_u - N/2) in [-1/2, 1/2): tap a sees g
+// only on one unit interval, where it is a degree-KB_DEG polynomial in s = 2 delta to < 2e-16
+// (tables.cu fits and checks it at plan time).  The coefficients travel as kernel parameters, so
+// every Horner step is one DFMA with a constant-bank operand: 2 S (KB_DEG+1) DFMA per visibility
+// and no load -- against ~45 terms of the I0 power series per tap before.
+//
+// The tile row pitch is odd (and > B+S-1, the pad column takes the zero-weight partner of the last
+// cell of a footprint row), so the lanes of a quarter warp hit distinct 16-byte bank groups.
 #include "common.cuh"
 
 struct GridParams {
@@ -29,22 +36,23 @@ struct GridParams {
     const long long* plane_start;
     int plane_first, n_planes;
     void* stack;
-    const double* kb_coef;
-    int kb_terms;
     int N, h, B, T, TWp, TH, C;
     int vis_c128;
     double inv_du;
     unsigned int* chunk_counter;
 };
+template <int S> struct GridParamsS {
+    GridParams g;
+    double poly[S][RICK_KB_DEG + 1];     // poly[a][k]: coefficient of s^k of tap a
+};
 
 #define GRID_WARPS 8
-#define GRID_CHUNK 128
+#define GRID_CHUNK 512
 
-__host__ __device__ inline int grid_pitch(int B, int S, int elem_bytes)
+__host__ __device__ inline int grid_pitch(int B, int S)
 {
-    const int m = elem_bytes == 16 ? 8 : 16;
-    int tw = B + S - 1;
-    while ((tw % m) != (S % m)) ++tw;
+    int tw = B + S;                      // one pad column
+    if ((tw & 1) == 0) ++tw;
     return tw;
 }
 
@@ -62,41 +70,44 @@ __device__ __forceinline__ void red_add(float2* a, float2 v) { atomicAdd(a, v); 
 __global__ void k_chunk_reset(unsigned int* c) { *c = 0u; }
 
 template <typename GT, int S>
-__global__ void __launch_bounds__(GRID_WARPS * 32) k_grid(const GridParams P)
+__global__ void __launch_bounds__(GRID_WARPS * 32) k_grid(const __grid_constant__ GridParamsS<S> PS)
 {
     typedef typename cell_t<GT>::type cell;
-    constexpr int ROUNDS = (S * S + 31) / 32;
+    constexpr int PW = (S + 1) / 2;                 // cell pairs per footprint row
+    constexpr int SP = 2 * PW;                      // padded footprint width (even)
+    constexpr int NPAIR = S * PW, ROUNDS = (NPAIR + 31) / 32;
+    constexpr int DEG = RICK_KB_DEG;
+    const GridParams& P = PS.g;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int TWp = P.TWp, TH = P.TH, N = P.N, h = P.h, B = P.B, T = P.T;
     const int tile_cells = TH * TWp;
 
-    // shared layout: [coef RICK_MAX_KB_TERMS dbl][per warp: tile | ku[32][S] | kv[32][S] | vr[32] | vi[32] | base[32]]
-    double* s_coef = reinterpret_cast<double*>(smem_raw);
-    const size_t per_warp = (size_t)tile_cells * sizeof(cell) + (size_t)(2 * 32 * S + 64) * sizeof(double) +
-                            32 * sizeof(int);
-    unsigned char* wbase = smem_raw + RICK_MAX_KB_TERMS * sizeof(double) + (size_t)warp * per_warp;
+    // shared layout per warp: tile | ku[32][SP] | kv[32][SP] | vr[32] | vi[32] | base[32]
+    const size_t tile_bytes = ((size_t)tile_cells * sizeof(cell) + 15) & ~(size_t)15;
+    const size_t per_warp = tile_bytes + (size_t)(2 * 32 * SP + 64) * sizeof(double) + 32 * sizeof(int);
+    unsigned char* wbase = smem_raw + (size_t)warp * per_warp;
     cell* tile = reinterpret_cast<cell*>(wbase);
-    double* s_ku = reinterpret_cast<double*>(wbase + (size_t)tile_cells * sizeof(cell));
-    double* s_kv = s_ku + 32 * S;
-    double* s_vr = s_kv + 32 * S;
+    double* s_ku = reinterpret_cast<double*>(wbase + tile_bytes);
+    double* s_kv = s_ku + 32 * SP;
+    double* s_vr = s_kv + 32 * SP;
     double* s_vi = s_vr + 32;
     int* s_base = reinterpret_cast<int*>(s_vi + 32);
 
-    for (int i = threadIdx.x; i < P.kb_terms; i += blockDim.x) s_coef[i] = P.kb_coef[i];
     cell zero;
     zero.x = 0;
     zero.y = 0;
     for (int i = lane; i < tile_cells; i += 32) tile[i] = zero;
-    __syncthreads();
+    for (int i = lane; i < 2 * 32 * SP; i += 32) s_ku[i] = 0.0;      // also the zero weight of the pad column
+    __syncwarp();
 
-    // footprint cell(s) of this lane: cell = lane + 32*rr -> (b, a)
-    int fa[ROUNDS], fb[ROUNDS], foff[ROUNDS];
+    // cell pair(s) of this lane: pair = lane + 32*rr -> row b, cells (b, 2 a2), (b, 2 a2 + 1)
+    int fb[ROUNDS], fa[ROUNDS], foff[ROUNDS];
 #pragma unroll
     for (int rr = 0; rr < ROUNDS; ++rr) {
-        const int c = lane + 32 * rr;
-        fb[rr] = c / S;
-        fa[rr] = c - fb[rr] * S;
+        const int pi = lane + 32 * rr;
+        fb[rr] = pi / PW;
+        fa[rr] = 2 * (pi - fb[rr] * PW);
         foff[rr] = fb[rr] * TWp + fa[rr];
     }
 
@@ -105,8 +116,6 @@ __global__ void __launch_bounds__(GRID_WARPS * 32) k_grid(const GridParams P)
     const long long n_chunks = (v_end - v_begin + GRID_CHUNK - 1) / GRID_CHUNK;
     const unsigned int TT = (unsigned)T * (unsigned)T;
     const double shift = (double)(N / 2) + 0.5;
-    const int K = P.kb_terms;
-    const double two_over_S = 2.0 / (double)S;
 
     uint32_t cur_key = RICK_KEY_DROPPED;
 
@@ -167,30 +176,27 @@ __global__ void __launch_bounds__(GRID_WARPS * 32) k_grid(const GridParams P)
                 s_vi[lane] = vi;
                 // top-left footprint cell, local to the tile: (i_u - h) - (tu*B - h) = i_u mod B
                 s_base[lane] = (iv - (iv / B) * B) * TWp + (iu - (iu / B) * B);
-                // kernel values: S independent Horner chains per axis
-                double yu[S], yv[S], au[S], av[S];
+                // kernel values: tap a at d_a = (a-h) - s/2, s = 2 (x - (i - N/2)); 2S Horner chains
+                const double su = 2.0 * (xu - (double)(iu - N / 2));
+                const double sv = 2.0 * (xv - (double)(iv - N / 2));
+                double au[S], av[S];
 #pragma unroll
                 for (int a = 0; a < S; ++a) {
-                    const double du = (double)(iu - N / 2 + a - h) - xu;
-                    const double dv = (double)(iv - N / 2 + a - h) - xv;
-                    const double ru = du * two_over_S, rv = dv * two_over_S;
-                    yu[a] = fmax(0.0, 1.0 - ru * ru);
-                    yv[a] = fmax(0.0, 1.0 - rv * rv);
-                    au[a] = s_coef[K - 1];
-                    av[a] = au[a];
+                    au[a] = PS.poly[a][DEG];
+                    av[a] = PS.poly[a][DEG];
                 }
-                for (int k = K - 2; k >= 0; --k) {
-                    const double ck = s_coef[k];
+#pragma unroll
+                for (int k = DEG - 1; k >= 0; --k) {
 #pragma unroll
                     for (int a = 0; a < S; ++a) {
-                        au[a] = fma(au[a], yu[a], ck);
-                        av[a] = fma(av[a], yv[a], ck);
+                        au[a] = fma(au[a], su, PS.poly[a][k]);
+                        av[a] = fma(av[a], sv, PS.poly[a][k]);
                     }
                 }
 #pragma unroll
                 for (int a = 0; a < S; ++a) {
-                    s_ku[lane * S + a] = au[a];
-                    s_kv[lane * S + a] = av[a];
+                    s_ku[lane * SP + a] = au[a];
+                    s_kv[lane * SP + a] = av[a];
                 }
             }
             __syncwarp();
@@ -205,12 +211,18 @@ __global__ void __launch_bounds__(GRID_WARPS * 32) k_grid(const GridParams P)
                 const double vr = s_vr[j], vi = s_vi[j];
 #pragma unroll
                 for (int rr = 0; rr < ROUNDS; ++rr) {
-                    if (lane + 32 * rr < S * S) {
-                        const double kk = s_ku[j * S + fa[rr]] * s_kv[j * S + fb[rr]];
-                        cell t = tile[base + foff[rr]];
-                        t.x += (GT)(vr * kk);
-                        t.y += (GT)(vi * kk);
-                        tile[base + foff[rr]] = t;
+                    if (lane + 32 * rr < NPAIR) {
+                        const double2 k2 = *reinterpret_cast<const double2*>(&s_ku[j * SP + fa[rr]]);
+                        const double kvb = s_kv[j * SP + fb[rr]];
+                        const double wr = vr * kvb, wi = vi * kvb;
+                        cell* tp = tile + base + foff[rr];
+                        cell t0 = tp[0], t1 = tp[1];
+                        t0.x += (GT)(wr * k2.x);
+                        t0.y += (GT)(wi * k2.x);
+                        t1.x += (GT)(wr * k2.y);
+                        t1.y += (GT)(wi * k2.y);
+                        tp[0] = t0;
+                        tp[1] = t1;
                     }
                 }
                 __syncwarp();
@@ -241,9 +253,14 @@ template <typename GT, int S>
 static int launch_grid(rick_plan_t* p, const GridParams& P)
 {
     typedef typename cell_t<GT>::type cell;
-    const size_t per_warp = (size_t)P.TH * P.TWp * sizeof(cell) + (size_t)(2 * 32 * S + 64) * sizeof(double) +
-                            32 * sizeof(int);
-    const size_t smem = RICK_MAX_KB_TERMS * sizeof(double) + GRID_WARPS * per_warp;
+    constexpr int SP = 2 * ((S + 1) / 2);
+    GridParamsS<S> PS;
+    PS.g = P;
+    for (int a = 0; a < S; ++a)
+        for (int k = 0; k <= RICK_KB_DEG; ++k) PS.poly[a][k] = p->kb_poly[a * (RICK_KB_DEG + 1) + k];
+    const size_t tile_bytes = ((size_t)P.TH * P.TWp * sizeof(cell) + 15) & ~(size_t)15;
+    const size_t per_warp = tile_bytes + (size_t)(2 * 32 * SP + 64) * sizeof(double) + 32 * sizeof(int);
+    const size_t smem = GRID_WARPS * per_warp;
     if (smem > 227 * 1024) {
         p->err = "tile/support too large for the gridder's shared memory";
         return RICK_ERR_INVALID;
@@ -253,7 +270,7 @@ static int launch_grid(rick_plan_t* p, const GridParams& P)
     RICK_CUDA(p, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_grid<GT, S>, GRID_WARPS * 32, smem));
     if (per_sm < 1) per_sm = 1;
     RICK_KERNEL(p, RK_RESET, k_chunk_reset<<<1, 1, 0, p->stream>>>(P.chunk_counter));
-    RICK_KERNEL(p, RK_GRID, k_grid<GT, S><<<p->n_sm * per_sm, GRID_WARPS * 32, smem, p->stream>>>(P));
+    RICK_KERNEL(p, RK_GRID, k_grid<GT, S><<<p->n_sm * per_sm, GRID_WARPS * 32, smem, p->stream>>>(PS));
     return RICK_OK;
 }
 
@@ -287,14 +304,12 @@ int rick_grid_planes(rick_plan_t* p, const void* vis, int vis_dtype, const doubl
     P.plane_first = plane_first;
     P.n_planes = n_planes;
     P.stack = p->stack;
-    P.kb_coef = p->kb_coef;
-    P.kb_terms = p->kb_terms;
     P.N = p->N;
     P.h = p->h;
     P.B = p->B;
     P.T = p->T;
     P.TH = p->B + p->S - 1;
-    P.TWp = grid_pitch(p->B, p->S, p->f32 ? 8 : 16);
+    P.TWp = grid_pitch(p->B, p->S);
     P.C = p->C;
     P.vis_c128 = vis_dtype == RICK_VIS_C128;
     P.inv_du = p->inv_du;

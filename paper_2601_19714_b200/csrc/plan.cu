@@ -86,7 +86,7 @@ extern "C" int rick_plan_destroy(rick_plan_t* p)
 {
     if (!p) return RICK_OK;
     cudaStreamSynchronize(p->stream);
-    free_dev(p->twiddle); free_dev(p->taper); free_dev(p->kb_coef); free_dev(p->stack); free_dev(p->image);
+    free_dev(p->twiddle); free_dev(p->taper); free_dev(p->stack); free_dev(p->image);
     free_dev(p->keys); free_dev(p->keys_a); free_dev(p->keys_b); free_dev(p->perm_a); free_dev(p->perm_b);
     free_dev(p->hist); free_dev(p->scan_tmp); free_dev(p->plane_start); free_dev(p->chan_scale);
     free_dev(p->wrange); free_dev(p->counters);
