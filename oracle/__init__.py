@@ -23,6 +23,7 @@ _lib = None
 _f64p = np.ctypeslib.ndpointer(dtype=np.float64, flags="C_CONTIGUOUS")
 _i32p = np.ctypeslib.ndpointer(dtype=np.int32, flags="C_CONTIGUOUS")
 _u32p = np.ctypeslib.ndpointer(dtype=np.uint32, flags="C_CONTIGUOUS")
+_u64p = np.ctypeslib.ndpointer(dtype=np.uint64, flags="C_CONTIGUOUS")
 _i64p = np.ctypeslib.ndpointer(dtype=np.int64, flags="C_CONTIGUOUS")
 
 
@@ -48,7 +49,7 @@ def lib():
         L.rko_taper.argtypes = [C.c_double, C.c_int, C.c_double]
         L.rko_num_threads.restype = C.c_int
         L.rko_fft2_centered.argtypes = [_f64p, C.c_int32]
-        L.rko_sort.argtypes = [C.c_int64, _u32p, _u32p]
+        L.rko_sort.argtypes = [C.c_int64, _u64p, _u32p]
         L.rko_wcorrect_accumulate.argtypes = [_f64p, C.c_int32, C.c_double, C.c_double, _f64p]
         L.rko_gridcorrect.argtypes = [_f64p, C.c_int32, C.c_int32, C.c_double]
         _lib = L
@@ -81,26 +82,27 @@ def _ptr(a, ctype):
 
 
 def index(uvw_m, freq_hz, N, Nw, S, dl, B, cube=0, w_min=float("nan"), w_max=float("nan")):
-    """Steps 1-4.  Returns dict(iu, iv, ip, key, xu, xv, w_min[n_img], w_max[n_img])."""
+    """Steps 1-4.  Returns dict(iu, iv, ip, key (uint64; all ones = dropped), xu, xv,
+    w_min[n_img], w_max[n_img])."""
     uvw = np.ascontiguousarray(uvw_m, dtype=np.float64)
     fr = np.ascontiguousarray(freq_hz, dtype=np.float64)
     R, Cn = uvw.shape[0], fr.shape[0]
     M = R * Cn
     n_img = Cn if cube else 1
     out = dict(iu=np.empty(M, np.int32), iv=np.empty(M, np.int32), ip=np.empty(M, np.int32),
-               key=np.empty(M, np.uint32), xu=np.empty(M, np.float64), xv=np.empty(M, np.float64),
+               key=np.empty(M, np.uint64), xu=np.empty(M, np.float64), xv=np.empty(M, np.float64),
                w_min=np.full(n_img, w_min, np.float64), w_max=np.full(n_img, w_max, np.float64))
     L = lib()
     L.rko_index(C.c_int64(R), C.c_int32(Cn), _ptr(uvw, C.c_double), _ptr(fr, C.c_double),
                 C.c_int32(N), C.c_int32(Nw), C.c_int32(S), C.c_double(dl), C.c_int32(B),
                 C.c_int32(cube), _ptr(out["w_min"], C.c_double), _ptr(out["w_max"], C.c_double),
                 _ptr(out["iu"], C.c_int32), _ptr(out["iv"], C.c_int32), _ptr(out["ip"], C.c_int32),
-                _ptr(out["key"], C.c_uint32), _ptr(out["xu"], C.c_double), _ptr(out["xv"], C.c_double))
+                _ptr(out["key"], C.c_uint64), _ptr(out["xu"], C.c_double), _ptr(out["xv"], C.c_double))
     return out
 
 
 def sort(key) -> np.ndarray:
-    key = np.ascontiguousarray(key, dtype=np.uint32)
+    key = np.ascontiguousarray(key, dtype=np.uint64)
     perm = np.empty(key.shape[0], np.uint32)
     lib().rko_sort(key.shape[0], key, perm)
     return perm

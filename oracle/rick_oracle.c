@@ -44,6 +44,7 @@
 
 #define RKO_C0 299792458.0
 #define RKO_PI 3.14159265358979323846264338327950288
+#define RKO_KEY_DROPPED 0xFFFFFFFFFFFFFFFFull
 
 /* ------------------------------------------------------------------------ */
 /* Kaiser-Bessel kernel (reading R5: exact evaluation, g(0)=1)  */
@@ -119,15 +120,19 @@ double rko_taper(double nu, int S, double beta)
 /* ------------------------------------------------------------------------ */
 
 /* Visibility k = r*C + c.  Outputs per visibility: iu, iv (centre cell), ip
- * (plane of its image), key (0xFFFFFFFF when dropped), xu, xv (cell
- * coordinates from the grid centre).  w_min/w_max: [n_img] (n_img = C when
+ * (plane of its image), key (64-bit; all ones when dropped), xu, xv (cell
+ * coordinates from the grid centre).
+ * key = ((((img*N_w + i_p)*T + i_v/B)*T + i_u/B)*B + i_v%B)*B + i_u%B
+ * (image, plane, uv tile of B x B cells, cell inside the tile: DESIGN.md
+ * step 4 / reading R22 -- the paper's bucket sort, leaves
+ * the order inside a bucket open).  w_min/w_max: [n_img] (n_img = C when
  * cube, else 1); on input NaN -> derived from ALL visibilities of that image
  * (on-grid or not).  Each operation individually rounded (no FMA; build with
  * -ffp-contract=off), in exactly this order. */
 int rko_index(int64_t n_rows, int32_t n_chan, const double *uvw_m, const double *freq_hz,
               int32_t N, int32_t Nw, int32_t S, double dl, int32_t B, int32_t cube,
               double *w_min, double *w_max,
-              int32_t *iu, int32_t *iv, int32_t *ip, uint32_t *key, double *xu, double *xv)
+              int32_t *iu, int32_t *iv, int32_t *ip, uint64_t *key, double *xu, double *xv)
 {
     const int32_t h = (S - 1) / 2, T = N / B;
     const double inv_du = (double)N * dl;
@@ -177,9 +182,10 @@ int rko_index(int64_t n_rows, int32_t n_chan, const double *uvw_m, const double 
             if (on) {
                 uint64_t kk = (uint64_t)img * (uint64_t)Nw + (uint64_t)i_p;
                 kk = (kk * (uint64_t)T + (uint64_t)(i_v / B)) * (uint64_t)T + (uint64_t)(i_u / B);
-                key[k] = (uint32_t)kk;
+                kk = (kk * (uint64_t)B + (uint64_t)(i_v % B)) * (uint64_t)B + (uint64_t)(i_u % B);
+                key[k] = kk;
             } else {
-                key[k] = 0xFFFFFFFFu;
+                key[k] = RKO_KEY_DROPPED;
             }
         }
     }
@@ -187,19 +193,23 @@ int rko_index(int64_t n_rows, int32_t n_chan, const double *uvw_m, const double 
     return 0;
 }
 
-/* Stable sort by key == sort by (key, original index). */
-static int cmp_u64(const void *a, const void *b)
+/* Stable sort by key == sort by (key, original index): perm[q] = index of the
+ * visibility at sorted position q. */
+typedef struct { uint64_t key; uint64_t idx; } rko_pair;
+
+static int cmp_pair(const void *a, const void *b)
 {
-    uint64_t x = *(const uint64_t *)a, y = *(const uint64_t *)b;
-    return (x > y) - (x < y);
+    const rko_pair *x = (const rko_pair *)a, *y = (const rko_pair *)b;
+    if (x->key != y->key) return (x->key > y->key) - (x->key < y->key);
+    return (x->idx > y->idx) - (x->idx < y->idx);
 }
 
-int rko_sort(int64_t M, const uint32_t *key, uint32_t *perm)
+int rko_sort(int64_t M, const uint64_t *key, uint32_t *perm)
 {
-    uint64_t *c = (uint64_t *)malloc(sizeof(uint64_t) * (size_t)(M > 0 ? M : 1));
-    for (int64_t k = 0; k < M; ++k) c[k] = ((uint64_t)key[k] << 32) | (uint64_t)(uint32_t)k;
-    qsort(c, (size_t)M, sizeof(uint64_t), cmp_u64);
-    for (int64_t k = 0; k < M; ++k) perm[k] = (uint32_t)(c[k] & 0xFFFFFFFFu);
+    rko_pair *c = (rko_pair *)malloc(sizeof(rko_pair) * (size_t)(M > 0 ? M : 1));
+    for (int64_t k = 0; k < M; ++k) { c[k].key = key[k]; c[k].idx = (uint64_t)k; }
+    qsort(c, (size_t)M, sizeof(rko_pair), cmp_pair);
+    for (int64_t k = 0; k < M; ++k) perm[k] = (uint32_t)c[k].idx;
     free(c);
     return 0;
 }
@@ -397,7 +407,7 @@ int rko_image(int64_t n_rows, int32_t n_chan, const double *uvw_m, const double 
     int32_t *iu = (int32_t *)malloc(sizeof(int32_t) * (size_t)(M + 1));
     int32_t *iv = (int32_t *)malloc(sizeof(int32_t) * (size_t)(M + 1));
     int32_t *ip = (int32_t *)malloc(sizeof(int32_t) * (size_t)(M + 1));
-    uint32_t *key = (uint32_t *)malloc(sizeof(uint32_t) * (size_t)(M + 1));
+    uint64_t *key = (uint64_t *)malloc(sizeof(uint64_t) * (size_t)(M + 1));
     double *xu = (double *)malloc(sizeof(double) * (size_t)(M + 1));
     double *xv = (double *)malloc(sizeof(double) * (size_t)(M + 1));
     double *wmin = (double *)malloc(sizeof(double) * (size_t)n_img);
@@ -411,7 +421,7 @@ int rko_image(int64_t n_rows, int32_t n_chan, const double *uvw_m, const double 
     int64_t n_gridded = 0;
     double sum_w = 0.0;
     for (int64_t k = 0; k < M; ++k)
-        if (key[k] != 0xFFFFFFFFu) {
+        if (key[k] != RKO_KEY_DROPPED) {
             const int32_t img = cube ? (int32_t)(k % n_chan) : 0;
             cnt[(int64_t)img * Nw + ip[k] + 1]++;
             n_gridded++;
@@ -422,7 +432,7 @@ int rko_image(int64_t n_rows, int32_t n_chan, const double *uvw_m, const double 
     int64_t *fill = (int64_t *)malloc(sizeof(int64_t) * (size_t)(n_pl + 1));
     memcpy(fill, cnt, sizeof(int64_t) * (size_t)(n_pl + 1));
     for (int64_t k = 0; k < M; ++k)
-        if (key[k] != 0xFFFFFFFFu) {
+        if (key[k] != RKO_KEY_DROPPED) {
             const int32_t img = cube ? (int32_t)(k % n_chan) : 0;
             list[fill[(int64_t)img * Nw + ip[k]]++] = k;
         }

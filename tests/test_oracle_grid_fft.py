@@ -46,7 +46,7 @@ def test_mass_invariant_linearity_weights(cfg1):
     wl = cfg1
     N = wl.n
     r = oracle.index(wl.uvw_m, wl.freq_hz, N, 1, S, wl.pixel_rad, 16)
-    keep = np.nonzero(r["key"] != 0xFFFFFFFF)[0]
+    keep = np.nonzero(r["key"] != np.uint64(0xFFFFFFFFFFFFFFFF))[0]
     vis = wl.vis.ravel()
     rng = np.random.default_rng(5)
     wgt = rng.uniform(0.5, 2.0, vis.shape[0]).astype(np.float32)

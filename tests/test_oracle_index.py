@@ -6,6 +6,7 @@ import numpy as np
 import oracle
 
 C0 = 299792458.0
+DROPPED = np.uint64(0xFFFFFFFFFFFFFFFF)
 
 
 def _one(u_cells, v_cells, N=64, Nw=4, S=7, w=(0.0,), B=16, freq=C0, dl=1e-3, **kw):
@@ -31,7 +32,7 @@ def test_on_grid_rule_eq5_halo():
     N, S = 64, 7   # h = 3: centre cells 3..60 are kept, 2 and 61 dropped
     r = _one([3 - 32, 2 - 32, 60 - 32, 61 - 32, 0, 0], [0, 0, 0, 0, 3 - 32, 61 - 32], N=N, S=S)
     assert list(r["iu"][:4]) == [3, 2, 60, 61]
-    dropped = r["key"] == 0xFFFFFFFF
+    dropped = r["key"] == DROPPED
     assert list(dropped) == [False, True, False, True, False, True]
 
 
@@ -54,10 +55,17 @@ def test_key_layout():
     r = _one([0.0, 17.0, -20.0], [0.0, -3.0, 20.0], w=[0.0, 10.0, 5.0], N=N, B=B, Nw=Nw)
     T = N // B
     for k in range(3):
-        expect = (r["ip"][k] * T + r["iv"][k] // B) * T + r["iu"][k] // B
-        assert r["key"][k] == expect
+        iu, iv, ip = int(r["iu"][k]), int(r["iv"][k]), int(r["ip"][k])
+        expect = (((ip * T + iv // B) * T + iu // B) * B + iv % B) * B + iu % B
+        assert int(r["key"][k]) == expect
     assert list(r["iu"]) == [32, 49, 12] and list(r["iv"]) == [32, 29, 52]
-    assert list(r["key"]) == [(0 * 4 + 2) * 4 + 2, (3 * 4 + 1) * 4 + 3, (2 * 4 + 3) * 4 + 0]
+    # (plane, tile row, tile column) then (row, column) inside the 16 x 16 tile
+    assert [int(x) for x in r["key"]] == [(((0 * 4 + 2) * 4 + 2) * 16 + 0) * 16 + 0,
+                                          (((3 * 4 + 1) * 4 + 3) * 16 + 13) * 16 + 1,
+                                          (((2 * 4 + 3) * 4 + 0) * 16 + 4) * 16 + 12]
+    # the cell inside the tile is the least significant part: same tile, same plane -> keys differ by the cell
+    r2 = _one([0.0, 1.0, 0.0], [0.0, 0.0, 1.0], N=N, B=B, Nw=Nw)
+    assert int(r2["key"][1]) - int(r2["key"][0]) == 1 and int(r2["key"][2]) - int(r2["key"][0]) == B
 
 
 def test_channel_scaling_and_cube_key():
@@ -72,8 +80,9 @@ def test_channel_scaling_and_cube_key():
     assert list(rc["w_min"]) == [1.0, 2.0] and list(rc["w_max"]) == [3.0, 6.0]
     T = N // 16
     img = np.array([0, 1, 0, 1])
-    expect = ((img * Nw + rc["ip"]) * T + rc["iv"] // 16) * T + rc["iu"] // 16
-    assert list(rc["key"]) == list(expect)
+    iu, iv, ip = rc["iu"].astype(np.int64), rc["iv"].astype(np.int64), rc["ip"].astype(np.int64)
+    expect = ((((img * Nw + ip) * T + iv // 16) * T + iu // 16) * 16 + iv % 16) * 16 + iu % 16
+    assert [int(x) for x in rc["key"]] == list(expect)
 
 
 def test_index_bruteforce_cfg1(cfg1):
@@ -96,7 +105,7 @@ def test_index_bruteforce_cfg1(cfg1):
         ip = min(wl.n_wplanes - 1, math.floor((wl_all[k] - wmin) * (1.0 / dw)))
         assert (r["iu"][k], r["iv"][k], r["ip"][k]) == (iu, iv, ip)
         on = iu - h >= 0 and iu + h <= N - 1 and iv - h >= 0 and iv + h <= N - 1
-        assert (r["key"][k] != 0xFFFFFFFF) == on
+        assert (r["key"][k] != DROPPED) == on
         n_drop += (not on)
         # nearest cell: |x - (i - N/2)| <= 1/2
         assert abs(xu - (iu - N / 2)) <= 0.5 and abs(xv - (iv - N / 2)) <= 0.5
@@ -115,4 +124,4 @@ def test_sort_is_stable_sort(cfg1):
     # ties keep index order
     same = ks[1:] == ks[:-1]
     assert np.all(perm[1:][same] > perm[:-1][same])
-    assert oracle.sort(np.zeros(0, np.uint32)).shape == (0,)
+    assert oracle.sort(np.zeros(0, np.uint64)).shape == (0,)

@@ -24,7 +24,7 @@ def test_against_w_snapped_and_exact_dft(cfg1, cfg1_oracle):
     wl, r = cfg1, cfg1_oracle
     N = wl.n
     idx = oracle.index(wl.uvw_m, wl.freq_hz, N, wl.n_wplanes, wl.support, wl.pixel_rad, 16)
-    keep = idx["key"] != 0xFFFFFFFF
+    keep = idx["key"] != np.uint64(0xFFFFFFFFFFFFFFFF)
     assert r["stats"]["n_gridded"] == int(keep.sum())
     assert r["stats"]["n_dropped"] == int((~keep).sum()) and r["stats"]["n_dropped"] > 0
     u, v, w = _uvw_lambda(wl)
@@ -64,7 +64,7 @@ def test_unit_source_at_phase_centre(cfg1):
     wgt = rng.uniform(0.5, 1.5, wl.vis.shape).astype(np.float32)
     rw = oracle.image(wl.uvw_m, wl.freq_hz, wl.vis, wgt, wl.n, wl.n_wplanes, wl.support, wl.pixel_rad)
     idx = oracle.index(wl.uvw_m, wl.freq_hz, N, wl.n_wplanes, wl.support, wl.pixel_rad, 16)
-    sw = wgt.ravel()[idx["key"] != 0xFFFFFFFF].astype(np.float64).sum()
+    sw = wgt.ravel()[idx["key"] != np.uint64(0xFFFFFFFFFFFFFFFF)].astype(np.float64).sum()
     assert abs(rw["stats"]["sum_w"] - sw) < 1e-9 * sw
     assert abs(rw["image"][N // 2, N // 2] / sw - 1) < 1e-6
 
@@ -93,7 +93,7 @@ def test_stage_outputs_are_consistent(cfg1, cfg1_oracle):
     sg, sf = r["stack_grid"], r["stack_fft"]
     assert sg.shape == (Nw, N, N)
     idx = oracle.index(wl.uvw_m, wl.freq_hz, N, Nw, wl.support, wl.pixel_rad, 16)
-    keep = idx["key"] != 0xFFFFFFFF
+    keep = idx["key"] != np.uint64(0xFFFFFFFFFFFFFFFF)
     # per-plane Parseval and FFT == numpy on the gridded plane
     for z in range(Nw):
         assert abs((np.abs(sf[z]) ** 2).sum() / (N * N * (np.abs(sg[z]) ** 2).sum()) - 1) < 1e-12
