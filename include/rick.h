@@ -23,7 +23,7 @@
  *     "host" = ordinary host memory.  Said per argument.
  *   Ownership: the caller owns every input and output buffer; the library borrows
  *     them until the work it enqueued on the plan's stream has completed and never
- *     frees them.  The plan owns keys, permutation, plane stack, image, tables and
+ *     frees them.  The plan owns sort items, plane stack, image, tables and
  *     frees them in rick_plan_destroy.
  *   Stream: every call enqueues on the plan's stream and returns without
  *     synchronising, except rick_get_stats, rick_image_host and rick_plan_destroy.
@@ -61,7 +61,7 @@ typedef struct {
     double  pixel_rad;   /* dl, radians per pixel, > 0                                          */
     double  kb_beta;     /* Kaiser-Bessel beta; <= 0 -> 2.34*S (reading R5)                     */
     int32_t grid_prec;   /* RICK_GRID_F64 (complex double mesh) | RICK_GRID_F32   */
-    int32_t tile;        /* sort-tile edge B in cells (power of two, 8..32); 0 -> 16            */
+    int32_t tile;        /* uv-tile edge B in cells (power of two, 8..32); 0 -> 16              */
     int32_t plane_batch; /* w-planes resident at once; 0 -> all N_w                             */
     int32_t cube;        /* 0: all channels into one image; 1: one image per channel (R16)      */
     int32_t reserved;    /* must be 0                                                           */
@@ -95,7 +95,8 @@ int rick_plan_destroy(rick_plan_t* p);
  *   weights      device, [R][C] float, or NULL (all 1: natural weighting)
  *   chan_freq_hz HOST, [C] double, > 0
  *   n_chan       C >= 1;  n_rows  R >= 0 (R = 0 gives an all-zero stack)
- * M = R*C must be < 2^32 - 1.  Scratch for keys / permutation grows as needed
+ * M = R*C must be < 2^32 - 1, and bits(n_img N_w N^2) + bits(M) <= 64 (one sort item per
+ * visibility).  Scratch for the sort items grows as needed
  * (RICK_ERR_OOM if it cannot).  Requires plane_batch == N_w and cube == 0. */
 int rick_grid(rick_plan_t* p, const void* vis, int32_t vis_dtype, const double* uvw_m,
               const float* weights, const double* chan_freq_hz, int32_t n_chan, int64_t n_rows);
@@ -137,8 +138,11 @@ const char* rick_last_error(const rick_plan_t* p);
 
 /* Debug accessors for stage-wise parity: device pointers owned by the plan, valid
  * until the next rick_* call on it; NULL if that stage has not run. */
-const uint32_t* rick_debug_keys(rick_plan_t* p);   /* [M] keys in visibility order          */
-const uint32_t* rick_debug_perm(rick_plan_t* p);   /* [M] stable permutation (sorted order) */
+/* [M] sort items (key << *idx_bits) | k, key = ((((img N_w + i_p) T + i_v/B) T + i_u/B) B + i_v%B) B + i_u%B
+ * (T = N/B; image, plane, uv tile, cell inside the tile: DESIGN.md step 4), the all-ones pattern
+ * of *key_bits bits for a dropped visibility.  sorted = 0: in visibility order (item k describes
+ * visibility k); sorted = 1: after the stable sort by key -- the low parts are then the permutation. */
+const uint64_t* rick_debug_items(rick_plan_t* p, int32_t sorted, int32_t* idx_bits, int32_t* key_bits);
 void*           rick_debug_planes(rick_plan_t* p); /* [N_w][N][N] complex of grid_prec      */
 
 /* Per-kernel timing with CUDA events on the plan's stream (for roofline reporting).

@@ -10,7 +10,6 @@
 
 #define RICK_C0 299792458.0
 #define RICK_MAX_CHAN 4096
-#define RICK_KEY_DROPPED 0xFFFFFFFFu
 #define RICK_KB_DEG 18          // degree of the per-tap polynomial of the Kaiser-Bessel kernel
 
 // Per-image w-plane geometry, computed on the device by k_wrange_finish (a0).
@@ -31,7 +30,7 @@ struct DevCounters {
 
 struct rick_plan_s {
     rick_plan_desc d;
-    int N, Nw, S, h, B, T, log2N;
+    int N, Nw, S, h, B, T, log2N, log2B;
     int f32;                 // grid precision
     int batch;               // resident planes
     double beta, dl, inv_du;
@@ -53,10 +52,12 @@ struct rick_plan_s {
 
     // per-call visibility scratch (grows)
     int64_t cap_vis;
-    uint32_t *keys, *keys_a, *keys_b, *perm_a, *perm_b;
+    // sort items (key << idx_bits) | k: unsorted, and the two ping-pong buffers of the radix sort
+    unsigned long long *items, *items_a, *items_b;
+    unsigned long long* sorted_items;      // points at items / items_a / items_b after the sort
+    int idx_bits, key_bits;                // item layout of the last rick_grid / rick_image
     uint32_t* hist; size_t hist_cap;
     uint32_t* scan_tmp; size_t scan_cap;
-    uint32_t *sorted_keys, *sorted_perm;   // point into keys_a/b, perm_a/b after the sort
     int64_t* plane_start;    // [n_planes_total + 1] offsets into the sorted order
     int64_t plane_start_cap;
     double* chan_scale;      // [C] device, s_c = f_c / c0

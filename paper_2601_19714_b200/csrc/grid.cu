@@ -4,23 +4,30 @@
 //   G[i_p][i_v+b][i_u+a] += (w V) g(d_a) g(d_b),  a,b in [-h,h],
 //   d_a = (i_u - N/2 + a) - x_u,  g(t) = I0(beta sqrt(1-(2t/S)^2)) / I0(beta)
 //
-// Design (B200): the visibilities arrive sorted by (image, plane, uv tile of B x B cells).
-// Each WARP takes fixed-size chunks of the sorted order from a dynamic counter (perfect
-// balance in visibilities, whatever the skew of the uv coverage) and owns a PRIVATE
-// shared-memory accumulation tile of (B+S-1)^2 cells -- the tile plus the kernel halo, the
-// single-GPU analogue of the paper's ghost region.  Per batch of 32 visibilities every lane
-// evaluates the 2S kernel values of its own visibility, stages them in shared memory, then the
-// warp walks the 32 visibilities one by one with its lanes spread over the footprint, each lane
-// owning two horizontally adjacent cells: plain read-modify-write, no shared-memory atomics
-// (cells of one footprint are distinct, and successive visibilities are ordered by __syncwarp).
-// When the tile key changes, the tile is flushed to HBM with fire-and-forget RED atomics
-// (non-zero cells only) and re-zeroed.
+// Design (B200): the visibilities arrive sorted by (image, plane, uv tile of B x B cells, cell
+// inside the tile) -- DESIGN.md step 4.  Each WARP takes fixed-size chunks of the sorted order from
+// a dynamic counter (perfect balance in visibilities, whatever the skew of the uv coverage) and
+// owns a PRIVATE shared-memory accumulation tile of (B+S-1)^2 cells -- the tile plus the kernel
+// halo, the single-GPU analogue of the paper's ghost region.  Per batch of 32 visibilities every
+// lane evaluates the 2S kernel values of its own visibility and stages them in shared memory
+// (the v-axis values already multiplied by w V); then the warp walks the 32 visibilities one by one
+// with its lanes spread over the footprint, each lane owning two horizontally adjacent cells.
+//   * Run accumulation: consecutive visibilities of the SAME centre cell have the same footprint,
+//     so their contributions are summed in REGISTERS (4 DFMA per lane per visibility, operands by
+//     two broadcast LDS.128); the shared-memory tile is read-modified-written once per run, when
+//     the centre cell changes (core-dense uv coverage: 5.5 visibilities per run in config 2).
+//     Before, every visibility paid the 2 x 49-cell RMW and the gridder ran at the shared-memory
+//     bandwidth.
+//   * When the tile changes, the tile is flushed to HBM with fire-and-forget RED atomics
+//     (non-zero cells only) and re-zeroed.
 //
 // Kernel values.  d_a = (a-h) - delta with delta = x_u - (i_u - N/2) in [-1/2, 1/2): tap a sees g
-// only on one unit interval, where it is a degree-KB_DEG polynomial in s = 2 delta to < 2e-16
-// (tables.cu fits and checks it at plan time).  The coefficients travel as kernel parameters, so
-// every Horner step is one DFMA with a constant-bank operand: 2 S (KB_DEG+1) DFMA per visibility
-// and no load -- against ~45 terms of the I0 power series per tap before.
+// only on one unit interval, where it is a degree-KB_DEG polynomial f_a(s), s = 2 delta, to < 2e-16
+// (tables.cu fits and checks it at plan time).  g is even, so the mirror tap is f_{S-1-a}(s) =
+// f_a(-s): with f_a = E(s^2) + s O(s^2) one even and one odd Horner chain give BOTH taps, and the
+// centre tap has O = 0 -- (S-1)/2 (KB_DEG+1) + KB_DEG/2 DFMA per axis instead of S KB_DEG.  The
+// coefficients travel as kernel parameters, so every Horner step is one DFMA with a constant-bank
+// operand and no load.
 //
 // The tile row pitch is odd (and > B+S-1, the pad column takes the zero-weight partner of the last
 // cell of a footprint row), so the lanes of a quarter warp hit distinct 16-byte bank groups.
@@ -31,19 +38,19 @@ struct GridParams {
     const float* wgt;
     const double* uvw;
     const double* chan_scale;
-    const uint32_t* skeys;
-    const uint32_t* sperm;
+    const unsigned long long* sitems;    // sorted items (key << idx_bits) | k
     const long long* plane_start;
+    int idx_bits;
     int plane_first, n_planes;
     void* stack;
-    int N, h, B, T, TWp, TH, C;
+    int N, h, B, log2B, T, TWp, TH, C;
     int vis_c128;
     double inv_du;
     unsigned int* chunk_counter;
 };
 template <int S> struct GridParamsS {
     GridParams g;
-    double poly[S][RICK_KB_DEG + 1];     // poly[a][k]: coefficient of s^k of tap a
+    double poly[(S + 1) / 2][RICK_KB_DEG + 1];     // poly[a][k]: coefficient of s^k of tap a <= h
 };
 
 #define GRID_WARPS 8
@@ -69,46 +76,57 @@ __device__ __forceinline__ void red_add(float2* a, float2 v) { atomicAdd(a, v); 
 
 __global__ void k_chunk_reset(unsigned int* c) { *c = 0u; }
 
+template <int S> __host__ __device__ constexpr size_t grid_stage_bytes()
+{
+    // ku[32][SP] doubles | kw[32][S] double2 | key[32] u64
+    return (size_t)32 * (2 * ((S + 1) / 2)) * 8 + (size_t)32 * S * 16 + 32 * 8;
+}
+
 template <typename GT, int S>
 __global__ void __launch_bounds__(GRID_WARPS * 32) k_grid(const __grid_constant__ GridParamsS<S> PS)
 {
     typedef typename cell_t<GT>::type cell;
+    typedef unsigned long long u64;
+    constexpr int H = (S - 1) / 2;
     constexpr int PW = (S + 1) / 2;                 // cell pairs per footprint row
     constexpr int SP = 2 * PW;                      // padded footprint width (even)
     constexpr int NPAIR = S * PW, ROUNDS = (NPAIR + 31) / 32;
     constexpr int DEG = RICK_KB_DEG;
+    static_assert(DEG % 2 == 0, "even/odd Horner split assumes an even degree");
     const GridParams& P = PS.g;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int TWp = P.TWp, TH = P.TH, N = P.N, h = P.h, B = P.B, T = P.T;
+    const int TWp = P.TWp, TH = P.TH, N = P.N, h = P.h, B = P.B, T = P.T, log2B = P.log2B;
     const int tile_cells = TH * TWp;
+    const int sub_bits = 2 * log2B, idx_bits = P.idx_bits;
+    const u64 idx_mask = (1ull << idx_bits) - 1ull;
 
-    // shared layout per warp: tile | ku[32][SP] | kv[32][SP] | vr[32] | vi[32] | base[32]
+    // shared layout per warp: tile | ku[32][SP] | kw[32][S] | key[32]
     const size_t tile_bytes = ((size_t)tile_cells * sizeof(cell) + 15) & ~(size_t)15;
-    const size_t per_warp = tile_bytes + (size_t)(2 * 32 * SP + 64) * sizeof(double) + 32 * sizeof(int);
+    const size_t per_warp = tile_bytes + grid_stage_bytes<S>();
     unsigned char* wbase = smem_raw + (size_t)warp * per_warp;
     cell* tile = reinterpret_cast<cell*>(wbase);
     double* s_ku = reinterpret_cast<double*>(wbase + tile_bytes);
-    double* s_kv = s_ku + 32 * SP;
-    double* s_vr = s_kv + 32 * SP;
-    double* s_vi = s_vr + 32;
-    int* s_base = reinterpret_cast<int*>(s_vi + 32);
+    double2* s_kw = reinterpret_cast<double2*>(s_ku + 32 * SP);
+    u64* s_key = reinterpret_cast<u64*>(s_kw + 32 * S);
 
     cell zero;
     zero.x = 0;
     zero.y = 0;
     for (int i = lane; i < tile_cells; i += 32) tile[i] = zero;
-    for (int i = lane; i < 2 * 32 * SP; i += 32) s_ku[i] = 0.0;      // also the zero weight of the pad column
+    for (int i = lane; i < 32 * SP; i += 32) s_ku[i] = 0.0;      // also the zero weight of the pad column
     __syncwarp();
 
     // cell pair(s) of this lane: pair = lane + 32*rr -> row b, cells (b, 2 a2), (b, 2 a2 + 1)
     int fb[ROUNDS], fa[ROUNDS], foff[ROUNDS];
+    double acc[ROUNDS][4];
 #pragma unroll
     for (int rr = 0; rr < ROUNDS; ++rr) {
         const int pi = lane + 32 * rr;
-        fb[rr] = pi / PW;
-        fa[rr] = 2 * (pi - fb[rr] * PW);
+        fb[rr] = pi < NPAIR ? pi / PW : 0;
+        fa[rr] = pi < NPAIR ? 2 * (pi - fb[rr] * PW) : 0;
         foff[rr] = fb[rr] * TWp + fa[rr];
+        acc[rr][0] = acc[rr][1] = acc[rr][2] = acc[rr][3] = 0.0;
     }
 
     const long long v_begin = P.plane_start[P.plane_first];
@@ -117,10 +135,31 @@ __global__ void __launch_bounds__(GRID_WARPS * 32) k_grid(const __grid_constant_
     const unsigned int TT = (unsigned)T * (unsigned)T;
     const double shift = (double)(N / 2) + 0.5;
 
-    uint32_t cur_key = RICK_KEY_DROPPED;
+    const u64 NOKEY = ~0ull;
+    u64 cur_cell = NOKEY;          // key of the run being summed in registers
+    int cur_base = 0;              // its top-left footprint cell, local to the tile
 
-    auto flush = [&](uint32_t key) {
-        const unsigned int pz = key / TT, rem = key - pz * TT;
+    // registers -> tile, once per run
+    auto flush_run = [&]() {
+#pragma unroll
+        for (int rr = 0; rr < ROUNDS; ++rr) {
+            if (lane + 32 * rr < NPAIR) {
+                cell* tp = tile + cur_base + foff[rr];
+                cell t0 = tp[0], t1 = tp[1];
+                t0.x += (GT)acc[rr][0];
+                t0.y += (GT)acc[rr][1];
+                t1.x += (GT)acc[rr][2];
+                t1.y += (GT)acc[rr][3];
+                tp[0] = t0;
+                tp[1] = t1;
+            }
+            acc[rr][0] = acc[rr][1] = acc[rr][2] = acc[rr][3] = 0.0;
+        }
+    };
+    // tile -> HBM, once per (tile, chunk)
+    auto flush_tile = [&](u64 tkey) {
+        __syncwarp();
+        const unsigned int pz = (unsigned int)(tkey / TT), rem = (unsigned int)(tkey - (u64)pz * TT);
         const int tv = (int)(rem / (unsigned)T), tu = (int)(rem - (unsigned)tv * (unsigned)T);
         cell* plane = reinterpret_cast<cell*>(P.stack) + (size_t)(pz - (unsigned)P.plane_first) * N * N;
         for (int row = 0; row < TH; ++row) {
@@ -146,11 +185,10 @@ __global__ void __launch_bounds__(GRID_WARPS * 32) k_grid(const __grid_constant_
 
         for (long long b0 = c_begin; b0 < c_end; b0 += 32) {
             const long long ks = b0 + lane;
-            const bool valid = ks < c_end;
-            uint32_t key = RICK_KEY_DROPPED;
-            if (valid) {
-                key = P.skeys[ks];
-                const unsigned int idx = P.sperm[ks];
+            if (ks < c_end) {
+                const u64 item = P.sitems[ks];
+                s_key[lane] = item >> idx_bits;
+                const unsigned int idx = (unsigned int)(item & idx_mask);
                 const unsigned int r = idx / (unsigned)P.C, c = idx - r * (unsigned)P.C;
                 const double s = P.chan_scale[c];
                 const double xu = __dmul_rn(__dmul_rn(P.uvw[3ull * r + 0], s), P.inv_du);
@@ -172,64 +210,72 @@ __global__ void __launch_bounds__(GRID_WARPS * 32) k_grid(const __grid_constant_
                     vr *= om;
                     vi *= om;
                 }
-                s_vr[lane] = vr;
-                s_vi[lane] = vi;
-                // top-left footprint cell, local to the tile: (i_u - h) - (tu*B - h) = i_u mod B
-                s_base[lane] = (iv - (iv / B) * B) * TWp + (iu - (iu / B) * B);
-                // kernel values: tap a at d_a = (a-h) - s/2, s = 2 (x - (i - N/2)); 2S Horner chains
+                // kernel values: tap a at d_a = (a-h) - s/2, s = 2 (x - (i - N/2)); mirror taps share E, O
                 const double su = 2.0 * (xu - (double)(iu - N / 2));
                 const double sv = 2.0 * (xv - (double)(iv - N / 2));
-                double au[S], av[S];
+                const double su2 = su * su, sv2 = sv * sv;
+                double fu[S], fv[S];
 #pragma unroll
-                for (int a = 0; a < S; ++a) {
-                    au[a] = PS.poly[a][DEG];
-                    av[a] = PS.poly[a][DEG];
-                }
+                for (int a = 0; a <= H; ++a) {
+                    double eu = PS.poly[a][DEG], ev = PS.poly[a][DEG];
+                    double ou = PS.poly[a][DEG - 1], ov = PS.poly[a][DEG - 1];
 #pragma unroll
-                for (int k = DEG - 1; k >= 0; --k) {
-#pragma unroll
-                    for (int a = 0; a < S; ++a) {
-                        au[a] = fma(au[a], su, PS.poly[a][k]);
-                        av[a] = fma(av[a], sv, PS.poly[a][k]);
+                    for (int k = DEG - 2; k >= 0; k -= 2) {
+                        eu = fma(eu, su2, PS.poly[a][k]);
+                        ev = fma(ev, sv2, PS.poly[a][k]);
+                        if (k >= 2 && a < H) {
+                            ou = fma(ou, su2, PS.poly[a][k - 1]);
+                            ov = fma(ov, sv2, PS.poly[a][k - 1]);
+                        }
+                    }
+                    if (a < H) {
+                        fu[a] = fma(su, ou, eu);
+                        fu[S - 1 - a] = fma(-su, ou, eu);
+                        fv[a] = fma(sv, ov, ev);
+                        fv[S - 1 - a] = fma(-sv, ov, ev);
+                    } else {
+                        fu[a] = eu;
+                        fv[a] = ev;
                     }
                 }
 #pragma unroll
                 for (int a = 0; a < S; ++a) {
-                    s_ku[lane * SP + a] = au[a];
-                    s_kv[lane * SP + a] = av[a];
+                    s_ku[lane * SP + a] = fu[a];
+                    s_kw[lane * S + a] = make_double2(vr * fv[a], vi * fv[a]);
                 }
             }
             __syncwarp();
             const int nb = (int)((c_end - b0) < 32 ? (c_end - b0) : 32);
             for (int j = 0; j < nb; ++j) {
-                const uint32_t kj = __shfl_sync(0xffffffffu, key, j);
-                if (kj != cur_key) {
-                    if (cur_key != RICK_KEY_DROPPED) flush(cur_key);
-                    cur_key = kj;
+                const u64 kj = s_key[j];
+                if (kj != cur_cell) {
+                    if (cur_cell != NOKEY) {
+                        flush_run();
+                        if ((kj >> sub_bits) != (cur_cell >> sub_bits)) flush_tile(cur_cell >> sub_bits);
+                    }
+                    cur_cell = kj;
+                    const int sub = (int)(kj & ((1ull << sub_bits) - 1ull));
+                    cur_base = (sub >> log2B) * TWp + (sub & (B - 1));
                 }
-                const int base = s_base[j];
-                const double vr = s_vr[j], vi = s_vi[j];
 #pragma unroll
                 for (int rr = 0; rr < ROUNDS; ++rr) {
                     if (lane + 32 * rr < NPAIR) {
                         const double2 k2 = *reinterpret_cast<const double2*>(&s_ku[j * SP + fa[rr]]);
-                        const double kvb = s_kv[j * SP + fb[rr]];
-                        const double wr = vr * kvb, wi = vi * kvb;
-                        cell* tp = tile + base + foff[rr];
-                        cell t0 = tp[0], t1 = tp[1];
-                        t0.x += (GT)(wr * k2.x);
-                        t0.y += (GT)(wi * k2.x);
-                        t1.x += (GT)(wr * k2.y);
-                        t1.y += (GT)(wi * k2.y);
-                        tp[0] = t0;
-                        tp[1] = t1;
+                        const double2 w2 = s_kw[j * S + fb[rr]];
+                        acc[rr][0] = fma(w2.x, k2.x, acc[rr][0]);
+                        acc[rr][1] = fma(w2.y, k2.x, acc[rr][1]);
+                        acc[rr][2] = fma(w2.x, k2.y, acc[rr][2]);
+                        acc[rr][3] = fma(w2.y, k2.y, acc[rr][3]);
                     }
                 }
-                __syncwarp();
             }
+            __syncwarp();
         }
-        if (cur_key != RICK_KEY_DROPPED) flush(cur_key);
-        cur_key = RICK_KEY_DROPPED;
+        if (cur_cell != NOKEY) {
+            flush_run();
+            flush_tile(cur_cell >> sub_bits);
+            cur_cell = NOKEY;
+        }
     }
 }
 
@@ -253,24 +299,25 @@ template <typename GT, int S>
 static int launch_grid(rick_plan_t* p, const GridParams& P)
 {
     typedef typename cell_t<GT>::type cell;
-    constexpr int SP = 2 * ((S + 1) / 2);
     GridParamsS<S> PS;
     PS.g = P;
-    for (int a = 0; a < S; ++a)
+    for (int a = 0; a < (S + 1) / 2; ++a)
         for (int k = 0; k <= RICK_KB_DEG; ++k) PS.poly[a][k] = p->kb_poly[a * (RICK_KB_DEG + 1) + k];
     const size_t tile_bytes = ((size_t)P.TH * P.TWp * sizeof(cell) + 15) & ~(size_t)15;
-    const size_t per_warp = tile_bytes + (size_t)(2 * 32 * SP + 64) * sizeof(double) + 32 * sizeof(int);
-    const size_t smem = GRID_WARPS * per_warp;
+    const size_t per_warp = tile_bytes + grid_stage_bytes<S>();
+    int warps = GRID_WARPS;                     // fewer warps per CTA when the tile is large
+    while (warps > 1 && warps * per_warp > 227 * 1024) warps >>= 1;
+    const size_t smem = warps * per_warp;
     if (smem > 227 * 1024) {
         p->err = "tile/support too large for the gridder's shared memory";
         return RICK_ERR_INVALID;
     }
     RICK_CUDA(p, cudaFuncSetAttribute(k_grid<GT, S>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int per_sm = 1;
-    RICK_CUDA(p, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_grid<GT, S>, GRID_WARPS * 32, smem));
+    RICK_CUDA(p, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_grid<GT, S>, warps * 32, smem));
     if (per_sm < 1) per_sm = 1;
     RICK_KERNEL(p, RK_RESET, k_chunk_reset<<<1, 1, 0, p->stream>>>(P.chunk_counter));
-    RICK_KERNEL(p, RK_GRID, k_grid<GT, S><<<p->n_sm * per_sm, GRID_WARPS * 32, smem, p->stream>>>(PS));
+    RICK_KERNEL(p, RK_GRID, k_grid<GT, S><<<p->n_sm * per_sm, warps * 32, smem, p->stream>>>(PS));
     return RICK_OK;
 }
 
@@ -298,8 +345,8 @@ int rick_grid_planes(rick_plan_t* p, const void* vis, int vis_dtype, const doubl
     P.wgt = weights;
     P.uvw = uvw_m;
     P.chan_scale = p->chan_scale;
-    P.skeys = p->sorted_keys;
-    P.sperm = p->sorted_perm;
+    P.sitems = p->sorted_items;
+    P.idx_bits = p->idx_bits;
     P.plane_start = (const long long*)p->plane_start;
     P.plane_first = plane_first;
     P.n_planes = n_planes;
@@ -307,6 +354,7 @@ int rick_grid_planes(rick_plan_t* p, const void* vis, int vis_dtype, const doubl
     P.N = p->N;
     P.h = p->h;
     P.B = p->B;
+    P.log2B = p->log2B;
     P.T = p->T;
     P.TH = p->B + p->S - 1;
     P.TWp = grid_pitch(p->B, p->S);

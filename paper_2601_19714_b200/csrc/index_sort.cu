@@ -8,10 +8,11 @@
 //   on-grid <=> i_u-h >= 0, i_u+h <= N-1 (same in v)                   (Eq. 5; R10)
 //   w_l = w_m * s_c;  dw = (w_max - w_min)/N_w;  i_p = min(N_w-1, floor((w_l - w_min) * (1/dw)))
 //                                                                     ("closest w-plane", :48; R4)
-//   key = ((img*N_w + i_p)*T + i_v/B)*T + i_u/B;  dropped -> 0xFFFFFFFF
+//   key = ((((img*N_w + i_p)*T + i_v/B)*T + i_u/B)*B + i_v%B)*B + i_u%B;  dropped -> all ones
+//   (image, plane, uv tile, cell inside the tile: DESIGN.md step 4, reading R22)
 // a2: the single-GPU analogue of the paper's bucket sort: a stable
-// least-significant-digit radix sort of (key, visibility index) pairs, which equals the
-// oracle's sort by (key, index).
+// least-significant-digit radix sort of 64-bit items (key << idx_bits) | k over the key bits,
+// which equals the oracle's sort by (key, index).
 #include "common.cuh"
 
 // ------------------------------------------------------------------------------------------
@@ -88,19 +89,21 @@ __global__ void k_wrange_finish(const DevCounters* c, const double* __restrict__
 }
 
 // ------------------------------------------------------------------------------------------
-// a1: one thread per visibility k = r*C + c.
+// a1: one thread per visibility k = r*C + c.  Writes the sort item (key << idx_bits) | k.
 // ------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256)
 k_index_key(const double* __restrict__ uvw, const float* __restrict__ wgt,
             const double* __restrict__ chan_scale, const WRange* __restrict__ wrange,
-            unsigned int M, unsigned int C, int N, int Nw, int h, int B, int T, int cube,
-            double inv_du, uint32_t* __restrict__ keys, DevCounters* cnt)
+            unsigned int M, unsigned int C, int N, int Nw, int h, int log2B, int T, int cube,
+            double inv_du, int idx_bits, unsigned long long key_dropped,
+            unsigned long long* __restrict__ items, DevCounters* cnt)
 {
     // grid-stride: statistics stay in registers, one set of atomics per block (same-address
     // atomics per warp made this kernel atomic-bound)
     unsigned int on = 0, off = 0;
     double sw = 0.0;
     const double shift = (double)(N / 2) + 0.5;
+    const int Bm = (1 << log2B) - 1;
     for (unsigned long long kk0 = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; kk0 < M;
          kk0 += (unsigned long long)gridDim.x * blockDim.x) {
         const unsigned int k = (unsigned int)kk0;
@@ -117,17 +120,18 @@ k_index_key(const double* __restrict__ uvw, const float* __restrict__ wgt,
         ip = ip > Nw - 1 ? Nw - 1 : ip;
         ip = ip < 0 ? 0 : ip;
         const bool ok = (iu - h >= 0) && (iu + h <= N - 1) && (iv - h >= 0) && (iv + h <= N - 1);
-        uint32_t key = RICK_KEY_DROPPED;
+        unsigned long long key = key_dropped;
         if (ok) {
             unsigned long long kk = (unsigned long long)img * (unsigned)Nw + (unsigned)ip;
-            kk = (kk * (unsigned)T + (unsigned)(iv / B)) * (unsigned)T + (unsigned)(iu / B);
-            key = (uint32_t)kk;
+            kk = (kk * (unsigned)T + (unsigned)(iv >> log2B)) * (unsigned)T + (unsigned)(iu >> log2B);
+            kk = (((kk << log2B) + (unsigned)(iv & Bm)) << log2B) + (unsigned)(iu & Bm);
+            key = kk;
             on++;
             sw += wgt ? (double)wgt[k] : 1.0;
         } else {
             off++;
         }
-        keys[k] = key;
+        items[k] = (key << idx_bits) | (unsigned long long)k;
     }
     // block-reduced statistics
     __shared__ unsigned int s_on[8], s_off[8];
@@ -160,25 +164,34 @@ k_index_key(const double* __restrict__ uvw, const float* __restrict__ wgt,
 }
 
 // ------------------------------------------------------------------------------------------
-// a2: LSD radix sort, <= 8-bit digits, stable.
+// a2: LSD radix sort of the 64-bit items over their key bits, <= 8-bit digits, stable.  The
+// visibility index sits in the low idx_bits of an item and is never a digit: stability keeps
+// equal keys in index order, so the sorted low parts ARE the permutation.
 // ------------------------------------------------------------------------------------------
 #define RS_THREADS 256
 #define RS_ITEMS 16
 #define RS_TILE (RS_THREADS * RS_ITEMS)
+typedef unsigned long long u64;
 
 __global__ void __launch_bounds__(RS_THREADS)
-k_radix_hist(const uint32_t* __restrict__ keys, unsigned int M, int shift, uint32_t mask, int nbins,
+k_radix_hist(const u64* __restrict__ items, unsigned int M, int shift, uint32_t mask, int nbins,
              uint32_t* __restrict__ hist, unsigned int nblocks)
 {
     __shared__ uint32_t hs[256];
     hs[threadIdx.x] = 0;
     __syncthreads();
     const unsigned long long base = (unsigned long long)blockIdx.x * RS_TILE;
+    u64 it[RS_ITEMS];
+#pragma unroll
+    for (int i = 0; i < RS_ITEMS; ++i) {
+        const unsigned long long idx = base + (unsigned)i * RS_THREADS + threadIdx.x;
+        it[i] = idx < M ? items[idx] : ~0ull;
+    }
 #pragma unroll
     for (int i = 0; i < RS_ITEMS; ++i) {
         const unsigned long long idx = base + (unsigned)i * RS_THREADS + threadIdx.x;
         const bool valid = idx < M;
-        const uint32_t d = valid ? ((keys[idx] >> shift) & mask) : 0xFFFFu;
+        const uint32_t d = valid ? ((uint32_t)(it[i] >> shift) & mask) : 0xFFFFu;
         const unsigned int m = __match_any_sync(0xffffffffu, d);
         if (valid && (int)(threadIdx.x & 31) == __ffs(m) - 1) atomicAdd(&hs[d], (uint32_t)__popc(m));
     }
@@ -186,26 +199,36 @@ k_radix_hist(const uint32_t* __restrict__ keys, unsigned int M, int shift, uint3
     if ((int)threadIdx.x < nbins) hist[(size_t)threadIdx.x * nblocks + blockIdx.x] = hs[threadIdx.x];
 }
 
-__global__ void __launch_bounds__(RS_THREADS)
-k_radix_scatter(const uint32_t* __restrict__ kin, const uint32_t* __restrict__ vin,
-                uint32_t* __restrict__ kout, uint32_t* __restrict__ vout, unsigned int M, int shift,
-                uint32_t mask, int nbins, const uint32_t* __restrict__ hist_scanned,
-                unsigned int nblocks)
+// One tile of RS_TILE items per block: stable rank of every item inside the tile (warp match +
+// per-warp digit counters), the tile is reordered by digit in shared memory, then written out
+// position by position -- consecutive threads write consecutive addresses of one digit's run, so
+// the stores coalesce (scattered 8-byte stores paid one L1 tag cycle per line: 32 per warp store).
+__global__ void __launch_bounds__(RS_THREADS, 3)
+k_radix_scatter(const u64* __restrict__ in, u64* __restrict__ out, unsigned int M, int shift,
+                uint32_t mask, int nbins, const uint32_t* __restrict__ hist_scanned, unsigned int nblocks)
 {
     __shared__ uint32_t cnt[RS_THREADS / 32][256];
+    __shared__ u64 buf[RS_TILE];
+    __shared__ uint32_t dig_start[256];
+    __shared__ long long gofs[256];
+    __shared__ uint32_t wsum[RS_THREADS / 32];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     for (int i = threadIdx.x; i < (RS_THREADS / 32) * 256; i += RS_THREADS) (&cnt[0][0])[i] = 0;
     __syncthreads();
-    const unsigned long long base =
-        (unsigned long long)blockIdx.x * RS_TILE + (unsigned)warp * (32 * RS_ITEMS);
-    uint32_t key[RS_ITEMS];
+    const unsigned long long tile0 = (unsigned long long)blockIdx.x * RS_TILE;
+    const unsigned long long base = tile0 + (unsigned)warp * (32 * RS_ITEMS);
+    u64 it[RS_ITEMS];
     uint32_t rank[RS_ITEMS];
 #pragma unroll
     for (int i = 0; i < RS_ITEMS; ++i) {
         const unsigned long long idx = base + (unsigned)i * 32 + lane;
+        it[i] = idx < M ? in[idx] : ~0ull;
+    }
+#pragma unroll
+    for (int i = 0; i < RS_ITEMS; ++i) {
+        const unsigned long long idx = base + (unsigned)i * 32 + lane;
         const bool valid = idx < M;
-        key[i] = valid ? kin[idx] : 0xFFFFFFFFu;
-        const uint32_t d = (key[i] >> shift) & mask;
+        const uint32_t d = (uint32_t)(it[i] >> shift) & mask;
         const unsigned int m = __match_any_sync(0xffffffffu, valid ? d : 0xFFFFu);
         const int leader = __ffs(m) - 1;
         uint32_t old = 0;
@@ -218,24 +241,49 @@ k_radix_scatter(const uint32_t* __restrict__ kin, const uint32_t* __restrict__ v
         __syncwarp();
     }
     __syncthreads();
-    if ((int)threadIdx.x < nbins) {
-        uint32_t run = hist_scanned[(size_t)threadIdx.x * nblocks + blockIdx.x];
+    // digit d = threadIdx.x: exclusive prefix over the warps, then over the digits of the tile
+    uint32_t total = 0;
+    {
+        const int d = threadIdx.x;
 #pragma unroll
         for (int w = 0; w < RS_THREADS / 32; ++w) {
-            const uint32_t t = cnt[w][threadIdx.x];
-            cnt[w][threadIdx.x] = run;
-            run += t;
+            const uint32_t t = cnt[w][d];
+            cnt[w][d] = total;
+            total += t;
         }
     }
+    uint32_t x = total;
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t y = __shfl_up_sync(0xffffffffu, x, o);
+        if (lane >= o) x += y;
+    }
+    if (lane == 31) wsum[warp] = x;
+    __syncthreads();
+    uint32_t woff = 0;
+#pragma unroll
+    for (int w = 0; w < RS_THREADS / 32; ++w) woff += (w < warp) ? wsum[w] : 0u;
+    const uint32_t start = woff + x - total;
+    dig_start[threadIdx.x] = start;
+    if ((int)threadIdx.x < nbins)
+        gofs[threadIdx.x] = (long long)hist_scanned[(size_t)threadIdx.x * nblocks + blockIdx.x] - (long long)start;
     __syncthreads();
 #pragma unroll
     for (int i = 0; i < RS_ITEMS; ++i) {
         const unsigned long long idx = base + (unsigned)i * 32 + lane;
         if (idx < M) {
-            const uint32_t d = (key[i] >> shift) & mask;
-            const uint32_t pos = cnt[warp][d] + rank[i];
-            kout[pos] = key[i];
-            vout[pos] = vin ? vin[idx] : (uint32_t)idx;
+            const uint32_t d = (uint32_t)(it[i] >> shift) & mask;
+            buf[dig_start[d] + cnt[warp][d] + rank[i]] = it[i];
+        }
+    }
+    __syncthreads();
+    const unsigned int n_valid = (unsigned int)((M - tile0) < RS_TILE ? (M - tile0) : RS_TILE);
+#pragma unroll
+    for (int i = 0; i < RS_ITEMS; ++i) {
+        const unsigned int pos = (unsigned)i * RS_THREADS + threadIdx.x;
+        if (pos < n_valid) {
+            const u64 v = buf[pos];
+            const uint32_t d = (uint32_t)(v >> shift) & mask;
+            out[gofs[d] + (long long)pos] = v;
         }
     }
 }
@@ -317,17 +365,18 @@ k_scan_apply(uint32_t* __restrict__ a, size_t n, const uint32_t* __restrict__ su
     }
 }
 
-// plane_start[z] = first sorted position whose key >= z*T*T  (z = 0..n_planes_total)
-__global__ void k_plane_starts(const uint32_t* __restrict__ skeys, unsigned int M, unsigned long long TT,
-                               int n_planes_total, long long* __restrict__ plane_start)
+// plane_start[z] = first sorted position whose key >= z*N*N  (z = 0..n_planes_total)
+__global__ void k_plane_starts(const u64* __restrict__ sitems, unsigned int M, int idx_bits,
+                               unsigned long long cells_per_plane, int n_planes_total,
+                               long long* __restrict__ plane_start)
 {
     const int z = blockIdx.x * blockDim.x + threadIdx.x;
     if (z > n_planes_total) return;
-    const unsigned long long target = (unsigned long long)z * TT;
+    const unsigned long long target = (unsigned long long)z * cells_per_plane;
     unsigned int lo = 0, hi = M;
     while (lo < hi) {
         const unsigned int mid = lo + (hi - lo) / 2;
-        if ((unsigned long long)skeys[mid] < target) lo = mid + 1; else hi = mid;
+        if ((sitems[mid] >> idx_bits) < target) lo = mid + 1; else hi = mid;
     }
     plane_start[z] = (long long)lo;
 }
@@ -360,21 +409,18 @@ int rick_index_sort(rick_plan_t* p, const double* uvw_m, const float* weights)
                                                           p->Nw, p->d.w_min, p->d.w_max,
                                                           (long long)p->R, p->wrange));
 
-    p->sorted_keys = p->keys;
-    p->sorted_perm = p->perm_a;
+    p->sorted_items = p->items;
     if (M > 0) {
+        const unsigned long long key_dropped = (1ull << p->key_bits) - 1ull;
         {
             unsigned int nb = (M + 255) / 256;
             if (nb > (unsigned)p->n_sm * 8u) nb = (unsigned)p->n_sm * 8u;
             RICK_KERNEL(p, RK_INDEX_KEY, k_index_key<<<nb, 256, 0, st>>>(uvw_m, weights, p->chan_scale, p->wrange, M,
-                                                    (unsigned)p->C, p->N, p->Nw, p->h, p->B, p->T,
-                                                    p->d.cube, p->inv_du, p->keys, p->counters));
+                                                    (unsigned)p->C, p->N, p->Nw, p->h, p->log2B, p->T,
+                                                    p->d.cube, p->inv_du, p->idx_bits, key_dropped, p->items,
+                                                    p->counters));
         }
-
-        // key bits: the all-ones pattern of the sorted bit range is reserved for the sentinel
-        const unsigned long long nkeys = (unsigned long long)n_planes_total * p->T * p->T;
-        int bits = 1;
-        while (((1ull << bits) - 1ull) < nkeys) ++bits;
+        const int bits = p->key_bits;
         const int npass = (bits + 7) / 8;
         const unsigned int nblocks = (M + RS_TILE - 1) / RS_TILE;
         int rc = ensure_u32(p, &p->hist, &p->hist_cap, (size_t)256 * nblocks);
@@ -384,33 +430,31 @@ int rick_index_sort(rick_plan_t* p, const double* uvw_m, const float* weights)
         rc = ensure_u32(p, &p->scan_tmp, &p->scan_cap, nsb_max);
         if (rc) return rc;
 
-        const uint32_t* kin = p->keys;
-        const uint32_t* vin = nullptr;
-        uint32_t* kbuf[2] = {p->keys_a, p->keys_b};
-        uint32_t* vbuf[2] = {p->perm_a, p->perm_b};
-        int shift = 0;
+        const u64* in = (const u64*)p->items;
+        u64* bufs[2] = {(u64*)p->items_a, (u64*)p->items_b};
+        int shift = p->idx_bits;
+        int done = 0;
         for (int pass = 0; pass < npass; ++pass) {
-            const int nb_bits = (bits - shift + (npass - pass) - 1) / (npass - pass);
+            const int nb_bits = (bits - done + (npass - pass) - 1) / (npass - pass);
             const int nbins = 1 << nb_bits;
             const uint32_t mask = (uint32_t)(nbins - 1);
-            RICK_KERNEL(p, RK_RADIX_HIST, k_radix_hist<<<nblocks, RS_THREADS, 0, st>>>(kin, M, shift, mask, nbins, p->hist, nblocks));
+            RICK_KERNEL(p, RK_RADIX_HIST, k_radix_hist<<<nblocks, RS_THREADS, 0, st>>>(in, M, shift, mask, nbins, p->hist, nblocks));
             const size_t n_hist = (size_t)nbins * nblocks;
             const unsigned int nsb = (unsigned int)((n_hist + SC_TILE - 1) / SC_TILE);
             RICK_KERNEL(p, RK_SCAN, k_scan_reduce<<<nsb, SC_THREADS, 0, st>>>(p->hist, n_hist, p->scan_tmp));
             RICK_KERNEL(p, RK_SCAN, k_scan_top<<<1, SC_THREADS, 0, st>>>(p->scan_tmp, nsb));
             RICK_KERNEL(p, RK_SCAN, k_scan_apply<<<nsb, SC_THREADS, 0, st>>>(p->hist, n_hist, p->scan_tmp));
-            uint32_t* ko = kbuf[pass & 1];
-            uint32_t* vo = vbuf[pass & 1];
-            RICK_KERNEL(p, RK_RADIX_SCATTER, k_radix_scatter<<<nblocks, RS_THREADS, 0, st>>>(kin, vin, ko, vo, M, shift, mask, nbins,
+            u64* o = bufs[pass & 1];
+            RICK_KERNEL(p, RK_RADIX_SCATTER, k_radix_scatter<<<nblocks, RS_THREADS, 0, st>>>(in, o, M, shift, mask, nbins,
                                                           p->hist, nblocks));
-            kin = ko;
-            vin = vo;
+            in = o;
             shift += nb_bits;
+            done += nb_bits;
         }
-        p->sorted_keys = (uint32_t*)kin;
-        p->sorted_perm = (uint32_t*)vin;
+        p->sorted_items = (unsigned long long*)in;
     }
     RICK_KERNEL(p, RK_PLANE_STARTS, k_plane_starts<<<(n_planes_total + 1 + 127) / 128, 128, 0, st>>>(
-        p->sorted_keys, M, (unsigned long long)p->T * p->T, n_planes_total, (long long*)p->plane_start));
+        (const u64*)p->sorted_items, M, p->idx_bits, (unsigned long long)p->N * p->N, n_planes_total,
+        (long long*)p->plane_start));
     return RICK_OK;
 }

@@ -87,7 +87,7 @@ extern "C" int rick_plan_destroy(rick_plan_t* p)
     if (!p) return RICK_OK;
     cudaStreamSynchronize(p->stream);
     free_dev(p->twiddle); free_dev(p->taper); free_dev(p->stack); free_dev(p->image);
-    free_dev(p->keys); free_dev(p->keys_a); free_dev(p->keys_b); free_dev(p->perm_a); free_dev(p->perm_b);
+    free_dev(p->items); free_dev(p->items_a); free_dev(p->items_b);
     free_dev(p->hist); free_dev(p->scan_tmp); free_dev(p->plane_start); free_dev(p->chan_scale);
     free_dev(p->wrange); free_dev(p->counters);
     free_dev(p->st_vis); free_dev(p->st_uvw); free_dev(p->st_wgt); free_dev(p->st_img);
@@ -150,6 +150,8 @@ extern "C" int rick_plan(rick_plan_t** out, const rick_plan_desc* d, void* cuda_
     p->T = d->n / B;
     p->log2N = 0;
     while ((1 << p->log2N) < d->n) p->log2N++;
+    p->log2B = 0;
+    while ((1 << p->log2B) < B) p->log2B++;
     p->f32 = d->grid_prec == RICK_GRID_F32;
     p->batch = d->plane_batch ? d->plane_batch : d->n_wplanes;
     p->beta = d->kb_beta > 0.0 ? d->kb_beta : 2.34 * (double)d->support;
@@ -166,6 +168,20 @@ extern "C" int rick_plan(rick_plan_t** out, const rick_plan_desc* d, void* cuda_
 }
 
 // ---------------------------------------------------------------------------------------
+// Sort item = (key << idx_bits) | k.  key < n_img * N_w * N^2 (image, plane, tile, cell in tile); the
+// all-ones pattern of key_bits is reserved for dropped visibilities.
+static void item_bits(const rick_plan_t* p, int32_t n_chan, unsigned long long M, int* key_bits, int* idx_bits)
+{
+    const unsigned long long n_img = p->d.cube ? (unsigned long long)n_chan : 1ull;
+    const unsigned long long nkeys = n_img * (unsigned long long)p->Nw * (unsigned long long)p->N * (unsigned long long)p->N;
+    int kb = 1;
+    while (kb < 63 && ((1ull << kb) - 1ull) < nkeys) ++kb;
+    int ib = 1;
+    while (ib < 32 && (1ull << ib) < M) ++ib;
+    *key_bits = kb;
+    *idx_bits = ib;
+}
+
 static int check_inputs(rick_plan_t* p, const void* vis, int32_t vis_dtype, const double* uvw_m,
                         const double* chan_freq_hz, int32_t n_chan, int64_t n_rows)
 {
@@ -177,9 +193,9 @@ static int check_inputs(rick_plan_t* p, const void* vis, int32_t vis_dtype, cons
         if (!(chan_freq_hz[c] > 0.0) || !isfinite(chan_freq_hz[c])) { p->err = "bad frequency"; return RICK_ERR_INVALID; }
     const unsigned long long M = (unsigned long long)n_rows * (unsigned long long)n_chan;
     if (M >= 0xFFFFFFFFull) { p->err = "too many visibilities for 32-bit indices"; return RICK_ERR_INVALID; }
-    const unsigned long long n_img = p->d.cube ? (unsigned long long)n_chan : 1ull;
-    const unsigned long long nkeys = n_img * (unsigned long long)p->Nw * (unsigned long long)p->T * p->T;
-    if (nkeys >= 0xFFFFFFFFull) { p->err = "key space exceeds 32 bits (use a larger tile)"; return RICK_ERR_INVALID; }
+    int kb, ib;
+    item_bits(p, n_chan, M, &kb, &ib);
+    if (kb + ib > 64) { p->err = "image x plane x cell key and visibility index do not fit one 64-bit sort item"; return RICK_ERR_INVALID; }
     return RICK_OK;
 }
 
@@ -198,21 +214,18 @@ static int prepare(rick_plan_t* p, const double* chan_freq_hz, int32_t n_chan, i
     p->M = n_rows * (int64_t)n_chan;
     p->n_img = p->d.cube ? n_chan : 1;
     int rc;
+    item_bits(p, n_chan, (unsigned long long)p->M, &p->key_bits, &p->idx_bits);
     if (p->M > p->cap_vis) {
         p->cap_vis = 0;
-        if ((rc = grow(p, &p->keys, (size_t)p->M))) return rc;
-        if ((rc = grow(p, &p->keys_a, (size_t)p->M))) return rc;
-        if ((rc = grow(p, &p->keys_b, (size_t)p->M))) return rc;
-        if ((rc = grow(p, &p->perm_a, (size_t)p->M))) return rc;
-        if ((rc = grow(p, &p->perm_b, (size_t)p->M))) return rc;
+        if ((rc = grow(p, &p->items, (size_t)p->M))) return rc;
+        if ((rc = grow(p, &p->items_a, (size_t)p->M))) return rc;
+        if ((rc = grow(p, &p->items_b, (size_t)p->M))) return rc;
         p->cap_vis = p->M;
     }
-    if (!p->keys) {   // M == 0 on a fresh plan: keep the pointers valid
-        if ((rc = grow(p, &p->keys, 1))) return rc;
-        if ((rc = grow(p, &p->keys_a, 1))) return rc;
-        if ((rc = grow(p, &p->keys_b, 1))) return rc;
-        if ((rc = grow(p, &p->perm_a, 1))) return rc;
-        if ((rc = grow(p, &p->perm_b, 1))) return rc;
+    if (!p->items) {   // M == 0 on a fresh plan: keep the pointers valid
+        if ((rc = grow(p, &p->items, 1))) return rc;
+        if ((rc = grow(p, &p->items_a, 1))) return rc;
+        if ((rc = grow(p, &p->items_b, 1))) return rc;
     }
     const int64_t n_pl = (int64_t)p->n_img * p->Nw + 1;
     if (n_pl > p->plane_start_cap) {
@@ -398,6 +411,11 @@ extern "C" int rick_get_stats(rick_plan_t* p, rick_stats* out)
     return RICK_OK;
 }
 
-extern "C" const uint32_t* rick_debug_keys(rick_plan_t* p) { return (p && p->cap_vis >= 0 && p->keys) ? p->keys : nullptr; }
-extern "C" const uint32_t* rick_debug_perm(rick_plan_t* p) { return p ? p->sorted_perm : nullptr; }
+extern "C" const uint64_t* rick_debug_items(rick_plan_t* p, int32_t sorted, int32_t* idx_bits, int32_t* key_bits)
+{
+    if (!p || !p->items) return nullptr;
+    if (idx_bits) *idx_bits = p->idx_bits;
+    if (key_bits) *key_bits = p->key_bits;
+    return (const uint64_t*)(sorted ? p->sorted_items : p->items);
+}
 extern "C" void* rick_debug_planes(rick_plan_t* p) { return (p && p->state >= 1) ? p->stack : nullptr; }

@@ -98,6 +98,13 @@ int rick_tables_build(rick_plan_t* p)
             for (int k = 0; k < NN; ++k) { mono[k] += cheb[j] * Tn[k]; Tm[k] = Tc[k]; Tc[k] = Tn[k]; }
         }
         for (int k = 0; k < NN; ++k) p->kb_poly[a * NN + k] = (double)mono[k];
+        // g is even: the mirror tap is f_{S-1-a}(s) = f_a(-s) and the centre tap is an even function.
+        // The gridder evaluates only the taps a <= h and uses exactly this symmetry, so impose it on
+        // the table the check below runs on.
+        if (a > h)
+            for (int k = 0; k < NN; ++k) p->kb_poly[a * NN + k] = ((k & 1) ? -1.0 : 1.0) * p->kb_poly[(S - 1 - a) * NN + k];
+        if (a == h)
+            for (int k = 1; k < NN; k += 2) p->kb_poly[a * NN + k] = 0.0;
         // check the double-precision Horner evaluation against the series
         for (int i = 0; i <= 256; ++i) {
             const double sd = -1.0 + (double)i / 128.0;

@@ -23,8 +23,8 @@ RICK_VIS_C64, RICK_VIS_C128 = 0, 1
 
 EXPORTS = ["rick_plan", "rick_plan_destroy", "rick_grid", "rick_fft_wplanes",
            "rick_wcorrect_accumulate", "rick_gridcorrect", "rick_image", "rick_image_host",
-           "rick_get_image", "rick_get_stats", "rick_last_error", "rick_debug_keys",
-           "rick_debug_perm", "rick_debug_planes", "rick_version", "rick_profile",
+           "rick_get_image", "rick_get_stats", "rick_last_error", "rick_debug_items",
+           "rick_debug_planes", "rick_version", "rick_profile",
            "rick_profile_read", "rick_kernel_name"]
 
 
@@ -72,10 +72,8 @@ def load_library():
     L.rick_get_stats.argtypes = [vp, C.POINTER(Stats)]
     L.rick_last_error.argtypes = [vp]
     L.rick_last_error.restype = C.c_char_p
-    L.rick_debug_keys.argtypes = [vp]
-    L.rick_debug_keys.restype = vp
-    L.rick_debug_perm.argtypes = [vp]
-    L.rick_debug_perm.restype = vp
+    L.rick_debug_items.argtypes = [vp, i32, C.POINTER(i32), C.POINTER(i32)]
+    L.rick_debug_items.restype = vp
     L.rick_debug_planes.argtypes = [vp]
     L.rick_debug_planes.restype = vp
     L.rick_version.restype = C.c_char_p
@@ -208,7 +206,7 @@ class Plan:
     def _copy_from(self, ptr, nbytes, dtype, shape):
         if not ptr:
             return None
-        typestr = {torch.int32: "<i4", torch.complex64: "<c8", torch.complex128: "<c16"}[dtype]
+        typestr = {torch.int64: "<i8", torch.complex64: "<c8", torch.complex128: "<c16"}[dtype]
 
         class _View:            # zero-copy view of plan-owned device memory
             __cuda_array_interface__ = {"shape": tuple(shape), "typestr": typestr,
@@ -218,15 +216,28 @@ class Plan:
         assert out.numel() * out.element_size() == nbytes
         return out
 
-    def debug_keys(self) -> Optional[torch.Tensor]:
+    def debug_items(self, sorted_: bool):
+        """(items int64 CUDA tensor [M], idx_bits, key_bits): rick_debug_items (copy, synchronising)."""
         m = self._n_vis
-        return self._copy_from(self._lib.rick_debug_keys(self._h), 4 * m, torch.int32, (m,)) if m else \
-            torch.empty(0, dtype=torch.int32, device="cuda")
+        ib, kb = C.c_int32(), C.c_int32()
+        ptr = self._lib.rick_debug_items(self._h, 1 if sorted_ else 0, C.byref(ib), C.byref(kb))
+        if not m:
+            return torch.empty(0, dtype=torch.int64, device="cuda"), ib.value, kb.value
+        return self._copy_from(ptr, 8 * m, torch.int64, (m,)), ib.value, kb.value
 
-    def debug_perm(self) -> Optional[torch.Tensor]:
-        m = self._n_vis
-        return self._copy_from(self._lib.rick_debug_perm(self._h), 4 * m, torch.int32, (m,)) if m else \
-            torch.empty(0, dtype=torch.int32, device="cuda")
+    def debug_keys(self) -> np.ndarray:
+        """[M] uint64 keys in visibility order; a dropped visibility reads as all ones (64 bits)."""
+        items, ib, kb = self.debug_items(False)
+        it = items.cpu().numpy().view(np.uint64)
+        assert np.array_equal(it & np.uint64((1 << ib) - 1), np.arange(it.shape[0], dtype=np.uint64))
+        key = it >> np.uint64(ib)
+        key[key == np.uint64((1 << kb) - 1)] = np.uint64(0xFFFFFFFFFFFFFFFF)
+        return key
+
+    def debug_perm(self) -> np.ndarray:
+        """[M] uint32: visibility index at every sorted position."""
+        items, ib, _ = self.debug_items(True)
+        return (items.cpu().numpy().view(np.uint64) & np.uint64((1 << ib) - 1)).astype(np.uint32)
 
     def debug_planes(self) -> Optional[torch.Tensor]:
         dt = torch.complex64 if self.f32 else torch.complex128

@@ -39,8 +39,8 @@ def _staged(wl, tile=0):
     vis, uvw, wgt = rick.to_device(wl)
     out = {}
     plan.rick_grid(vis, uvw, wgt, wl.freq_hz)
-    out["keys"] = plan.debug_keys().cpu().numpy().view(np.uint32)
-    out["perm"] = plan.debug_perm().cpu().numpy().view(np.uint32)
+    out["keys"] = plan.debug_keys()
+    out["perm"] = plan.debug_perm()
     out["grid"] = plan.debug_planes().cpu().numpy()
     plan.rick_fft_wplanes()
     out["fft"] = plan.debug_planes().cpu().numpy()
@@ -188,8 +188,8 @@ def test_cube_mode():
     vis, uvw, wgt = rick.to_device(wl)
     plan = rick.plan_from_workload(wl)
     cube = plan.rick_image(vis, uvw, wgt, wl.freq_hz).cpu().numpy()
-    keys = plan.debug_keys().cpu().numpy().view(np.uint32)
-    perm = plan.debug_perm().cpu().numpy().view(np.uint32)
+    keys = plan.debug_keys()
+    perm = plan.debug_perm()
     plan.destroy()
     o = _oracle(wl)
     assert cube.shape == (5, wl.n, wl.n)
