@@ -35,6 +35,9 @@ struct rick_plan_s {
     int batch;               // resident planes
     double beta, dl, inv_du;
     cudaStream_t stream;
+    cudaStream_t stream2;    // low-priority side stream: the zero-fill runs beside index + sort
+    cudaStream_t stream3;    // copy stream of rick_image_host (visibilities in, image parts out)
+    cudaEvent_t ev_fork, ev_join, ev_vis, ev_part;
     int n_sm;
     int state;               // 0 idle, 1 gridded, 2 transformed, 3 corrected, 4 tapered
     std::string err;
@@ -102,15 +105,16 @@ enum { RK_TABLES = 0, RK_RESET, RK_WRANGE, RK_INDEX_KEY, RK_RADIX_HIST, RK_SCAN,
        RK_PLANE_STARTS, RK_ZERO, RK_GRID, RK_FFT_ROWS, RK_FFT_COLS, RK_WCORRECT, RK_TAPER, RK_COLS_WCORRECT,
        RK_NKERNELS };
 
-void rick_prof_begin(rick_plan_t* p, int id);   // plan.cu; no-ops unless profiling is on
-void rick_prof_end(rick_plan_t* p);
+void rick_prof_begin(rick_plan_t* p, int id, cudaStream_t st);   // plan.cu; no-ops unless profiling is on
+void rick_prof_end(rick_plan_t* p, cudaStream_t st);
 
 // launch one kernel: optional CUDA-event bracket, launch counter, launch-error check
-#define RICK_KERNEL(p, id, ...)                                                        \
+#define RICK_KERNEL(p, id, ...) RICK_KERNEL_ON(p, (p)->stream, id, __VA_ARGS__)
+#define RICK_KERNEL_ON(p, st, id, ...)                                                 \
     do {                                                                               \
-        rick_prof_begin((p), (id));                                                    \
+        rick_prof_begin((p), (id), (st));                                              \
         __VA_ARGS__;                                                                   \
-        rick_prof_end((p));                                                            \
+        rick_prof_end((p), (st));                                                      \
         RICK_LAUNCHED(p);                                                              \
     } while (0)
 
@@ -127,7 +131,7 @@ void rick_prof_end(rick_plan_t* p);
 // stage entry points (each enqueues on p->stream)
 int rick_tables_build(rick_plan_t* p);                                   // tables.cu
 int rick_index_sort(rick_plan_t* p, const double* uvw_m, const float* weights);   // index_sort.cu
-int rick_zero_planes(rick_plan_t* p, int n_planes);                      // grid.cu
+int rick_zero_planes(rick_plan_t* p, int n_planes, cudaStream_t st);      // grid.cu
 int rick_grid_planes(rick_plan_t* p, const void* vis, int vis_dtype, const double* uvw_m,
                      const float* weights, int plane_first, int n_planes);      // grid.cu
 int rick_fft_planes(rick_plan_t* p, int n_planes);                       // fft.cu: rows then columns
@@ -136,7 +140,8 @@ int rick_fft_cols(rick_plan_t* p, int n_planes);                         // fft.
 int rick_cols12_init(rick_plan_t* p);                                    // fft_cols12.cu
 int rick_cols12_fft(rick_plan_t* p, int n_planes);                       // fft_cols12.cu
 int rick_cols12_wcorrect(rick_plan_t* p, int img, int z_first, int n_planes, double* image,
-                         int accumulate, int fuse_taper);                // fft_cols12.cu
+                         int accumulate, int fuse_taper, int strip_begin, int strip_end);   // fft_cols12.cu
+int rick_cols12_strips(void);                                            // fft_cols12.cu
 int rick_wcorrect(rick_plan_t* p, int img, int z_first, int n_planes, double* image,
                   int accumulate, int fuse_taper);                     // wcorrect.cu
 int rick_taper_divide(rick_plan_t* p, double* image);                    // wcorrect.cu

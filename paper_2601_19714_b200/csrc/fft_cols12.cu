@@ -111,7 +111,7 @@ k_cols12_fft(const __grid_constant__ CUtensorMap tmap, double2* __restrict__ sta
 __global__ void __launch_bounds__(C12_THREADS, 1)
 k_cols12_wcorrect(const __grid_constant__ CUtensorMap tmap, const double2* __restrict__ tw, int n_planes,
                   int z_first, double dl, const WRange* __restrict__ wr, double* __restrict__ image,
-                  int accumulate, const double* __restrict__ taper)
+                  int accumulate, const double* __restrict__ taper, int strip_begin, int strip_end)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double2* stg = reinterpret_cast<double2*>(smem_raw);
@@ -132,15 +132,15 @@ k_cols12_wcorrect(const __grid_constant__ CUtensorMap tmap, const double2* __res
     const uint32_t tS = tbase + ((uint32_t)(32 * (R.w & 3)) << 16) + (uint32_t)((R.w >> 2) * 128);
     const uint32_t tStep = tS + 64;
 
-    int strip = blockIdx.x;
-    if (threadIdx.x == 0 && strip < C12_STRIPS) {
+    int strip = strip_begin + (int)blockIdx.x;
+    if (threadIdx.x == 0 && strip < strip_end) {
         mbar_arrive_expect_tx(bar, C12_STAGE_BYTES);
         tma_load_5d(stg, &tmap, bar, 4 * strip, 0, 0, 0, n_planes - 1);
     }
     uint32_t parity = 0;
     const double dw = wr->dw;
     const double w_first = wr->w_min + ((double)z_first + 0.5) * dw;
-    for (; strip < C12_STRIPS; strip += gridDim.x) {
+    for (; strip < strip_end; strip += gridDim.x) {
         const int p = strip * C12_WC + R.c;
         const double l = (double)(p - C12_N / 2) * dl;
         // step = exp(2 pi i dw (n-1)) of this thread's 16 pixels (rows t3 + 256 ((e+8)&15)) -> TMEM
@@ -163,7 +163,7 @@ k_cols12_wcorrect(const __grid_constant__ CUtensorMap tmap, const double2* __res
         }
         tmem_wait_st();
         for (int plane = n_planes - 1; plane >= 0; --plane) {
-            const bool more = plane > 0 || strip + (int)gridDim.x < C12_STRIPS;
+            const bool more = plane > 0 || strip + (int)gridDim.x < strip_end;
             double2 v[16];
             strip_fft(v, R, stg, ex, tw, bar, parity, more, &tmap, plane > 0 ? strip : strip + (int)gridDim.x,
                       plane > 0 ? plane - 1 : n_planes - 1);
@@ -273,12 +273,20 @@ int rick_cols12_fft(rick_plan_t* p, int n_planes)
     return RICK_OK;
 }
 
+// strips [strip_begin, strip_end) only (columns 2 strip_begin .. 2 strip_end - 1 of the image); the
+// whole image is strips 0 .. 2047.  rick_image_host launches the pass in a few parts (each a whole
+// number of rounds of the persistent grid) so that the device -> host copy of one part runs under the
+// next part's kernel.
 int rick_cols12_wcorrect(rick_plan_t* p, int img, int z_first, int n_planes, double* image, int accumulate,
-                         int fuse_taper)
+                         int fuse_taper, int strip_begin, int strip_end)
 {
+    if (strip_end <= strip_begin) return RICK_OK;
     const CUtensorMap tm = *reinterpret_cast<const CUtensorMap*>(p->cols12_tmap);
-    RICK_KERNEL(p, RK_COLS_WCORRECT, k_cols12_wcorrect<<<p->n_sm, C12_THREADS, C12_SMEM, p->stream>>>(
+    const int n = strip_end - strip_begin;
+    RICK_KERNEL(p, RK_COLS_WCORRECT, k_cols12_wcorrect<<<n < p->n_sm ? n : p->n_sm, C12_THREADS, C12_SMEM, p->stream>>>(
         tm, (const double2*)p->twiddle, n_planes, z_first, p->dl, p->wrange + img, image, accumulate,
-        fuse_taper ? p->taper : nullptr));
+        fuse_taper ? p->taper : nullptr, strip_begin, strip_end));
     return RICK_OK;
 }
+
+int rick_cols12_strips(void) { return C12_STRIPS; }

@@ -20,7 +20,7 @@ static const char* const k_names[RK_NKERNELS] = {
     "tables", "reset", "wrange", "index_key", "radix_hist", "scan", "radix_scatter", "plane_starts",
     "zero", "grid", "fft_rows", "fft_cols", "wcorrect", "taper", "fft_cols_wcorrect"};
 
-void rick_prof_begin(rick_plan_t* p, int id)
+void rick_prof_begin(rick_plan_t* p, int id, cudaStream_t st)
 {
     if (!p->prof_on) return;
     if (p->prof_ev.size() < 2 * (p->prof_n + 1)) {
@@ -30,19 +30,20 @@ void rick_prof_begin(rick_plan_t* p, int id)
         p->prof_ev.push_back(b);
     }
     if (p->prof_id.size() <= p->prof_n) p->prof_id.push_back(id); else p->prof_id[p->prof_n] = id;
-    cudaEventRecord(p->prof_ev[2 * p->prof_n], p->stream);
+    cudaEventRecord(p->prof_ev[2 * p->prof_n], st);
 }
 
-void rick_prof_end(rick_plan_t* p)
+void rick_prof_end(rick_plan_t* p, cudaStream_t st)
 {
     if (!p->prof_on) return;
-    cudaEventRecord(p->prof_ev[2 * p->prof_n + 1], p->stream);
+    cudaEventRecord(p->prof_ev[2 * p->prof_n + 1], st);
     p->prof_n++;
 }
 
 static void prof_collect(rick_plan_t* p)
 {
     cudaStreamSynchronize(p->stream);
+    if (p->stream2) cudaStreamSynchronize(p->stream2);
     for (size_t i = 0; i < p->prof_n; ++i) {
         float ms = 0.f;
         if (cudaEventElapsedTime(&ms, p->prof_ev[2 * i], p->prof_ev[2 * i + 1]) == cudaSuccess) {
@@ -94,6 +95,12 @@ extern "C" int rick_plan_destroy(rick_plan_t* p)
     for (cudaEvent_t e : p->prof_ev) cudaEventDestroy(e);
     if (p->h_scale) cudaFreeHost(p->h_scale);
     if (p->ev_scale) cudaEventDestroy(p->ev_scale);
+    if (p->stream2) { cudaStreamSynchronize(p->stream2); cudaStreamDestroy(p->stream2); }
+    if (p->ev_fork) cudaEventDestroy(p->ev_fork);
+    if (p->ev_join) cudaEventDestroy(p->ev_join);
+    if (p->stream3) { cudaStreamSynchronize(p->stream3); cudaStreamDestroy(p->stream3); }
+    if (p->ev_vis) cudaEventDestroy(p->ev_vis);
+    if (p->ev_part) cudaEventDestroy(p->ev_part);
     delete p;
     return RICK_OK;
 }
@@ -109,6 +116,16 @@ static int plan_init(rick_plan_t* p)
     RICK_CUDA(p, cudaMalloc(&p->image, sizeof(double) * (size_t)p->N * p->N));
     RICK_CUDA(p, cudaMallocHost(&p->h_scale, sizeof(double) * RICK_MAX_CHAN));
     RICK_CUDA(p, cudaEventCreateWithFlags(&p->ev_scale, cudaEventDisableTiming));
+    {
+        int lo = 0, hi = 0;
+        RICK_CUDA(p, cudaDeviceGetStreamPriorityRange(&lo, &hi));      // lo = least priority
+        RICK_CUDA(p, cudaStreamCreateWithPriority(&p->stream2, cudaStreamNonBlocking, lo));
+        RICK_CUDA(p, cudaEventCreateWithFlags(&p->ev_fork, cudaEventDisableTiming));
+        RICK_CUDA(p, cudaEventCreateWithFlags(&p->ev_join, cudaEventDisableTiming));
+        RICK_CUDA(p, cudaStreamCreateWithFlags(&p->stream3, cudaStreamNonBlocking));
+        RICK_CUDA(p, cudaEventCreateWithFlags(&p->ev_vis, cudaEventDisableTiming));
+        RICK_CUDA(p, cudaEventCreateWithFlags(&p->ev_part, cudaEventDisableTiming));
+    }
     RICK_CUDA(p, cudaMalloc(&p->counters, sizeof(DevCounters)));
     RICK_CUDA(p, cudaMemsetAsync(p->counters, 0, sizeof(DevCounters), p->stream));
     const int rc = rick_tables_build(p);
@@ -251,6 +268,20 @@ static int prepare(rick_plan_t* p, const double* chan_freq_hz, int32_t n_chan, i
     return RICK_OK;
 }
 
+// a0..a2 on the plan's stream while the zero-fill of the first plane batch runs on the side stream
+// (it needs nothing from the sort, only that earlier readers of the stack are done); joined before a3.
+static int sort_and_zero(rick_plan_t* p, const double* uvw_m, const float* weights, int n_planes_first)
+{
+    int rc;
+    RICK_CUDA(p, cudaEventRecord(p->ev_fork, p->stream));
+    RICK_CUDA(p, cudaStreamWaitEvent(p->stream2, p->ev_fork, 0));
+    if ((rc = rick_zero_planes(p, n_planes_first, p->stream2))) return rc;
+    RICK_CUDA(p, cudaEventRecord(p->ev_join, p->stream2));
+    if ((rc = rick_index_sort(p, uvw_m, weights))) return rc;
+    RICK_CUDA(p, cudaStreamWaitEvent(p->stream, p->ev_join, 0));
+    return RICK_OK;
+}
+
 extern "C" int rick_grid(rick_plan_t* p, const void* vis, int32_t vis_dtype, const double* uvw_m,
                          const float* weights, const double* chan_freq_hz, int32_t n_chan, int64_t n_rows)
 {
@@ -261,8 +292,7 @@ extern "C" int rick_grid(rick_plan_t* p, const void* vis, int32_t vis_dtype, con
     if (rc) return rc;
     p->state = 0;
     if ((rc = prepare(p, chan_freq_hz, n_chan, n_rows))) return rc;
-    if ((rc = rick_index_sort(p, uvw_m, weights))) return rc;
-    if ((rc = rick_zero_planes(p, p->Nw))) return rc;
+    if ((rc = sort_and_zero(p, uvw_m, weights, p->Nw))) return rc;
     if ((rc = rick_grid_planes(p, vis, vis_dtype, uvw_m, weights, 0, p->Nw))) return rc;
     p->state = 1;
     return RICK_OK;
@@ -301,29 +331,51 @@ extern "C" int rick_gridcorrect(rick_plan_t* p)
     return RICK_OK;
 }
 
-extern "C" int rick_image(rick_plan_t* p, const void* vis, int32_t vis_dtype, const double* uvw_m,
-                          const float* weights, const double* chan_freq_hz, int32_t n_chan,
-                          int64_t n_rows, double* image_out)
+// a0..a6.  vis_ready (may be null): event the gridder must wait for (visibilities still being copied
+// by rick_image_host).  host_out (may be null; cube = 0 only): the image goes to HOST memory, part by
+// part on the copy stream while the next part of the last pass is still running.
+static int image_impl(rick_plan_t* p, const void* vis, int32_t vis_dtype, const double* uvw_m,
+                      const float* weights, const double* chan_freq_hz, int32_t n_chan,
+                      int64_t n_rows, double* image_out, cudaEvent_t vis_ready, double* host_out)
 {
-    if (!p) return RICK_ERR_INVALID;
-    p->err.clear();
     int rc = check_inputs(p, vis, vis_dtype, uvw_m, chan_freq_hz, n_chan, n_rows);
     if (rc) return rc;
     if (p->d.cube && !image_out) { p->err = "cube mode needs image_out"; return RICK_ERR_INVALID; }
     p->state = 0;
     if ((rc = prepare(p, chan_freq_hz, n_chan, n_rows))) return rc;
-    if ((rc = rick_index_sort(p, uvw_m, weights))) return rc;
+    if ((rc = sort_and_zero(p, uvw_m, weights, p->Nw < p->batch ? p->Nw : p->batch))) return rc;
+    if (vis_ready) RICK_CUDA(p, cudaStreamWaitEvent(p->stream, vis_ready, 0));
     const size_t NN = (size_t)p->N * p->N;
+    bool host_done = false;
     for (int img = 0; img < p->n_img; ++img) {
         double* dst = p->d.cube ? image_out + (size_t)img * NN : p->image;
         for (int z0 = 0; z0 < p->Nw; z0 += p->batch) {
             const int nb = p->Nw - z0 < p->batch ? p->Nw - z0 : p->batch;
             const int last = z0 + nb >= p->Nw;
-            if ((rc = rick_zero_planes(p, nb))) return rc;
+            if ((img > 0 || z0 > 0) && (rc = rick_zero_planes(p, nb, p->stream))) return rc;
             if ((rc = rick_grid_planes(p, vis, vis_dtype, uvw_m, weights, img * p->Nw + z0, nb))) return rc;
             if (p->cols12_ok) {   // column pass fused with the w-correction: the transformed planes are never written
                 if ((rc = rick_fft_rows(p, nb))) return rc;
-                if ((rc = rick_cols12_wcorrect(p, img, z0, nb, dst, z0 > 0, last))) return rc;
+                const int strips = rick_cols12_strips();
+                if (host_out && last && !p->d.cube) {
+                    // whole rounds of the persistent grid per part: 4 + 4 + 3 + rest rounds of n_sm strips
+                    const int rounds[4] = {4, 4, 3, 1 << 20};
+                    int s0 = 0;
+                    for (int k = 0; k < 4 && s0 < strips; ++k) {
+                        long long s1 = (long long)s0 + (long long)rounds[k] * p->n_sm;
+                        if (s1 > strips) s1 = strips;
+                        if ((rc = rick_cols12_wcorrect(p, img, z0, nb, dst, z0 > 0, last, s0, (int)s1))) return rc;
+                        RICK_CUDA(p, cudaEventRecord(p->ev_part, p->stream));
+                        RICK_CUDA(p, cudaStreamWaitEvent(p->stream3, p->ev_part, 0));
+                        const size_t c0 = 2 * (size_t)s0, nc = 2 * (size_t)(s1 - s0);
+                        RICK_CUDA(p, cudaMemcpy2DAsync(host_out + c0, sizeof(double) * p->N, dst + c0, sizeof(double) * p->N,
+                                                       sizeof(double) * nc, (size_t)p->N, cudaMemcpyDeviceToHost, p->stream3));
+                        s0 = (int)s1;
+                    }
+                    host_done = true;
+                } else {
+                    if ((rc = rick_cols12_wcorrect(p, img, z0, nb, dst, z0 > 0, last, 0, strips))) return rc;
+                }
             } else {
                 if ((rc = rick_fft_planes(p, nb))) return rc;
                 if ((rc = rick_wcorrect(p, img, z0, nb, dst, z0 > 0, last))) return rc;
@@ -336,7 +388,21 @@ extern "C" int rick_image(rick_plan_t* p, const void* vis, int32_t vis_dtype, co
         // the staged state machine may continue only if the whole stack is what is resident
         p->state = 4;
     }
+    if (host_out && !host_done) {
+        const size_t n_img = p->d.cube ? (size_t)n_chan : 1;
+        RICK_CUDA(p, cudaMemcpyAsync(host_out, p->d.cube ? image_out : p->image, sizeof(double) * NN * n_img,
+                                     cudaMemcpyDeviceToHost, p->stream));
+    }
     return RICK_OK;
+}
+
+extern "C" int rick_image(rick_plan_t* p, const void* vis, int32_t vis_dtype, const double* uvw_m,
+                          const float* weights, const double* chan_freq_hz, int32_t n_chan,
+                          int64_t n_rows, double* image_out)
+{
+    if (!p) return RICK_ERR_INVALID;
+    p->err.clear();
+    return image_impl(p, vis, vis_dtype, uvw_m, weights, chan_freq_hz, n_chan, n_rows, image_out, nullptr, nullptr);
 }
 
 template <typename Tp> static int ensure_bytes(rick_plan_t* p, Tp** buf, size_t* cap, size_t bytes)
@@ -366,18 +432,23 @@ extern "C" int rick_image_host(rick_plan_t* p, const void* vis_host, int32_t vis
     if ((rc = ensure_bytes(p, &p->st_vis, &p->st_vis_cap, vis_bytes))) return rc;
     if ((rc = ensure_bytes(p, &p->st_uvw, &p->st_uvw_cap, sizeof(double) * 3 * (size_t)n_rows))) return rc;
     if (weights_host && (rc = ensure_bytes(p, &p->st_wgt, &p->st_wgt_cap, sizeof(float) * M))) return rc;
-    if ((rc = ensure_bytes(p, &p->st_img, &p->st_img_cap, sizeof(double) * NN * n_img))) return rc;
+    if (p->d.cube && (rc = ensure_bytes(p, &p->st_img, &p->st_img_cap, sizeof(double) * NN * n_img))) return rc;
+    // uvw first on the plan's stream (a0..a2 need nothing else); the visibilities follow on the copy
+    // stream and land while index + sort + zero-fill run; the gridder waits for ev_vis.
     if (M) {
-        RICK_CUDA(p, cudaMemcpyAsync(p->st_vis, vis_host, vis_bytes, cudaMemcpyHostToDevice, p->stream));
         RICK_CUDA(p, cudaMemcpyAsync(p->st_uvw, uvw_m_host, sizeof(double) * 3 * (size_t)n_rows, cudaMemcpyHostToDevice, p->stream));
+        RICK_CUDA(p, cudaEventRecord(p->ev_fork, p->stream));
+        RICK_CUDA(p, cudaStreamWaitEvent(p->stream3, p->ev_fork, 0));
+        RICK_CUDA(p, cudaMemcpyAsync(p->st_vis, vis_host, vis_bytes, cudaMemcpyHostToDevice, p->stream3));
         if (weights_host)
-            RICK_CUDA(p, cudaMemcpyAsync(p->st_wgt, weights_host, sizeof(float) * M, cudaMemcpyHostToDevice, p->stream));
+            RICK_CUDA(p, cudaMemcpyAsync(p->st_wgt, weights_host, sizeof(float) * M, cudaMemcpyHostToDevice, p->stream3));
+        RICK_CUDA(p, cudaEventRecord(p->ev_vis, p->stream3));
     }
-    rc = rick_image(p, p->st_vis, vis_dtype, p->st_uvw, weights_host ? p->st_wgt : nullptr, chan_freq_hz,
-                    n_chan, n_rows, p->st_img);
+    rc = image_impl(p, p->st_vis, vis_dtype, p->st_uvw, weights_host ? p->st_wgt : nullptr, chan_freq_hz,
+                    n_chan, n_rows, p->d.cube ? p->st_img : nullptr, M ? p->ev_vis : nullptr, image_out_host);
     if (rc) return rc;
-    RICK_CUDA(p, cudaMemcpyAsync(image_out_host, p->st_img, sizeof(double) * NN * n_img, cudaMemcpyDeviceToHost, p->stream));
     RICK_CUDA(p, cudaStreamSynchronize(p->stream));
+    RICK_CUDA(p, cudaStreamSynchronize(p->stream3));
     return RICK_OK;
 }
 

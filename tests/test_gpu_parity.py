@@ -130,6 +130,19 @@ def test_n4096_tma_tmem_column_kernels():
         e = _rel(img, o["image"])
         print(f"N=4096 fused rick_image plane_batch={pb}: rel L2 {e:.2e}")
         assert e <= TOL64 and _rel(img2, o["image"]) <= TOL64
+    # host-buffer entry at N = 4096: visibilities copied under index + sort, the image returned part by
+    # part (whole rounds of the persistent column kernel) on the copy stream
+    import torch
+    plan = rick.plan_from_workload(wl)
+    hv = torch.from_numpy(wl.vis).pin_memory()
+    hu = torch.from_numpy(wl.uvw_m).pin_memory()
+    hout = torch.full((wl.n, wl.n), float("nan"), dtype=torch.float64).pin_memory()
+    plan.rick_image_host(hv, hu, None, wl.freq_hz, hout)
+    assert _rel(hout.numpy(), o["image"]) <= TOL64
+    hout.fill_(float("nan"))
+    plan.rick_image_host(hv, hu, None, wl.freq_hz, hout)          # staging reuse
+    assert _rel(hout.numpy(), o["image"]) <= TOL64
+    plan.destroy()
     # one plane only (Horner degenerates to S = P_0)
     wl1 = synth.make_config(2, n_times=2, n_wplanes=1, n_src=4)
     plan = rick.plan_from_workload(wl1)
