@@ -1,0 +1,118 @@
+"""GPU parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times
+(rick_image on device buffers, the plan as plan_from_workload builds it).
+
+The CPU oracle finishes these in tens of seconds on the GPU box's host cores, so the whole
+image is compared element by element where the config allows it:
+
+  configs[1] MeerKAT-like  4096^2 x 32 planes fp64, 16.5M vis: whole image + keys + permutation + stats
+  configs[2] LOFAR-like    8192^2 x 64 planes fp64, 14.5M vis: whole image + stats
+  configs[3] large-pixel   16384^2 x 32 planes fp32 grid, streamed plane batches: the "rows r mod 16 = 0"
+                           subset (BASELINE.json: 1/16 visibility subset) through both sides, whole image
+  configs[4] cube          4096^2 x 16 planes x 128 channels: the GPU images the full 66M-visibility cube;
+                           the oracle images channels {0, 1, 63, 64, 126, 127} + two seeded picks, one at
+                           a time (a cube channel is an independent single-channel problem, reading R16)
+
+Bars (north_star): relative L2 <= 1e-10 (fp64 grid) / <= 1e-4 (fp32 grid); integer work bit-exact.
+"""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2601_19714_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+TOL64, TOL32 = 1e-10, 1e-4
+
+
+def _rel(a, b):
+    nb = np.linalg.norm(np.asarray(b).ravel())
+    return np.linalg.norm((np.asarray(a) - np.asarray(b)).ravel()) / (nb if nb > 0 else 1.0)
+
+
+def _rick():
+    import torch
+    assert torch.cuda.is_available(), "these tests need the B200"
+    from paper_2601_19714_b200 import rick
+    return rick
+
+
+def _gpu_image(wl, **over):
+    """(plan, image as a CUDA tensor, stats) of one rick_image call on device buffers."""
+    rick = _rick()
+    plan = rick.plan_from_workload(wl, **over)
+    vis, uvw, wgt = rick.to_device(wl)
+    img = plan.rick_image(vis, uvw, wgt, wl.freq_hz)
+    st = plan.rick_get_stats()
+    return plan, img, st
+
+
+def _report(name, img, ref):
+    N = ref.shape[-1]
+    inner = slice(N // 4, 3 * N // 4)
+    pk = np.unravel_index(np.argmax(np.abs(ref)), ref.shape)
+    e, ei = _rel(img, ref), _rel(img[..., inner, inner], ref[..., inner, inner])
+    print(f"{name}: rel L2 {e:.3e} (inner half {ei:.3e}); peak pixel {pk} oracle {ref[pk]:.9e} gpu {img[pk]:.9e}")
+    return e
+
+
+def _stats_equal(st, so):
+    assert st["n_vis"] == so["n_vis"] and st["n_gridded"] == so["n_gridded"] and st["n_dropped"] == so["n_dropped"]
+    assert st["w_min"] == so["w_min"] and st["w_max"] == so["w_max"]
+    assert abs(st["sum_w"] - so["sum_w"]) <= 1e-9 * max(1.0, so["sum_w"])
+
+
+def test_cfg2_full_meerkat_whole_image_keys_perm():
+    wl = synth.make_config(2, device="cuda")
+    assert wl.n_vis == 16515072 and wl.n == 4096 and wl.n_wplanes == 32
+    plan, img, st = _gpu_image(wl)
+    keys, perm = plan.debug_keys(), plan.debug_perm()
+    plan.destroy()
+    o = oracle.image(wl.uvw_m, wl.freq_hz, wl.vis, None, wl.n, wl.n_wplanes, wl.support, wl.pixel_rad)
+    _stats_equal(st, o["stats"])
+    idx = oracle.index(wl.uvw_m, wl.freq_hz, wl.n, wl.n_wplanes, wl.support, wl.pixel_rad, 16)
+    assert np.array_equal(keys, idx["key"])                        # bit-exact
+    assert np.array_equal(perm, oracle.sort(idx["key"]))           # bit-exact, stable
+    assert _report("cfg2 full", img.cpu().numpy(), o["image"]) <= TOL64
+
+
+def test_cfg3_full_lofar_whole_image():
+    wl = synth.make_config(3, device="cuda")
+    assert wl.n_vis == 14499840 and wl.n == 8192 and wl.n_wplanes == 64
+    plan, img, st = _gpu_image(wl)
+    plan.destroy()
+    o = oracle.image(wl.uvw_m, wl.freq_hz, wl.vis, None, wl.n, wl.n_wplanes, wl.support, wl.pixel_rad)
+    _stats_equal(st, o["stats"])
+    assert o["stats"]["n_dropped"] > 0
+    assert _report("cfg3 full", img.cpu().numpy(), o["image"]) <= TOL64
+
+
+def test_cfg4_full_grid_fp32_subset_rows_mod16():
+    import dataclasses
+    full = synth.make_config(4, device="cuda")
+    assert full.n_vis == 66060288 and full.n == 16384 and full.grid_prec == "f32" and full.plane_batch == 8
+    wl = dataclasses.replace(full, uvw_m=np.ascontiguousarray(full.uvw_m[::16]),
+                             vis=np.ascontiguousarray(full.vis[::16]))
+    del full
+    plan, img, st = _gpu_image(wl)
+    plan.destroy()
+    o = oracle.image(wl.uvw_m, wl.freq_hz, wl.vis, None, wl.n, wl.n_wplanes, wl.support, wl.pixel_rad)
+    _stats_equal(st, o["stats"])
+    assert _report("cfg4 (rows mod 16 = 0, fp32 grid, 4 plane batches)", img.cpu().numpy(), o["image"]) <= TOL32
+
+
+def test_cfg5_full_cube_sampled_channels():
+    wl = synth.make_config(5, device="cuda")
+    assert wl.n_vis == 66060288 and wl.n_chan == 128 and wl.cube == 1
+    plan, cube, st = _gpu_image(wl)
+    plan.destroy()
+    assert tuple(cube.shape) == (128, wl.n, wl.n) and st["n_vis"] == wl.n_vis
+    rng = np.random.Generator(np.random.PCG64(5))
+    chans = [0, 1, 63, 64, 126, 127] + sorted(int(c) for c in rng.choice(np.arange(2, 126), 2, replace=False))
+    n_gridded = 0
+    for c in chans:
+        o = oracle.image(wl.uvw_m, wl.freq_hz[c:c + 1], np.ascontiguousarray(wl.vis[:, c:c + 1]), None,
+                         wl.n, wl.n_wplanes, wl.support, wl.pixel_rad)
+        assert _report(f"cfg5 channel {c}", cube[c].cpu().numpy(), o["image"]) <= TOL64
+        n_gridded += o["stats"]["n_gridded"]
+    assert st["n_gridded"] + st["n_dropped"] == wl.n_vis and st["n_gridded"] >= n_gridded
