@@ -154,7 +154,7 @@ def main():
         return sum(prof[n][0] for n in names if n in prof) / args.steps
     fused = ms_of("fft_cols_wcorrect") > 0
     t_sortgrid = ms_of("reset", "wrange", "index_key", "radix_hist", "scan", "radix_scatter", "plane_starts",
-                       "zero", "grid")
+                       "zero", "grid", "row_occupancy")
     stages = {
         "grid_mvis_s_a0_a3": n_gridded / (t_sortgrid * 1e-3) / 1e6 if t_sortgrid else None,
         "grid_kernel_mvis_s": n_gridded / (ms_of("grid") * 1e-3) / 1e6 if ms_of("grid") else None,
@@ -174,7 +174,10 @@ def main():
     alg_bytes = {"fft_rows": 2 * stack_bytes, "fft_cols": 2 * stack_bytes, "zero": stack_bytes,
                  "wcorrect": stack_bytes + image_bytes, "fft_cols_wcorrect": stack_bytes + image_bytes}
     dom = max((k for k in prof if prof[k][1]), key=lambda k: prof[k][0])
-    traffic_ncu = {"fft_rows": None, "fft_cols": None}      # filled from profiles/ when captured
+    # dram__bytes_read.sum + dram__bytes_write.sum per launch, from profiles/r1b_ncu_full.md (configs[1] only)
+    traffic_ncu = {}
+    if args.config == 2 and not args.small:
+        traffic_ncu = {"fft_rows": 17.120e9, "fft_cols_wcorrect": 8.889e9, "grid": 0.816e9}
     if dom in alg_bytes:
         avg_ms = prof[dom][0] / prof[dom][1]
         ach = alg_bytes[dom] / (avg_ms * 1e-3) / 1e9
@@ -187,7 +190,7 @@ def main():
         ach = n_gridded * S2 * 2 / (avg_ms * 1e-3) / 1e9            # G scalar accumulations / s
         peak = 148 * 1.965 * 16.0                                    # 16 fp64 RMW / clk / SM (128 B/clk smem)
         roofline = {"kernel": dom, "bound": "alu", "achieved": ach, "peak": peak, "unit": "Gacc/s",
-                    "frac": ach / peak, "traffic": None, "avg_launch_ms": avg_ms}
+                    "frac": ach / peak, "traffic": traffic_ncu.get(dom), "avg_launch_ms": avg_ms}
     roofline["share_of_step"] = prof[dom][0] / args.steps / ms_per_step
 
     # end to end through the public host-buffer call: pinned host inputs, image read back

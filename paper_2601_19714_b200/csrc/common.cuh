@@ -63,6 +63,12 @@ struct rick_plan_s {
     uint32_t* scan_tmp; size_t scan_cap;
     int64_t* plane_start;    // [n_planes_total + 1] offsets into the sorted order
     int64_t plane_start_cap;
+    // row occupancy: row_occ[pg][row] = 1 when some visibility of global
+    // plane pg has row in its footprint band (tile-row granularity), rebuilt by every sort;
+    // row_dirty[slot][row] = 1 when that row of the resident slot may hold non-zero data.  Rows that
+    // are neither are zero in HBM and stay untouched by zero-fill, gridder and the row pass.
+    unsigned char* row_occ; size_t row_occ_cap;
+    unsigned char* row_dirty;
     double* chan_scale;      // [C] device, s_c = f_c / c0
     WRange* wrange;          // [n_img] device
     int chan_cap;
@@ -103,7 +109,7 @@ struct rick_plan_s {
 // kernel classes for rick_profile_read / rick_kernel_name
 enum { RK_TABLES = 0, RK_RESET, RK_WRANGE, RK_INDEX_KEY, RK_RADIX_HIST, RK_SCAN, RK_RADIX_SCATTER,
        RK_PLANE_STARTS, RK_ZERO, RK_GRID, RK_FFT_ROWS, RK_FFT_COLS, RK_WCORRECT, RK_TAPER, RK_COLS_WCORRECT,
-       RK_NKERNELS };
+       RK_ROW_OCC, RK_NKERNELS };
 
 void rick_prof_begin(rick_plan_t* p, int id, cudaStream_t st);   // plan.cu; no-ops unless profiling is on
 void rick_prof_end(rick_plan_t* p, cudaStream_t st);
@@ -131,11 +137,13 @@ void rick_prof_end(rick_plan_t* p, cudaStream_t st);
 // stage entry points (each enqueues on p->stream)
 int rick_tables_build(rick_plan_t* p);                                   // tables.cu
 int rick_index_sort(rick_plan_t* p, const double* uvw_m, const float* weights);   // index_sort.cu
-int rick_zero_planes(rick_plan_t* p, int n_planes, cudaStream_t st);      // grid.cu
+int rick_zero_dirty(rick_plan_t* p, int n_slots, cudaStream_t st);        // grid.cu: zero the dirty rows of slots 0..n_slots-1
+int rick_mark_dirty(rick_plan_t* p, int plane_first, int n_planes);      // grid.cu: dirty |= occupancy of the batch
+int rick_all_dirty(rick_plan_t* p, int n_slots);                         // grid.cu: after an in-place column pass
 int rick_grid_planes(rick_plan_t* p, const void* vis, int vis_dtype, const double* uvw_m,
                      const float* weights, int plane_first, int n_planes);      // grid.cu
-int rick_fft_planes(rick_plan_t* p, int n_planes);                       // fft.cu: rows then columns
-int rick_fft_rows(rick_plan_t* p, int n_planes);                         // fft.cu
+int rick_fft_planes(rick_plan_t* p, int plane_first, int n_planes);      // fft.cu: rows then columns (in place)
+int rick_fft_rows(rick_plan_t* p, int plane_first, int n_planes);        // fft.cu: occupied rows only
 int rick_fft_cols(rick_plan_t* p, int n_planes);                         // fft.cu (generic strided pass)
 int rick_cols12_init(rick_plan_t* p);                                    // fft_cols12.cu
 int rick_cols12_fft(rick_plan_t* p, int n_planes);                       // fft_cols12.cu

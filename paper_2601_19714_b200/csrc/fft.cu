@@ -19,11 +19,19 @@ template <typename T, int LOG2N> struct RowCfg {
 template <typename T, int LOG2N>
 __global__ void __launch_bounds__(RowCfg<T, LOG2N>::THREADS)
 k_fft_rows(typename cplx_of<T>::type* __restrict__ stack,
-           const typename cplx_of<T>::type* __restrict__ tw)
+           const typename cplx_of<T>::type* __restrict__ tw, const unsigned char* __restrict__ occ)
 {
     typedef typename cplx_of<T>::type C;
     typedef RowCfg<T, LOG2N> K;
     extern __shared__ __align__(16) unsigned char smem_raw[];
+    // rows no visibility touches are zero in HBM and their transform is zero: skip them (the CTA's
+    // rows are skipped together, all or none, because the stages synchronise the whole CTA)
+    {
+        bool any = false;
+#pragma unroll
+        for (int i = 0; i < K::RPC; ++i) any |= occ[(size_t)blockIdx.x * K::RPC + i] != 0;
+        if (!any) return;
+    }
     const int rl = threadIdx.x / K::NT, t = threadIdx.x - rl * K::NT;
     C* sm = reinterpret_cast<C*>(smem_raw) + (size_t)rl * (K::N + K::N / 16);
     C* g = stack + ((size_t)blockIdx.x * K::RPC + rl) * K::N;
@@ -67,7 +75,7 @@ k_fft_cols(typename cplx_of<T>::type* __restrict__ stack,
 }
 
 template <typename T, int LOG2N>
-static int launch_fft(rick_plan_t* p, int n_planes, int which)   // which: 1 rows, 2 columns, 3 both
+static int launch_fft(rick_plan_t* p, int plane_first, int n_planes, int which)   // which: 1 rows, 2 columns, 3 both
 {
     typedef typename cplx_of<T>::type C;
     typedef RowCfg<T, LOG2N> KR;
@@ -76,9 +84,12 @@ static int launch_fft(rick_plan_t* p, int n_planes, int which)   // which: 1 row
         RICK_CUDA(p, cudaFuncSetAttribute(k_fft_rows<T, LOG2N>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                           (int)KR::SMEM));
         const unsigned int row_blocks = (unsigned int)((size_t)n_planes * KR::N / KR::RPC);
-        RICK_KERNEL(p, RK_FFT_ROWS, k_fft_rows<T, LOG2N><<<row_blocks, KR::THREADS, KR::SMEM, p->stream>>>((C*)p->stack, (const C*)p->twiddle));
+        RICK_KERNEL(p, RK_FFT_ROWS, k_fft_rows<T, LOG2N><<<row_blocks, KR::THREADS, KR::SMEM, p->stream>>>((C*)p->stack, (const C*)p->twiddle, p->row_occ + (size_t)plane_first * p->N));
     }
     if (which & 2) {
+        // the in-place column passes write every row of the slots they transform
+        const int rcd = rick_all_dirty(p, n_planes);
+        if (rcd) return rcd;
         if (!p->f32 && p->cols12_ok) return rick_cols12_fft(p, n_planes);
         RICK_CUDA(p, cudaFuncSetAttribute(k_fft_cols<T, LOG2N>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                           (int)KC::SMEM));
@@ -88,37 +99,37 @@ static int launch_fft(rick_plan_t* p, int n_planes, int which)   // which: 1 row
     return RICK_OK;
 }
 
-static int fft_dispatch(rick_plan_t* p, int n_planes, int which)
+static int fft_dispatch(rick_plan_t* p, int plane_first, int n_planes, int which)
 {
     if (n_planes <= 0) return RICK_OK;
     if (p->f32) {
         switch (p->log2N) {
-            case 6: return launch_fft<float, 6>(p, n_planes, which);
-            case 7: return launch_fft<float, 7>(p, n_planes, which);
-            case 8: return launch_fft<float, 8>(p, n_planes, which);
-            case 9: return launch_fft<float, 9>(p, n_planes, which);
-            case 10: return launch_fft<float, 10>(p, n_planes, which);
-            case 11: return launch_fft<float, 11>(p, n_planes, which);
-            case 12: return launch_fft<float, 12>(p, n_planes, which);
-            case 13: return launch_fft<float, 13>(p, n_planes, which);
-            case 14: return launch_fft<float, 14>(p, n_planes, which);
+            case 6: return launch_fft<float, 6>(p, plane_first, n_planes, which);
+            case 7: return launch_fft<float, 7>(p, plane_first, n_planes, which);
+            case 8: return launch_fft<float, 8>(p, plane_first, n_planes, which);
+            case 9: return launch_fft<float, 9>(p, plane_first, n_planes, which);
+            case 10: return launch_fft<float, 10>(p, plane_first, n_planes, which);
+            case 11: return launch_fft<float, 11>(p, plane_first, n_planes, which);
+            case 12: return launch_fft<float, 12>(p, plane_first, n_planes, which);
+            case 13: return launch_fft<float, 13>(p, plane_first, n_planes, which);
+            case 14: return launch_fft<float, 14>(p, plane_first, n_planes, which);
         }
     } else {
         switch (p->log2N) {
-            case 6: return launch_fft<double, 6>(p, n_planes, which);
-            case 7: return launch_fft<double, 7>(p, n_planes, which);
-            case 8: return launch_fft<double, 8>(p, n_planes, which);
-            case 9: return launch_fft<double, 9>(p, n_planes, which);
-            case 10: return launch_fft<double, 10>(p, n_planes, which);
-            case 11: return launch_fft<double, 11>(p, n_planes, which);
-            case 12: return launch_fft<double, 12>(p, n_planes, which);
-            case 13: return launch_fft<double, 13>(p, n_planes, which);
+            case 6: return launch_fft<double, 6>(p, plane_first, n_planes, which);
+            case 7: return launch_fft<double, 7>(p, plane_first, n_planes, which);
+            case 8: return launch_fft<double, 8>(p, plane_first, n_planes, which);
+            case 9: return launch_fft<double, 9>(p, plane_first, n_planes, which);
+            case 10: return launch_fft<double, 10>(p, plane_first, n_planes, which);
+            case 11: return launch_fft<double, 11>(p, plane_first, n_planes, which);
+            case 12: return launch_fft<double, 12>(p, plane_first, n_planes, which);
+            case 13: return launch_fft<double, 13>(p, plane_first, n_planes, which);
         }
     }
     p->err = "grid edge not supported by the FFT at this precision";
     return RICK_ERR_INVALID;
 }
 
-int rick_fft_planes(rick_plan_t* p, int n_planes) { return fft_dispatch(p, n_planes, 3); }
-int rick_fft_rows(rick_plan_t* p, int n_planes) { return fft_dispatch(p, n_planes, 1); }
-int rick_fft_cols(rick_plan_t* p, int n_planes) { return fft_dispatch(p, n_planes, 2); }
+int rick_fft_planes(rick_plan_t* p, int plane_first, int n_planes) { return fft_dispatch(p, plane_first, n_planes, 3); }
+int rick_fft_rows(rick_plan_t* p, int plane_first, int n_planes) { return fft_dispatch(p, plane_first, n_planes, 1); }
+int rick_fft_cols(rick_plan_t* p, int n_planes) { return fft_dispatch(p, 0, n_planes, 2); }

@@ -321,26 +321,54 @@ __global__ void __launch_bounds__(GRID_WARPS * 32) k_grid(const __grid_constant_
     }
 }
 
-// zero-fill of the resident planes (the gridder accumulates with atomics).  ONE CTA per SM, eight
-// 16-byte stores in flight per thread: measured on B200 this already writes at the full 6.1 TB/s of
-// the 8-CTA/SM version, and it leaves the SMs (and some of the memory queues) to the index / sort
-// kernels that run beside it on the plan's main stream (2 CTAs/SM starved them: index_key 0.08 -> 1.4 ms).
-__global__ void __launch_bounds__(256) k_zero(uint4* __restrict__ dst, size_t n16)
+// Zero-fill.  The gridder accumulates with atomics into a stack that must start from zero, but only
+// rows that were written since they were last cleared can be non-zero: the plan keeps one "dirty" byte
+// per (resident slot, row) and this kernel clears exactly those rows.
+// A small persistent grid walks the (slot, row) pairs -- a clean row costs one byte read -- so the
+// kernel, which runs on the low-priority side stream, never floods the block scheduler in front of
+// the index / sort kernels of the main stream.  16-byte stores; a row is N * E bytes.
+__global__ void __launch_bounds__(256) k_zero_dirty_rows(uint4* __restrict__ stack, unsigned char* __restrict__ dirty,
+                                                         size_t n_rows, size_t row16)
 {
     const uint4 z = make_uint4(0, 0, 0, 0);
-    const size_t stride = (size_t)gridDim.x * blockDim.x;
-    size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    for (; i + 7 * stride < n16; i += 8 * stride) {
-#pragma unroll
-        for (int k = 0; k < 8; ++k) dst[i + k * stride] = z;
+    for (size_t r = blockIdx.x; r < n_rows; r += gridDim.x) {      // slot-major row index
+        const bool d = dirty[r] != 0;
+        __syncthreads();                          // every thread has read the flag before it is cleared
+        if (!d) continue;
+        uint4* dst = stack + r * row16;
+        for (size_t i = threadIdx.x; i < row16; i += 256) dst[i] = z;
+        if (threadIdx.x == 0) dirty[r] = 0;      // only this CTA ever looks at row r
     }
-    for (; i < n16; i += stride) dst[i] = z;
 }
 
-int rick_zero_planes(rick_plan_t* p, int n_planes, cudaStream_t st)
+__global__ void __launch_bounds__(256) k_mark_dirty(unsigned char* __restrict__ dirty, const unsigned char* __restrict__ occ,
+                                                    size_t n)
 {
-    const size_t n16 = p->plane_bytes / 16 * (size_t)n_planes;
-    RICK_KERNEL_ON(p, st, RK_ZERO, k_zero<<<p->n_sm, 256, 0, st>>>(reinterpret_cast<uint4*>(p->stack), n16));
+    const size_t i = (size_t)blockIdx.x * 256 + threadIdx.x;
+    if (i < n && occ[i]) dirty[i] = 1;
+}
+
+int rick_zero_dirty(rick_plan_t* p, int n_slots, cudaStream_t st)
+{
+    const size_t row16 = p->plane_bytes / 16 / (size_t)p->N;
+    RICK_KERNEL_ON(p, st, RK_ZERO, k_zero_dirty_rows<<<p->n_sm * 4, 256, 0, st>>>(
+        reinterpret_cast<uint4*>(p->stack), p->row_dirty, (size_t)n_slots * p->N, row16));
+    return RICK_OK;
+}
+
+// rows of the batch [plane_first, plane_first + n_planes) that the gridder / row pass will write
+int rick_mark_dirty(rick_plan_t* p, int plane_first, int n_planes)
+{
+    const size_t n = (size_t)n_planes * p->N;
+    RICK_KERNEL(p, RK_ROW_OCC, k_mark_dirty<<<(unsigned)((n + 255) / 256), 256, 0, p->stream>>>(
+        p->row_dirty, p->row_occ + (size_t)plane_first * p->N, n));
+    return RICK_OK;
+}
+
+// an in-place column pass writes every row of the slots it transformed
+int rick_all_dirty(rick_plan_t* p, int n_slots)
+{
+    RICK_CUDA(p, cudaMemsetAsync(p->row_dirty, 1, (size_t)n_slots * p->N, p->stream));
     return RICK_OK;
 }
 

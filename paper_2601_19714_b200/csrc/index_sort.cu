@@ -381,6 +381,30 @@ __global__ void k_plane_starts(const u64* __restrict__ sitems, unsigned int M, i
     plane_start[z] = (long long)lo;
 }
 
+// Row occupancy at tile-row granularity.  One thread per (global plane pg, tile row tv): the sorted
+// keys of that tile row are the range [lower_bound(prefix), lower_bound(prefix + 1)) with
+// prefix = pg * T + tv over key / (N * B); a non-empty range marks the rows tv*B - h .. tv*B + B-1 + h
+// (the tile rows plus the kernel halo) of plane pg.  occ is cleared by the caller first.
+__global__ void k_row_occupancy(const u64* __restrict__ sitems, unsigned int M, int idx_bits, int N, int B, int T, int h,
+                                int n_planes_total, unsigned char* __restrict__ occ)
+{
+    const int g = blockIdx.x * blockDim.x + threadIdx.x;
+    if (g >= n_planes_total * T) return;
+    const unsigned long long span = (unsigned long long)N * (unsigned long long)B;      // keys per tile row
+    const unsigned long long t0 = (unsigned long long)g * span, t1 = t0 + span;
+    unsigned int lo = 0, hi = M;
+    while (lo < hi) {
+        const unsigned int mid = lo + (hi - lo) / 2;
+        if ((sitems[mid] >> idx_bits) < t0) lo = mid + 1; else hi = mid;
+    }
+    if (lo >= M || (sitems[lo] >> idx_bits) >= t1) return;      // empty tile row
+    const int pg = g / T, tv = g - pg * T;
+    int r0 = tv * B - h, r1 = tv * B + B - 1 + h;
+    r0 = r0 < 0 ? 0 : r0;
+    r1 = r1 > N - 1 ? N - 1 : r1;
+    for (int r = r0; r <= r1; ++r) occ[(size_t)pg * N + r] = 1;
+}
+
 // ------------------------------------------------------------------------------------------
 static int ensure_u32(rick_plan_t* p, uint32_t** buf, size_t* cap, size_t need)
 {
@@ -456,5 +480,11 @@ int rick_index_sort(rick_plan_t* p, const double* uvw_m, const float* weights)
     RICK_KERNEL(p, RK_PLANE_STARTS, k_plane_starts<<<(n_planes_total + 1 + 127) / 128, 128, 0, st>>>(
         (const u64*)p->sorted_items, M, p->idx_bits, (unsigned long long)p->N * p->N, n_planes_total,
         (long long*)p->plane_start));
+    RICK_CUDA(p, cudaMemsetAsync(p->row_occ, 0, (size_t)n_planes_total * p->N, st));
+    if (M > 0) {
+        const int n = n_planes_total * p->T;
+        RICK_KERNEL(p, RK_ROW_OCC, k_row_occupancy<<<(n + 127) / 128, 128, 0, st>>>(
+            (const u64*)p->sorted_items, M, p->idx_bits, p->N, p->B, p->T, p->h, n_planes_total, p->row_occ));
+    }
     return RICK_OK;
 }

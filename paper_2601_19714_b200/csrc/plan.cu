@@ -18,7 +18,7 @@ static void free_dev(void* q)
 // per-kernel CUDA-event timing
 static const char* const k_names[RK_NKERNELS] = {
     "tables", "reset", "wrange", "index_key", "radix_hist", "scan", "radix_scatter", "plane_starts",
-    "zero", "grid", "fft_rows", "fft_cols", "wcorrect", "taper", "fft_cols_wcorrect"};
+    "zero", "grid", "fft_rows", "fft_cols", "wcorrect", "taper", "fft_cols_wcorrect", "row_occupancy"};
 
 void rick_prof_begin(rick_plan_t* p, int id, cudaStream_t st)
 {
@@ -90,6 +90,7 @@ extern "C" int rick_plan_destroy(rick_plan_t* p)
     free_dev(p->twiddle); free_dev(p->taper); free_dev(p->stack); free_dev(p->image);
     free_dev(p->items); free_dev(p->items_a); free_dev(p->items_b);
     free_dev(p->hist); free_dev(p->scan_tmp); free_dev(p->plane_start); free_dev(p->chan_scale);
+    free_dev(p->row_occ); free_dev(p->row_dirty);
     free_dev(p->wrange); free_dev(p->counters);
     free_dev(p->st_vis); free_dev(p->st_uvw); free_dev(p->st_wgt); free_dev(p->st_img);
     for (cudaEvent_t e : p->prof_ev) cudaEventDestroy(e);
@@ -113,6 +114,11 @@ static int plan_init(rick_plan_t* p)
     const size_t cell = p->f32 ? 8 : 16;
     p->plane_bytes = (size_t)p->N * p->N * cell;
     RICK_CUDA(p, cudaMalloc(&p->stack, p->plane_bytes * (size_t)p->batch));
+    // the resident stack starts all-zero and no row is dirty: from here on only rows that were written
+    // are ever cleared again (rick_zero_dirty)
+    RICK_CUDA(p, cudaMemsetAsync(p->stack, 0, p->plane_bytes * (size_t)p->batch, p->stream));
+    RICK_CUDA(p, cudaMalloc(&p->row_dirty, (size_t)p->batch * p->N));
+    RICK_CUDA(p, cudaMemsetAsync(p->row_dirty, 0, (size_t)p->batch * p->N, p->stream));
     RICK_CUDA(p, cudaMalloc(&p->image, sizeof(double) * (size_t)p->N * p->N));
     RICK_CUDA(p, cudaMallocHost(&p->h_scale, sizeof(double) * RICK_MAX_CHAN));
     RICK_CUDA(p, cudaEventCreateWithFlags(&p->ev_scale, cudaEventDisableTiming));
@@ -249,6 +255,12 @@ static int prepare(rick_plan_t* p, const double* chan_freq_hz, int32_t n_chan, i
         if ((rc = grow(p, &p->plane_start, (size_t)n_pl))) return rc;
         p->plane_start_cap = n_pl;
     }
+    const size_t occ_bytes = (size_t)(n_pl - 1) * p->N;
+    if (occ_bytes > p->row_occ_cap) {
+        p->row_occ_cap = 0;
+        if ((rc = grow(p, &p->row_occ, occ_bytes))) return rc;
+        p->row_occ_cap = occ_bytes;
+    }
     if (n_chan > p->chan_cap) {
         if ((rc = grow(p, &p->chan_scale, (size_t)n_chan))) return rc;
         if ((rc = grow(p, &p->wrange, (size_t)n_chan))) return rc;
@@ -268,14 +280,16 @@ static int prepare(rick_plan_t* p, const double* chan_freq_hz, int32_t n_chan, i
     return RICK_OK;
 }
 
-// a0..a2 on the plan's stream while the zero-fill of the first plane batch runs on the side stream
-// (it needs nothing from the sort, only that earlier readers of the stack are done); joined before a3.
+// a0..a2 on the plan's stream while the rows the previous call left dirty are cleared on the side
+// stream (that needs nothing from the sort, only that earlier readers of the stack are done); joined
+// before a3.  Afterwards the whole resident stack is zero.
 static int sort_and_zero(rick_plan_t* p, const double* uvw_m, const float* weights, int n_planes_first)
 {
     int rc;
+    (void)n_planes_first;
     RICK_CUDA(p, cudaEventRecord(p->ev_fork, p->stream));
     RICK_CUDA(p, cudaStreamWaitEvent(p->stream2, p->ev_fork, 0));
-    if ((rc = rick_zero_planes(p, n_planes_first, p->stream2))) return rc;
+    if ((rc = rick_zero_dirty(p, p->batch, p->stream2))) return rc;
     RICK_CUDA(p, cudaEventRecord(p->ev_join, p->stream2));
     if ((rc = rick_index_sort(p, uvw_m, weights))) return rc;
     RICK_CUDA(p, cudaStreamWaitEvent(p->stream, p->ev_join, 0));
@@ -293,6 +307,7 @@ extern "C" int rick_grid(rick_plan_t* p, const void* vis, int32_t vis_dtype, con
     p->state = 0;
     if ((rc = prepare(p, chan_freq_hz, n_chan, n_rows))) return rc;
     if ((rc = sort_and_zero(p, uvw_m, weights, p->Nw))) return rc;
+    if ((rc = rick_mark_dirty(p, 0, p->Nw))) return rc;
     if ((rc = rick_grid_planes(p, vis, vis_dtype, uvw_m, weights, 0, p->Nw))) return rc;
     p->state = 1;
     return RICK_OK;
@@ -303,7 +318,7 @@ extern "C" int rick_fft_wplanes(rick_plan_t* p)
     if (!p) return RICK_ERR_INVALID;
     p->err.clear();
     if (p->state != 1) { p->err = "rick_fft_wplanes needs a gridded stack"; return RICK_ERR_STATE; }
-    const int rc = rick_fft_planes(p, p->Nw);
+    const int rc = rick_fft_planes(p, 0, p->Nw);
     if (rc) return rc;
     p->state = 2;
     return RICK_OK;
@@ -352,10 +367,11 @@ static int image_impl(rick_plan_t* p, const void* vis, int32_t vis_dtype, const 
         for (int z0 = 0; z0 < p->Nw; z0 += p->batch) {
             const int nb = p->Nw - z0 < p->batch ? p->Nw - z0 : p->batch;
             const int last = z0 + nb >= p->Nw;
-            if ((img > 0 || z0 > 0) && (rc = rick_zero_planes(p, nb, p->stream))) return rc;
+            if ((img > 0 || z0 > 0) && (rc = rick_zero_dirty(p, p->batch, p->stream))) return rc;
+            if ((rc = rick_mark_dirty(p, img * p->Nw + z0, nb))) return rc;
             if ((rc = rick_grid_planes(p, vis, vis_dtype, uvw_m, weights, img * p->Nw + z0, nb))) return rc;
             if (p->cols12_ok) {   // column pass fused with the w-correction: the transformed planes are never written
-                if ((rc = rick_fft_rows(p, nb))) return rc;
+                if ((rc = rick_fft_rows(p, img * p->Nw + z0, nb))) return rc;
                 const int strips = rick_cols12_strips();
                 if (host_out && last && !p->d.cube) {
                     // whole rounds of the persistent grid per part: 4 + 4 + 3 + rest rounds of n_sm strips
@@ -377,7 +393,7 @@ static int image_impl(rick_plan_t* p, const void* vis, int32_t vis_dtype, const 
                     if ((rc = rick_cols12_wcorrect(p, img, z0, nb, dst, z0 > 0, last, 0, strips))) return rc;
                 }
             } else {
-                if ((rc = rick_fft_planes(p, nb))) return rc;
+                if ((rc = rick_fft_planes(p, img * p->Nw + z0, nb))) return rc;
                 if ((rc = rick_wcorrect(p, img, z0, nb, dst, z0 > 0, last))) return rc;
             }
         }
