@@ -69,6 +69,10 @@ struct rick_plan_s {
     // are neither are zero in HBM and stay untouched by zero-fill, gridder and the row pass.
     unsigned char* row_occ; size_t row_occ_cap;
     unsigned char* row_dirty;
+    // tile occupancy: tile_occ[pg][tv][tu] = 1 when the footprint of some
+    // visibility of global plane pg reaches the B x B tile (tv, tu); rebuilt by every sort.  In rick_image
+    // the zero-fill clears, and the row pass reads, only those tiles of an occupied row.
+    unsigned char* tile_occ; size_t tile_occ_cap;
     double* chan_scale;      // [C] device, s_c = f_c / c0
     WRange* wrange;          // [n_img] device
     int chan_cap;
@@ -138,6 +142,7 @@ void rick_prof_end(rick_plan_t* p, cudaStream_t st);
 int rick_tables_build(rick_plan_t* p);                                   // tables.cu
 int rick_index_sort(rick_plan_t* p, const double* uvw_m, const float* weights);   // index_sort.cu
 int rick_zero_dirty(rick_plan_t* p, int n_slots, cudaStream_t st);        // grid.cu: zero the dirty rows of slots 0..n_slots-1
+int rick_zero_sparse(rick_plan_t* p, int plane_first, int n_slots);     // grid.cu: stale rows whole, occupied rows by tile
 int rick_mark_dirty(rick_plan_t* p, int plane_first, int n_planes);      // grid.cu: dirty |= occupancy of the batch
 int rick_all_dirty(rick_plan_t* p, int n_slots);                         // grid.cu: after an in-place column pass
 int rick_grid_planes(rick_plan_t* p, const void* vis, int vis_dtype, const double* uvw_m,

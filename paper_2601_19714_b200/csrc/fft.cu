@@ -19,7 +19,8 @@ template <typename T, int LOG2N> struct RowCfg {
 template <typename T, int LOG2N>
 __global__ void __launch_bounds__(RowCfg<T, LOG2N>::THREADS)
 k_fft_rows(typename cplx_of<T>::type* __restrict__ stack,
-           const typename cplx_of<T>::type* __restrict__ tw, const unsigned char* __restrict__ occ)
+           const typename cplx_of<T>::type* __restrict__ tw, const unsigned char* __restrict__ occ,
+           const unsigned char* __restrict__ tocc, int log2B)
 {
     typedef typename cplx_of<T>::type C;
     typedef RowCfg<T, LOG2N> K;
@@ -35,9 +36,30 @@ k_fft_rows(typename cplx_of<T>::type* __restrict__ stack,
     const int rl = threadIdx.x / K::NT, t = threadIdx.x - rl * K::NT;
     C* sm = reinterpret_cast<C*>(smem_raw) + (size_t)rl * (K::N + K::N / 16);
     C* g = stack + ((size_t)blockIdx.x * K::RPC + rl) * K::N;
+    // only the tiles some footprint reaches hold gridded data (tile_occ); whatever else the row holds
+    // (rick_image leaves the previous transform there) is not read and counts as zero
+    __shared__ unsigned char s_to[K::RPC][K::N / 8];
+    {
+        const int Tn = K::N >> log2B;
+        for (int i = threadIdx.x; i < K::RPC * Tn; i += K::THREADS) {
+            const int a = i / Tn, ti = i - a * Tn;
+            const size_t R = (size_t)blockIdx.x * K::RPC + a;          // slot-major row
+            const size_t slot = R / K::N;
+            const int row = (int)(R - slot * K::N);
+            s_to[a][ti] = tocc[(slot * Tn + (size_t)(row >> log2B)) * Tn + ti];
+        }
+        __syncthreads();
+    }
     C v[16];
 #pragma unroll
-    for (int e = 0; e < 16; ++e) v[e] = g[t + K::NT * ((e + 8) & 15)];
+    for (int e = 0; e < 16; ++e) {
+        const int i = t + K::NT * ((e + 8) & 15);
+        C x;
+        x.x = 0;
+        x.y = 0;
+        if (s_to[rl][i >> log2B]) x = g[i];
+        v[e] = x;
+    }
     fft_thread<T, LOG2N>(v, t, sm, 1, 0, tw);
 #pragma unroll
     for (int e = 0; e < 16; ++e) g[t + K::NT * ((e + 8) & 15)] = v[e];
@@ -84,7 +106,8 @@ static int launch_fft(rick_plan_t* p, int plane_first, int n_planes, int which) 
         RICK_CUDA(p, cudaFuncSetAttribute(k_fft_rows<T, LOG2N>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                           (int)KR::SMEM));
         const unsigned int row_blocks = (unsigned int)((size_t)n_planes * KR::N / KR::RPC);
-        RICK_KERNEL(p, RK_FFT_ROWS, k_fft_rows<T, LOG2N><<<row_blocks, KR::THREADS, KR::SMEM, p->stream>>>((C*)p->stack, (const C*)p->twiddle, p->row_occ + (size_t)plane_first * p->N));
+        RICK_KERNEL(p, RK_FFT_ROWS, k_fft_rows<T, LOG2N><<<row_blocks, KR::THREADS, KR::SMEM, p->stream>>>((C*)p->stack, (const C*)p->twiddle, p->row_occ + (size_t)plane_first * p->N,
+            p->tile_occ + (size_t)plane_first * p->T * p->T, p->log2B));
     }
     if (which & 2) {
         // the in-place column passes write every row of the slots they transform

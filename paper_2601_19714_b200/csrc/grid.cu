@@ -341,6 +341,46 @@ __global__ void __launch_bounds__(256) k_zero_dirty_rows(uint4* __restrict__ sta
     }
 }
 
+// Zero-fill of rick_image ("known-zero tiles").  One warp per (slot, row) of the resident batch:
+//   dirty, not occupied now  -> the row holds stale data the column pass would read: cleared whole;
+//   dirty and occupied now   -> the row pass reads only the tiles some footprint reaches (tile_occ) and
+//                               overwrites the whole row, so only those tiles are cleared for the gridder;
+//   not dirty                -> already zero.
+// unit16 = 16-byte units per tile row (B * E / 16), row16 = units per row.
+__global__ void __launch_bounds__(256) k_zero_sparse(uint4* __restrict__ stack, unsigned char* __restrict__ dirty,
+                                                     const unsigned char* __restrict__ occ,
+                                                     const unsigned char* __restrict__ tocc, size_t n_rows, int N,
+                                                     int log2B, int T, size_t row16, int unit16)
+{
+    const uint4 z = make_uint4(0, 0, 0, 0);
+    const int lane = threadIdx.x & 31;
+    const size_t warp = ((size_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const size_t n_warps = ((size_t)gridDim.x * blockDim.x) >> 5;
+    for (size_t r = warp; r < n_rows; r += n_warps) {            // slot-major row index
+        if (!dirty[r]) continue;
+        uint4* dst = stack + r * row16;
+        if (!occ[r]) {
+            for (size_t i = lane; i < row16; i += 32) dst[i] = z;
+            __syncwarp();
+            if (lane == 0) dirty[r] = 0;
+            continue;
+        }
+        const size_t slot = r / (size_t)N;
+        const int row = (int)(r - slot * (size_t)N);
+        const unsigned char* to = tocc + (slot * (size_t)T + (size_t)(row >> log2B)) * (size_t)T;
+        for (int t0 = 0; t0 < T; t0 += 32) {
+            const int ti = t0 + lane;
+            unsigned int m = __ballot_sync(0xffffffffu, ti < T && to[ti] != 0);
+            while (m) {
+                const int b = __ffs(m) - 1;
+                m &= m - 1;
+                uint4* d = dst + (size_t)(t0 + b) * unit16;
+                for (int i = lane; i < unit16; i += 32) d[i] = z;
+            }
+        }
+    }
+}
+
 __global__ void __launch_bounds__(256) k_mark_dirty(unsigned char* __restrict__ dirty, const unsigned char* __restrict__ occ,
                                                     size_t n)
 {
@@ -353,6 +393,18 @@ int rick_zero_dirty(rick_plan_t* p, int n_slots, cudaStream_t st)
     const size_t row16 = p->plane_bytes / 16 / (size_t)p->N;
     RICK_KERNEL_ON(p, st, RK_ZERO, k_zero_dirty_rows<<<p->n_sm * 4, 256, 0, st>>>(
         reinterpret_cast<uint4*>(p->stack), p->row_dirty, (size_t)n_slots * p->N, row16));
+    return RICK_OK;
+}
+
+// slots 0..n_slots-1 are about to receive global planes plane_first.. (occupancy of the current sort)
+int rick_zero_sparse(rick_plan_t* p, int plane_first, int n_slots)
+{
+    const size_t cell = p->f32 ? 8 : 16;
+    const size_t row16 = p->plane_bytes / 16 / (size_t)p->N;
+    const int unit16 = (int)((size_t)p->B * cell / 16);
+    RICK_KERNEL(p, RK_ZERO, k_zero_sparse<<<p->n_sm * 8, 256, 0, p->stream>>>(
+        reinterpret_cast<uint4*>(p->stack), p->row_dirty, p->row_occ + (size_t)plane_first * p->N,
+        p->tile_occ + (size_t)plane_first * p->T * p->T, (size_t)n_slots * p->N, p->N, p->log2B, p->T, row16, unit16));
     return RICK_OK;
 }
 

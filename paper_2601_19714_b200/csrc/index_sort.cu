@@ -405,6 +405,32 @@ __global__ void k_row_occupancy(const u64* __restrict__ sitems, unsigned int M, 
     for (int r = r0; r <= r1; ++r) occ[(size_t)pg * N + r] = 1;
 }
 
+// Tile occupancy.  One thread per sorted item; the first item of every run of equal keys (= one
+// centre cell, reading R22) marks the B x B tiles its S x S footprint reaches: rows
+// (i_v-h)>>log2B .. (i_v+h)>>log2B, columns likewise (on-grid visibilities only, so every tile
+// exists).  Plain stores of 1 (idempotent, no atomics).  occ is cleared by the caller first.
+__global__ void __launch_bounds__(256)
+k_tile_occupancy(const u64* __restrict__ sitems, const long long* __restrict__ plane_start, int n_planes_total,
+                 int idx_bits, int log2B, int log2T, int h, unsigned char* __restrict__ tocc)
+{
+    const long long n_valid = plane_start[n_planes_total];       // dropped visibilities sort last
+    const int Bm = (1 << log2B) - 1, Tm = (1 << log2T) - 1;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n_valid;
+         i += (long long)gridDim.x * blockDim.x) {
+        const u64 key = sitems[i] >> idx_bits;
+        if (i > 0 && (sitems[i - 1] >> idx_bits) == key) continue;
+        const int cu = (int)(key & (u64)Bm), cv = (int)((key >> log2B) & (u64)Bm);
+        const u64 tkey = key >> (2 * log2B);
+        const int tu = (int)(tkey & (u64)Tm), tv = (int)((tkey >> log2T) & (u64)Tm);
+        const u64 pg = tkey >> (2 * log2T);
+        const int iu = (tu << log2B) + cu, iv = (tv << log2B) + cv;
+        const int u0 = (iu - h) >> log2B, u1 = (iu + h) >> log2B, v0 = (iv - h) >> log2B, v1 = (iv + h) >> log2B;
+        unsigned char* o = tocc + ((size_t)pg << (2 * log2T));
+        for (int a = v0; a <= v1; ++a)
+            for (int b = u0; b <= u1; ++b) o[((size_t)a << log2T) + b] = 1;
+    }
+}
+
 // ------------------------------------------------------------------------------------------
 static int ensure_u32(rick_plan_t* p, uint32_t** buf, size_t* cap, size_t need)
 {
@@ -485,6 +511,14 @@ int rick_index_sort(rick_plan_t* p, const double* uvw_m, const float* weights)
         const int n = n_planes_total * p->T;
         RICK_KERNEL(p, RK_ROW_OCC, k_row_occupancy<<<(n + 127) / 128, 128, 0, st>>>(
             (const u64*)p->sorted_items, M, p->idx_bits, p->N, p->B, p->T, p->h, n_planes_total, p->row_occ));
+    }
+    RICK_CUDA(p, cudaMemsetAsync(p->tile_occ, 0, (size_t)n_planes_total * p->T * p->T, st));
+    if (M > 0) {
+        unsigned int nb = (M + 255) / 256;
+        if (nb > (unsigned)p->n_sm * 8u) nb = (unsigned)p->n_sm * 8u;
+        RICK_KERNEL(p, RK_ROW_OCC, k_tile_occupancy<<<nb, 256, 0, st>>>(
+            (const u64*)p->sorted_items, (const long long*)p->plane_start, n_planes_total, p->idx_bits, p->log2B,
+            p->log2N - p->log2B, p->h, p->tile_occ));
     }
     return RICK_OK;
 }

@@ -90,7 +90,7 @@ extern "C" int rick_plan_destroy(rick_plan_t* p)
     free_dev(p->twiddle); free_dev(p->taper); free_dev(p->stack); free_dev(p->image);
     free_dev(p->items); free_dev(p->items_a); free_dev(p->items_b);
     free_dev(p->hist); free_dev(p->scan_tmp); free_dev(p->plane_start); free_dev(p->chan_scale);
-    free_dev(p->row_occ); free_dev(p->row_dirty);
+    free_dev(p->row_occ); free_dev(p->row_dirty); free_dev(p->tile_occ);
     free_dev(p->wrange); free_dev(p->counters);
     free_dev(p->st_vis); free_dev(p->st_uvw); free_dev(p->st_wgt); free_dev(p->st_img);
     for (cudaEvent_t e : p->prof_ev) cudaEventDestroy(e);
@@ -261,6 +261,12 @@ static int prepare(rick_plan_t* p, const double* chan_freq_hz, int32_t n_chan, i
         if ((rc = grow(p, &p->row_occ, occ_bytes))) return rc;
         p->row_occ_cap = occ_bytes;
     }
+    const size_t tocc_bytes = (size_t)(n_pl - 1) * p->T * p->T;
+    if (tocc_bytes > p->tile_occ_cap) {
+        p->tile_occ_cap = 0;
+        if ((rc = grow(p, &p->tile_occ, tocc_bytes))) return rc;
+        p->tile_occ_cap = tocc_bytes;
+    }
     if (n_chan > p->chan_cap) {
         if ((rc = grow(p, &p->chan_scale, (size_t)n_chan))) return rc;
         if ((rc = grow(p, &p->wrange, (size_t)n_chan))) return rc;
@@ -358,7 +364,8 @@ static int image_impl(rick_plan_t* p, const void* vis, int32_t vis_dtype, const 
     if (p->d.cube && !image_out) { p->err = "cube mode needs image_out"; return RICK_ERR_INVALID; }
     p->state = 0;
     if ((rc = prepare(p, chan_freq_hz, n_chan, n_rows))) return rc;
-    if ((rc = sort_and_zero(p, uvw_m, weights, p->Nw < p->batch ? p->Nw : p->batch))) return rc;
+    // a0..a2, then the zero-fill that needs this sort's occupancy (stale rows whole, occupied rows by tile)
+    if ((rc = rick_index_sort(p, uvw_m, weights))) return rc;
     if (vis_ready) RICK_CUDA(p, cudaStreamWaitEvent(p->stream, vis_ready, 0));
     const size_t NN = (size_t)p->N * p->N;
     bool host_done = false;
@@ -367,7 +374,7 @@ static int image_impl(rick_plan_t* p, const void* vis, int32_t vis_dtype, const 
         for (int z0 = 0; z0 < p->Nw; z0 += p->batch) {
             const int nb = p->Nw - z0 < p->batch ? p->Nw - z0 : p->batch;
             const int last = z0 + nb >= p->Nw;
-            if ((img > 0 || z0 > 0) && (rc = rick_zero_dirty(p, p->batch, p->stream))) return rc;
+            if ((rc = rick_zero_sparse(p, img * p->Nw + z0, nb))) return rc;
             if ((rc = rick_mark_dirty(p, img * p->Nw + z0, nb))) return rc;
             if ((rc = rick_grid_planes(p, vis, vis_dtype, uvw_m, weights, img * p->Nw + z0, nb))) return rc;
             if (p->cols12_ok) {   // column pass fused with the w-correction: the transformed planes are never written
