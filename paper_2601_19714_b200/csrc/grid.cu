@@ -76,21 +76,80 @@ __device__ __forceinline__ void red_add(float2* a, float2 v) { atomicAdd(a, v); 
 
 __global__ void k_chunk_reset(unsigned int* c) { *c = 0u; }
 
+// shared-window (32-bit) addressing of the walk
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ double2 lds_d2(uint32_t a)
+{
+    double2 v;
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ double lds_d(uint32_t a)
+{
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ uint2 lds_u2(uint32_t a)
+{
+    uint2 v;
+    asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(a));
+    return v;
+}
+// D (8 x 8) += A (8 x 4, row) B (4 x 8, col) in fp64: lane l holds A[l>>2][l&3], B[l&3][l>>2],
+// D[l>>2][2(l&3)], D[l>>2][2(l&3)+1]
+__device__ __forceinline__ void dmma884(double (&d)[2], double a, double b)
+{
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};"
+                 : "+d"(d[0]), "+d"(d[1]) : "d"(a), "d"(b));
+}
+// two horizontally adjacent tile cells <-> registers (re0, re1), (im0, im1)
+template <typename GT> __device__ __forceinline__ void tile_load2(uint32_t a, double (&re)[2], double (&im)[2]);
+template <typename GT> __device__ __forceinline__ void tile_store2(uint32_t a, const double (&re)[2], const double (&im)[2]);
+template <> __device__ __forceinline__ void tile_load2<double>(uint32_t a, double (&re)[2], double (&im)[2])
+{
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%4];\n\tld.shared.v2.f64 {%2, %3}, [%4+16];"
+                 : "=d"(re[0]), "=d"(im[0]), "=d"(re[1]), "=d"(im[1]) : "r"(a));
+}
+template <> __device__ __forceinline__ void tile_store2<double>(uint32_t a, const double (&re)[2], const double (&im)[2])
+{
+    asm volatile("st.shared.v2.f64 [%4], {%0, %1};\n\tst.shared.v2.f64 [%4+16], {%2, %3};"
+                 :: "d"(re[0]), "d"(im[0]), "d"(re[1]), "d"(im[1]), "r"(a) : "memory");
+}
+// fp32 grid: cells are 8 bytes and the row pitch is odd, so only 8-byte alignment
+template <> __device__ __forceinline__ void tile_load2<float>(uint32_t a, double (&re)[2], double (&im)[2])
+{
+    float t0, t1, t2, t3;
+    asm volatile("ld.shared.v2.f32 {%0, %1}, [%4];\n\tld.shared.v2.f32 {%2, %3}, [%4+8];"
+                 : "=f"(t0), "=f"(t1), "=f"(t2), "=f"(t3) : "r"(a));
+    re[0] = (double)t0;
+    im[0] = (double)t1;
+    re[1] = (double)t2;
+    im[1] = (double)t3;
+}
+template <> __device__ __forceinline__ void tile_store2<float>(uint32_t a, const double (&re)[2], const double (&im)[2])
+{
+    const float t0 = (float)re[0], t1 = (float)im[0], t2 = (float)re[1], t3 = (float)im[1];
+    asm volatile("st.shared.v2.f32 [%4], {%0, %1};\n\tst.shared.v2.f32 [%4+8], {%2, %3};"
+                 :: "f"(t0), "f"(t1), "f"(t2), "f"(t3), "r"(a) : "memory");
+}
+
+#define GRID_KS 36      // staging row stride in visibilities (32 + the overhang of the last group of 4)
+
 template <int S> __host__ __device__ constexpr size_t grid_stage_bytes()
 {
-    // ku[32][SP] doubles | kw[32][S] double2 | key[32] u64
-    return (size_t)32 * (2 * ((S + 1) / 2)) * 8 + (size_t)32 * S * 16 + 32 * 8;
+    // kw[S][KS] double2 | ku[S][KS] double | run[34] uint2
+    return (size_t)S * GRID_KS * 16 + (size_t)S * GRID_KS * 8 + 34 * 8;
 }
 
 template <typename GT, int S>
-__global__ void __launch_bounds__(GRID_WARPS * 32) k_grid(const __grid_constant__ GridParamsS<S> PS)
+__global__ void __launch_bounds__(GRID_WARPS * 32, 2) k_grid(const __grid_constant__ GridParamsS<S> PS)
 {
     typedef typename cell_t<GT>::type cell;
     typedef unsigned long long u64;
     constexpr int H = (S - 1) / 2;
-    constexpr int PW = (S + 1) / 2;                 // cell pairs per footprint row
-    constexpr int SP = 2 * PW;                      // padded footprint width (even)
-    constexpr int NPAIR = S * PW, ROUNDS = (NPAIR + 31) / 32;
+    constexpr int MT = (S + 7) / 8;                 // 8 x 8 fragments per footprint axis
+    constexpr int KS = GRID_KS;
     constexpr int DEG = RICK_KB_DEG;
     static_assert(DEG % 2 == 0, "even/odd Horner split assumes an even degree");
     const GridParams& P = PS.g;
@@ -101,41 +160,46 @@ __global__ void __launch_bounds__(GRID_WARPS * 32) k_grid(const __grid_constant_
     const int sub_bits = 2 * log2B, idx_bits = P.idx_bits;
     const u64 idx_mask = (1ull << idx_bits) - 1ull;
 
-    // shared layout per warp: tile | ku[32][SP] | kw[32][S] | key[32]
+    // shared layout per warp: tile | kw[S][KS] | ku[S][KS] | run[34]
     const size_t tile_bytes = ((size_t)tile_cells * sizeof(cell) + 15) & ~(size_t)15;
     const size_t per_warp = tile_bytes + grid_stage_bytes<S>();
     unsigned char* wbase = smem_raw + (size_t)warp * per_warp;
     cell* tile = reinterpret_cast<cell*>(wbase);
-    double* s_ku = reinterpret_cast<double*>(wbase + tile_bytes);
-    double2* s_kw = reinterpret_cast<double2*>(s_ku + 32 * SP);
-    u64* s_key = reinterpret_cast<u64*>(s_kw + 32 * S);
+    double2* s_kw = reinterpret_cast<double2*>(wbase + tile_bytes);
+    double* s_ku = reinterpret_cast<double*>(s_kw + S * KS);
+    uint2* s_run = reinterpret_cast<uint2*>(s_ku + S * KS);
 
     cell zero;
     zero.x = 0;
     zero.y = 0;
     for (int i = lane; i < tile_cells; i += 32) tile[i] = zero;
-    for (int i = lane; i < 32 * SP; i += 32) s_ku[i] = 0.0;      // also the zero weight of the pad column
+    for (int i = lane; i < S * KS; i += 32) {       // the overhang columns 32..35 stay finite (masked to 0 anyway)
+        s_ku[i] = 0.0;
+        s_kw[i] = make_double2(0.0, 0.0);
+    }
     __syncwarp();
 
-    // cell pair(s) of this lane: pair = lane + 32*rr -> row b, cells (b, 2 a2), (b, 2 a2 + 1).
-    // Lanes without a pair read valid staging addresses (pair 0) and are masked at the flush only,
-    // so the accumulation loop has no per-lane branch.
-    int foff[ROUNDS];
-    bool has[ROUNDS];
-    const double2* pku[ROUNDS];
-    const double2* pkw[ROUNDS];
-    double acc[ROUNDS][4];
+    // Fragment roles (DMMA m8n8k4; M = footprint row b, N = footprint column a, K = visibility):
+    // lane = 4 g + q feeds A[g][q] = (w V) g_v[b = g + 8 mt] of visibility jj + q, B[q][g] = g_u[a = g + 8 nt]
+    // of the same visibility, and owns the cell pair (b = g + 8 mt, a = 8 nt + 2 q, + 1) of the footprint.
+    const int g = lane >> 2, q = lane & 3;
+    bool has[MT][MT], row_ok[MT];
+    uint32_t a_tile[MT][MT], a_kw[MT], a_ku[MT];
+    double c_re[MT][MT][2], c_im[MT][MT][2];
 #pragma unroll
-    for (int rr = 0; rr < ROUNDS; ++rr) {
-        const int pi = lane + 32 * rr;
-        has[rr] = pi < NPAIR;
-        const int b = has[rr] ? pi / PW : 0;
-        const int a2 = has[rr] ? 2 * (pi - b * PW) : 0;
-        foff[rr] = b * TWp + a2;
-        pku[rr] = reinterpret_cast<const double2*>(s_ku + a2);
-        pkw[rr] = s_kw + b;
-        acc[rr][0] = acc[rr][1] = acc[rr][2] = acc[rr][3] = 0.0;
+    for (int mt = 0; mt < MT; ++mt) {
+        row_ok[mt] = g + 8 * mt < S;
+        const int rw = row_ok[mt] ? g + 8 * mt : 0;
+        a_kw[mt] = smem_u32(s_kw + rw * KS + q);
+        a_ku[mt] = smem_u32(s_ku + rw * KS + q);
+#pragma unroll
+        for (int nt = 0; nt < MT; ++nt) {
+            has[mt][nt] = row_ok[mt] && (8 * nt + 2 * q < S);
+            a_tile[mt][nt] = smem_u32(tile + (has[mt][nt] ? (g + 8 * mt) * TWp + 8 * nt + 2 * q : 0));
+            c_re[mt][nt][0] = c_re[mt][nt][1] = c_im[mt][nt][0] = c_im[mt][nt][1] = 0.0;
+        }
     }
+    const uint32_t a_run = smem_u32(s_run);
 
     const long long v_begin = P.plane_start[P.plane_first];
     const long long v_end = P.plane_start[P.plane_first + P.n_planes];
@@ -145,25 +209,25 @@ __global__ void __launch_bounds__(GRID_WARPS * 32) k_grid(const __grid_constant_
     const unsigned int C = (unsigned)P.C;
 
     const u64 NOKEY = ~0ull;
-    u64 cur_cell = NOKEY;          // key of the run being summed in registers
-    int cur_base = 0;              // its top-left footprint cell, local to the tile
+    u64 last_key = NOKEY;          // key of the visibility before this batch (NOKEY: nothing pending)
+    u64 cur_tile = 0;              // (image, plane, tile) of the run held in the accumulators
+    uint32_t cur_off = 0;          // byte offset of its top-left footprint cell inside the tile
+    bool have_run = false;
 
-    // registers -> tile, once per run
-    auto flush_run = [&]() {
+    // accumulators <-> tile: a run starts FROM the tile's cells and is stored back when it ends
+    auto run_load = [&]() {
 #pragma unroll
-        for (int rr = 0; rr < ROUNDS; ++rr) {
-            if (has[rr]) {
-                cell* tp = tile + cur_base + foff[rr];
-                cell t0 = tp[0], t1 = tp[1];
-                t0.x += (GT)acc[rr][0];
-                t0.y += (GT)acc[rr][1];
-                t1.x += (GT)acc[rr][2];
-                t1.y += (GT)acc[rr][3];
-                tp[0] = t0;
-                tp[1] = t1;
-            }
-            acc[rr][0] = acc[rr][1] = acc[rr][2] = acc[rr][3] = 0.0;
-        }
+        for (int mt = 0; mt < MT; ++mt)
+#pragma unroll
+            for (int nt = 0; nt < MT; ++nt)
+                if (has[mt][nt]) tile_load2<GT>(a_tile[mt][nt] + cur_off, c_re[mt][nt], c_im[mt][nt]);
+    };
+    auto run_store = [&]() {
+#pragma unroll
+        for (int mt = 0; mt < MT; ++mt)
+#pragma unroll
+            for (int nt = 0; nt < MT; ++nt)
+                if (has[mt][nt]) tile_store2<GT>(a_tile[mt][nt] + cur_off, c_re[mt][nt], c_im[mt][nt]);
     };
     // tile -> HBM, once per (tile, chunk)
     auto flush_tile = [&](u64 tkey) {
@@ -171,12 +235,12 @@ __global__ void __launch_bounds__(GRID_WARPS * 32) k_grid(const __grid_constant_
         const unsigned int pz = (unsigned int)(tkey / TT), rem = (unsigned int)(tkey - (u64)pz * TT);
         const int tv = (int)(rem / (unsigned)T), tu = (int)(rem - (unsigned)tv * (unsigned)T);
         cell* plane = reinterpret_cast<cell*>(P.stack) + (size_t)(pz - (unsigned)P.plane_first) * N * N;
+        const long long g0 = (long long)(tv * B - h) * N + (tu * B - h);     // may be < 0 on the grid edge
         for (int row = 0; row < TH; ++row) {
             for (int col = lane; col < TH; col += 32) {
                 cell v = tile[row * TWp + col];
                 if (v.x != 0 || v.y != 0) {
-                    const int gv = tv * B - h + row, gu = tu * B - h + col;
-                    red_add(plane + ((size_t)gv * N + gu), v);
+                    red_add(plane + (g0 + (long long)row * N + col), v);
                     tile[row * TWp + col] = zero;
                 }
             }
@@ -228,14 +292,34 @@ __global__ void __launch_bounds__(GRID_WARPS * 32) k_grid(const __grid_constant_
         load_vis(load_item(c_begin + lane, c_end), cur);
         u64 item_next = load_item(c_begin + 32 + lane, c_end);
         for (long long b0 = c_begin; b0 < c_end; b0 += 32) {
-            // ---- stage this batch: kernel values of the lane's own visibility ----
-            const bool valid = cur.key != NOKEY;
-            // a run starts where the key differs from the previous visibility's (lane 0: from the run in registers)
-            u64 prev = __shfl_up_sync(0xffffffffu, cur.key, 1);
-            if (lane == 0) prev = cur_cell;
-            const unsigned int run_mask = __ballot_sync(0xffffffffu, valid && cur.key != prev);
+            // ---- stage this batch: kernel values of the lane's own visibility, run descriptors ----
+            const int nb = (int)((c_end - b0) < 32 ? (c_end - b0) : 32);
+            const u64 key = cur.key;
+            const bool valid = key != NOKEY;
+            // a run starts where the key differs from the previous visibility's; a tile where its
+            // (image, plane, tile) part does
+            u64 prev = __shfl_up_sync(0xffffffffu, key, 1);
+            if (lane == 0) prev = last_key;
+            const unsigned int run_mask = __ballot_sync(0xffffffffu, valid && key != prev);
+            const unsigned int tile_mask = __ballot_sync(0xffffffffu, valid && (key >> sub_bits) != (prev >> sub_bits));
+            last_key = __shfl_sync(0xffffffffu, key, 31);      // NOKEY after a short (= last) batch
+            // descriptor r: x = first visibility | count << 8 | new tile << 16 | continuation << 17, y = byte
+            // offset of the footprint in the tile.  A batch that opens inside a run gets a continuation first.
+            const unsigned int cont = (run_mask & 1u) ? 0u : 1u;
+            const int n_runs = __popc(run_mask) + (int)cont;
+            if (valid && (((run_mask >> lane) & 1u) || lane == 0)) {
+                const unsigned int above = lane < 31 ? (run_mask >> (lane + 1)) : 0u;
+                int end = above ? lane + __ffs(above) : nb;
+                end = end < nb ? end : nb;
+                const int sub = (int)(key & ((1ull << sub_bits) - 1ull));
+                const unsigned int r = (unsigned)__popc(run_mask & ((1u << lane) - 1u)) + (((run_mask >> lane) & 1u) ? cont : 0u);
+                uint2 d;
+                d.x = (unsigned)lane | ((unsigned)(end - lane) << 8) | (((tile_mask >> lane) & 1u) << 16) |
+                      ((((run_mask >> lane) & 1u) ^ 1u) << 17);
+                d.y = (uint32_t)(((sub >> log2B) * TWp + (sub & (B - 1))) * (int)sizeof(cell));
+                s_run[r] = d;
+            }
             if (valid) {
-                s_key[lane] = cur.key;
                 const double xu = __dmul_rn(__dmul_rn(cur.um, cur.s), P.inv_du);
                 const double xv = __dmul_rn(__dmul_rn(cur.vm, cur.s), P.inv_du);
                 const int iu = (int)floor(__dadd_rn(xu, shift));
@@ -270,8 +354,8 @@ __global__ void __launch_bounds__(GRID_WARPS * 32) k_grid(const __grid_constant_
                 }
 #pragma unroll
                 for (int a = 0; a < S; ++a) {
-                    s_ku[lane * SP + a] = fu[a];
-                    s_kw[lane * S + a] = make_double2(cur.vr * fv[a], cur.vi * fv[a]);
+                    s_ku[a * KS + lane] = fu[a];
+                    s_kw[a * KS + lane] = make_double2(cur.vr * fv[a], cur.vi * fv[a]);
                 }
             }
             __syncwarp();
@@ -279,44 +363,53 @@ __global__ void __launch_bounds__(GRID_WARPS * 32) k_grid(const __grid_constant_
             load_vis(item_next, cur);
             item_next = load_item(b0 + 64 + lane, c_end);
 
-            // ---- walk the batch run by run (run_mask is warp-uniform) ----
-            const int nb = (int)((c_end - b0) < 32 ? (c_end - b0) : 32);
-            int j = 0;
-            while (j < nb) {
-                if ((run_mask >> j) & 1u) {
-                    const u64 kj = s_key[j];
-                    if (cur_cell != NOKEY) {
-                        flush_run();
-                        if ((kj >> sub_bits) != (cur_cell >> sub_bits)) flush_tile(cur_cell >> sub_bits);
+            // ---- walk the batch run by run: rank-4 updates of the footprint on the fp64 tensor pipe ----
+            uint2 d = lds_u2(a_run);
+            for (int r = 0; r < n_runs; ++r) {
+                const uint2 dn = lds_u2(a_run + 8u * (uint32_t)(r + 1));      // next descriptor (slot 33 exists)
+                const int j = (int)(d.x & 255u), end = j + (int)((d.x >> 8) & 255u);
+                if (!((d.x >> 17) & 1u)) {
+                    const bool new_tile = (d.x >> 16) & 1u;
+                    if (have_run) {
+                        run_store();
+                        if (new_tile) flush_tile(cur_tile);
                     }
-                    cur_cell = kj;
-                    const int sub = (int)(kj & ((1ull << sub_bits) - 1ull));
-                    cur_base = (sub >> log2B) * TWp + (sub & (B - 1));
+                    have_run = true;
+                    cur_off = d.y;
+                    if (new_tile) cur_tile = __shfl_sync(0xffffffffu, key, j) >> sub_bits;
+                    run_load();
                 }
-                const unsigned int rest = j < 31 ? (run_mask >> (j + 1)) : 0u;
-                int end = rest ? j + __ffs(rest) : nb;
-                end = end < nb ? end : nb;
-#pragma unroll 4
-                for (int jj = j; jj < end; ++jj) {
+                for (int jj = j; jj < end; jj += 4) {
+                    const bool live = jj + q < end;
+                    double2 av[MT];
+                    double bv[MT];
 #pragma unroll
-                    for (int rr = 0; rr < ROUNDS; ++rr) {
-                        const double2 k2 = pku[rr][jj * PW];
-                        const double2 w2 = pkw[rr][jj * S];
-                        acc[rr][0] = fma(w2.x, k2.x, acc[rr][0]);
-                        acc[rr][1] = fma(w2.y, k2.x, acc[rr][1]);
-                        acc[rr][2] = fma(w2.x, k2.y, acc[rr][2]);
-                        acc[rr][3] = fma(w2.y, k2.y, acc[rr][3]);
+                    for (int mt = 0; mt < MT; ++mt) {
+                        av[mt] = make_double2(0.0, 0.0);
+                        bv[mt] = 0.0;
+                        if (live && row_ok[mt]) {
+                            av[mt] = lds_d2(a_kw[mt] + (uint32_t)jj * 16u);
+                            bv[mt] = lds_d(a_ku[mt] + (uint32_t)jj * 8u);
+                        }
                     }
+#pragma unroll
+                    for (int mt = 0; mt < MT; ++mt)
+#pragma unroll
+                        for (int nt = 0; nt < MT; ++nt) {
+                            dmma884(c_re[mt][nt], av[mt].x, bv[nt]);
+                            dmma884(c_im[mt][nt], av[mt].y, bv[nt]);
+                        }
                 }
-                j = end;
+                d = dn;
             }
             __syncwarp();
         }
-        if (cur_cell != NOKEY) {
-            flush_run();
-            flush_tile(cur_cell >> sub_bits);
-            cur_cell = NOKEY;
+        if (have_run) {
+            run_store();
+            flush_tile(cur_tile);
+            have_run = false;
         }
+        last_key = NOKEY;
         chunk = __shfl_sync(0xffffffffu, next_chunk, 0);
     }
 }
