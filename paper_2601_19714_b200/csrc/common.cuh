@@ -73,6 +73,7 @@ struct rick_plan_s {
     // visibility of global plane pg reaches the B x B tile (tv, tu); rebuilt by every sort.  In rick_image
     // the zero-fill clears, and the row pass reads, only those tiles of an occupied row.
     unsigned char* tile_occ; size_t tile_occ_cap;
+    unsigned int* row_list; size_t row_list_cap;   // work list of the row pass (+ its counter at [cap])
     double* chan_scale;      // [C] device, s_c = f_c / c0
     WRange* wrange;          // [n_img] device
     int chan_cap;

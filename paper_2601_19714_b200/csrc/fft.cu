@@ -16,53 +16,67 @@ template <typename T, int LOG2N> struct RowCfg {
     static constexpr size_t SMEM = (size_t)RPC * (N + N / 16) * 2 * sizeof(T);
 };
 
+// Work list of the row pass: the groups of RPC consecutive rows (slot-major) with at least one occupied row.
+__global__ void __launch_bounds__(256) k_row_list(const unsigned char* __restrict__ occ, unsigned int n_groups, int rpc,
+                                                  unsigned int* __restrict__ list, unsigned int* __restrict__ count)
+{
+    const unsigned int gidx = blockIdx.x * 256u + threadIdx.x;
+    bool any = false;
+    if (gidx < n_groups)
+        for (int i = 0; i < rpc; ++i) any |= occ[(size_t)gidx * rpc + i] != 0;
+    // warp-aggregated append (the order of the list does not matter)
+    const unsigned int m = __ballot_sync(0xffffffffu, any);
+    if (!m) return;
+    const int lane = threadIdx.x & 31;
+    unsigned int base = 0;
+    if (lane == __ffs(m) - 1) base = atomicAdd(count, (unsigned)__popc(m));
+    base = __shfl_sync(0xffffffffu, base, __ffs(m) - 1);
+    if (any) list[base + __popc(m & ((1u << lane) - 1u))] = gidx;
+}
+
 template <typename T, int LOG2N>
-__global__ void __launch_bounds__(RowCfg<T, LOG2N>::THREADS)
+__global__ void __launch_bounds__(RowCfg<T, LOG2N>::THREADS, (RowCfg<T, LOG2N>::THREADS <= 256 ? 3 : 1))
 k_fft_rows(typename cplx_of<T>::type* __restrict__ stack,
-           const typename cplx_of<T>::type* __restrict__ tw, const unsigned char* __restrict__ occ,
-           const unsigned char* __restrict__ tocc, int log2B)
+           const typename cplx_of<T>::type* __restrict__ tw, const unsigned int* __restrict__ list,
+           const unsigned int* __restrict__ count, const unsigned char* __restrict__ tocc, int log2B)
 {
     typedef typename cplx_of<T>::type C;
     typedef RowCfg<T, LOG2N> K;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    // rows no visibility touches are zero in HBM and their transform is zero: skip them (the CTA's
-    // rows are skipped together, all or none, because the stages synchronise the whole CTA)
-    {
-        bool any = false;
-#pragma unroll
-        for (int i = 0; i < K::RPC; ++i) any |= occ[(size_t)blockIdx.x * K::RPC + i] != 0;
-        if (!any) return;
-    }
+    // Rows no visibility touches are zero in HBM and their transform is zero: they are not on the list.
+    // Persistent CTAs walk the list of occupied row groups.
     const int rl = threadIdx.x / K::NT, t = threadIdx.x - rl * K::NT;
     C* sm = reinterpret_cast<C*>(smem_raw) + (size_t)rl * (K::N + K::N / 16);
-    C* g = stack + ((size_t)blockIdx.x * K::RPC + rl) * K::N;
-    // only the tiles some footprint reaches hold gridded data (tile_occ); whatever else the row holds
-    // (rick_image leaves the previous transform there) is not read and counts as zero
     __shared__ unsigned char s_to[K::RPC][K::N / 8];
-    {
-        const int Tn = K::N >> log2B;
+    const int Tn = K::N >> log2B;
+    const unsigned int n_work = *count;
+    for (unsigned int w = blockIdx.x; w < n_work; w += gridDim.x) {
+        const size_t grp = list[w];
+        C* g = stack + (grp * K::RPC + rl) * K::N;
+        // only the tiles some footprint reaches hold gridded data (tile_occ); whatever else the row holds
+        // (rick_image leaves the previous transform there) is not read and counts as zero
         for (int i = threadIdx.x; i < K::RPC * Tn; i += K::THREADS) {
             const int a = i / Tn, ti = i - a * Tn;
-            const size_t R = (size_t)blockIdx.x * K::RPC + a;          // slot-major row
+            const size_t R = grp * K::RPC + a;          // slot-major row
             const size_t slot = R / K::N;
             const int row = (int)(R - slot * K::N);
             s_to[a][ti] = tocc[(slot * Tn + (size_t)(row >> log2B)) * Tn + ti];
         }
         __syncthreads();
-    }
-    C v[16];
+        C v[16];
 #pragma unroll
-    for (int e = 0; e < 16; ++e) {
-        const int i = t + K::NT * ((e + 8) & 15);
-        C x;
-        x.x = 0;
-        x.y = 0;
-        if (s_to[rl][i >> log2B]) x = g[i];
-        v[e] = x;
-    }
-    fft_thread<T, LOG2N>(v, t, sm, 1, 0, tw);
+        for (int e = 0; e < 16; ++e) {
+            const int i = t + K::NT * ((e + 8) & 15);
+            C x;
+            x.x = 0;
+            x.y = 0;
+            if (s_to[rl][i >> log2B]) x = g[i];
+            v[e] = x;
+        }
+        fft_thread<T, LOG2N>(v, t, sm, 1, 0, tw);
 #pragma unroll
-    for (int e = 0; e < 16; ++e) g[t + K::NT * ((e + 8) & 15)] = v[e];
+        for (int e = 0; e < 16; ++e) g[t + K::NT * ((e + 8) & 15)] = v[e];
+    }
 }
 
 template <typename T, int LOG2N> struct ColCfg {
@@ -105,8 +119,25 @@ static int launch_fft(rick_plan_t* p, int plane_first, int n_planes, int which) 
     if (which & 1) {
         RICK_CUDA(p, cudaFuncSetAttribute(k_fft_rows<T, LOG2N>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                           (int)KR::SMEM));
-        const unsigned int row_blocks = (unsigned int)((size_t)n_planes * KR::N / KR::RPC);
-        RICK_KERNEL(p, RK_FFT_ROWS, k_fft_rows<T, LOG2N><<<row_blocks, KR::THREADS, KR::SMEM, p->stream>>>((C*)p->stack, (const C*)p->twiddle, p->row_occ + (size_t)plane_first * p->N,
+        const unsigned int n_groups = (unsigned int)((size_t)n_planes * KR::N / KR::RPC);
+        if (n_groups > p->row_list_cap) {
+            if (p->row_list) cudaFree(p->row_list);
+            p->row_list = nullptr;
+            p->row_list_cap = 0;
+            RICK_CUDA(p, cudaMalloc(&p->row_list, sizeof(unsigned int) * ((size_t)n_groups + 1)));
+            p->row_list_cap = n_groups;
+        }
+        unsigned int* count = p->row_list + p->row_list_cap;
+        RICK_CUDA(p, cudaMemsetAsync(count, 0, sizeof(unsigned int), p->stream));
+        RICK_KERNEL(p, RK_ROW_OCC, k_row_list<<<(n_groups + 255) / 256, 256, 0, p->stream>>>(
+            p->row_occ + (size_t)plane_first * p->N, n_groups, KR::RPC, p->row_list, count));
+        int per_sm = 1;
+        RICK_CUDA(p, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_fft_rows<T, LOG2N>, KR::THREADS, KR::SMEM));
+        if (per_sm < 1) per_sm = 1;
+        unsigned int row_blocks = (unsigned int)(p->n_sm * per_sm);
+        if (row_blocks > n_groups) row_blocks = n_groups;
+        RICK_KERNEL(p, RK_FFT_ROWS, k_fft_rows<T, LOG2N><<<row_blocks, KR::THREADS, KR::SMEM, p->stream>>>(
+            (C*)p->stack, (const C*)p->twiddle, p->row_list, count,
             p->tile_occ + (size_t)plane_first * p->T * p->T, p->log2B));
     }
     if (which & 2) {

@@ -103,43 +103,36 @@ __device__ __forceinline__ void dmma884(double (&d)[2], double a, double b)
     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};"
                  : "+d"(d[0]), "+d"(d[1]) : "d"(a), "d"(b));
 }
-// two horizontally adjacent tile cells <-> registers (re0, re1), (im0, im1)
-template <typename GT> __device__ __forceinline__ void tile_load2(uint32_t a, double (&re)[2], double (&im)[2]);
-template <typename GT> __device__ __forceinline__ void tile_store2(uint32_t a, const double (&re)[2], const double (&im)[2]);
-template <> __device__ __forceinline__ void tile_load2<double>(uint32_t a, double (&re)[2], double (&im)[2])
+// one tile cell <-> the (re, im) register pair of an accumulator fragment
+template <typename GT> __device__ __forceinline__ void tile_load(uint32_t a, double (&c)[2]);
+template <typename GT> __device__ __forceinline__ void tile_store(uint32_t a, const double (&c)[2]);
+template <> __device__ __forceinline__ void tile_load<double>(uint32_t a, double (&c)[2])
 {
-    asm volatile("ld.shared.v2.f64 {%0, %1}, [%4];\n\tld.shared.v2.f64 {%2, %3}, [%4+16];"
-                 : "=d"(re[0]), "=d"(im[0]), "=d"(re[1]), "=d"(im[1]) : "r"(a));
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(c[0]), "=d"(c[1]) : "r"(a));
 }
-template <> __device__ __forceinline__ void tile_store2<double>(uint32_t a, const double (&re)[2], const double (&im)[2])
+template <> __device__ __forceinline__ void tile_store<double>(uint32_t a, const double (&c)[2])
 {
-    asm volatile("st.shared.v2.f64 [%4], {%0, %1};\n\tst.shared.v2.f64 [%4+16], {%2, %3};"
-                 :: "d"(re[0]), "d"(im[0]), "d"(re[1]), "d"(im[1]), "r"(a) : "memory");
+    asm volatile("st.shared.v2.f64 [%2], {%0, %1};" :: "d"(c[0]), "d"(c[1]), "r"(a) : "memory");
 }
-// fp32 grid: cells are 8 bytes and the row pitch is odd, so only 8-byte alignment
-template <> __device__ __forceinline__ void tile_load2<float>(uint32_t a, double (&re)[2], double (&im)[2])
+template <> __device__ __forceinline__ void tile_load<float>(uint32_t a, double (&c)[2])
 {
-    float t0, t1, t2, t3;
-    asm volatile("ld.shared.v2.f32 {%0, %1}, [%4];\n\tld.shared.v2.f32 {%2, %3}, [%4+8];"
-                 : "=f"(t0), "=f"(t1), "=f"(t2), "=f"(t3) : "r"(a));
-    re[0] = (double)t0;
-    im[0] = (double)t1;
-    re[1] = (double)t2;
-    im[1] = (double)t3;
+    float t0, t1;
+    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(t0), "=f"(t1) : "r"(a));
+    c[0] = (double)t0;
+    c[1] = (double)t1;
 }
-template <> __device__ __forceinline__ void tile_store2<float>(uint32_t a, const double (&re)[2], const double (&im)[2])
+template <> __device__ __forceinline__ void tile_store<float>(uint32_t a, const double (&c)[2])
 {
-    const float t0 = (float)re[0], t1 = (float)im[0], t2 = (float)re[1], t3 = (float)im[1];
-    asm volatile("st.shared.v2.f32 [%4], {%0, %1};\n\tst.shared.v2.f32 [%4+8], {%2, %3};"
-                 :: "f"(t0), "f"(t1), "f"(t2), "f"(t3), "r"(a) : "memory");
+    const float t0 = (float)c[0], t1 = (float)c[1];
+    asm volatile("st.shared.v2.f32 [%2], {%0, %1};" :: "f"(t0), "f"(t1), "r"(a) : "memory");
 }
 
 #define GRID_KS 36      // staging row stride in visibilities (32 + the overhang of the last group of 4)
 
 template <int S> __host__ __device__ constexpr size_t grid_stage_bytes()
 {
-    // kw[S][KS] double2 | ku[S][KS] double | run[34] uint2
-    return (size_t)S * GRID_KS * 16 + (size_t)S * GRID_KS * 8 + 34 * 8;
+    // kb[2S][KS] double | ka[S][KS] double | run[34] uint2
+    return (size_t)2 * S * GRID_KS * 8 + (size_t)S * GRID_KS * 8 + 34 * 8;
 }
 
 template <typename GT, int S>
@@ -148,7 +141,8 @@ __global__ void __launch_bounds__(GRID_WARPS * 32, 2) k_grid(const __grid_consta
     typedef typename cell_t<GT>::type cell;
     typedef unsigned long long u64;
     constexpr int H = (S - 1) / 2;
-    constexpr int MT = (S + 7) / 8;                 // 8 x 8 fragments per footprint axis
+    constexpr int MT = (S + 7) / 8;                 // 8-row fragments of the footprint
+    constexpr int NT = (2 * S + 7) / 8;             // 8-column fragments: columns are (cell a, re | im)
     constexpr int KS = GRID_KS;
     constexpr int DEG = RICK_KB_DEG;
     static_assert(DEG % 2 == 0, "even/odd Horner split assumes an even degree");
@@ -160,45 +154,48 @@ __global__ void __launch_bounds__(GRID_WARPS * 32, 2) k_grid(const __grid_consta
     const int sub_bits = 2 * log2B, idx_bits = P.idx_bits;
     const u64 idx_mask = (1ull << idx_bits) - 1ull;
 
-    // shared layout per warp: tile | kw[S][KS] | ku[S][KS] | run[34]
+    // shared layout per warp: tile | kb[2S][KS] | ka[S][KS] | run[34]
     const size_t tile_bytes = ((size_t)tile_cells * sizeof(cell) + 15) & ~(size_t)15;
     const size_t per_warp = tile_bytes + grid_stage_bytes<S>();
     unsigned char* wbase = smem_raw + (size_t)warp * per_warp;
     cell* tile = reinterpret_cast<cell*>(wbase);
-    double2* s_kw = reinterpret_cast<double2*>(wbase + tile_bytes);
-    double* s_ku = reinterpret_cast<double*>(s_kw + S * KS);
-    uint2* s_run = reinterpret_cast<uint2*>(s_ku + S * KS);
+    double* s_kb = reinterpret_cast<double*>(wbase + tile_bytes);      // [2 a + c][k] = g_u[a] (w V)_c of visibility k
+    double* s_ka = s_kb + 2 * S * KS;                                  // [b][k] = g_v[b] of visibility k
+    uint2* s_run = reinterpret_cast<uint2*>(s_ka + S * KS);
 
     cell zero;
     zero.x = 0;
     zero.y = 0;
     for (int i = lane; i < tile_cells; i += 32) tile[i] = zero;
-    for (int i = lane; i < S * KS; i += 32) {       // the overhang columns 32..35 stay finite (masked to 0 anyway)
-        s_ku[i] = 0.0;
-        s_kw[i] = make_double2(0.0, 0.0);
-    }
+    for (int i = lane; i < 3 * S * KS; i += 32) s_kb[i] = 0.0;      // kb and ka
     __syncwarp();
 
-    // Fragment roles (DMMA m8n8k4; M = footprint row b, N = footprint column a, K = visibility):
-    // lane = 4 g + q feeds A[g][q] = (w V) g_v[b = g + 8 mt] of visibility jj + q, B[q][g] = g_u[a = g + 8 nt]
-    // of the same visibility, and owns the cell pair (b = g + 8 mt, a = 8 nt + 2 q, + 1) of the footprint.
+    // Fragment roles (DMMA m8n8k4; M = footprint row b, N = (footprint column a, re | im), K = visibility):
+    // lane = 4 g + q feeds A[g][q] = g_v[b = g + 8 mt] of visibility jj + q and B[q][g] = g_u[a] (w V)_c,
+    // 2 a + c = g + 8 nt, of the same visibility; its two accumulators of fragment (mt, nt) are the (re, im)
+    // of footprint cell (b = g + 8 mt, a = 4 nt + q) -- the register pair a 16-byte tile access moves.
     const int g = lane >> 2, q = lane & 3;
-    bool has[MT][MT], row_ok[MT];
-    uint32_t a_tile[MT][MT], a_kw[MT], a_ku[MT];
-    double c_re[MT][MT][2], c_im[MT][MT][2];
+    bool has[MT][NT], row_ok[MT], col_ok[NT];
+    uint32_t a_tile[MT][NT], a_ka[MT], a_kb[NT];
+    double c[MT][NT][2];
 #pragma unroll
     for (int mt = 0; mt < MT; ++mt) {
         row_ok[mt] = g + 8 * mt < S;
-        const int rw = row_ok[mt] ? g + 8 * mt : 0;
-        a_kw[mt] = smem_u32(s_kw + rw * KS + q);
-        a_ku[mt] = smem_u32(s_ku + rw * KS + q);
-#pragma unroll
-        for (int nt = 0; nt < MT; ++nt) {
-            has[mt][nt] = row_ok[mt] && (8 * nt + 2 * q < S);
-            a_tile[mt][nt] = smem_u32(tile + (has[mt][nt] ? (g + 8 * mt) * TWp + 8 * nt + 2 * q : 0));
-            c_re[mt][nt][0] = c_re[mt][nt][1] = c_im[mt][nt][0] = c_im[mt][nt][1] = 0.0;
-        }
+        a_ka[mt] = smem_u32(s_ka + (row_ok[mt] ? g + 8 * mt : 0) * KS + q);
     }
+#pragma unroll
+    for (int nt = 0; nt < NT; ++nt) {
+        col_ok[nt] = g + 8 * nt < 2 * S;
+        a_kb[nt] = smem_u32(s_kb + (col_ok[nt] ? g + 8 * nt : 0) * KS + q);
+    }
+#pragma unroll
+    for (int mt = 0; mt < MT; ++mt)
+#pragma unroll
+        for (int nt = 0; nt < NT; ++nt) {
+            has[mt][nt] = row_ok[mt] && (4 * nt + q < S);
+            a_tile[mt][nt] = smem_u32(tile + (has[mt][nt] ? (g + 8 * mt) * TWp + 4 * nt + q : 0));
+            c[mt][nt][0] = c[mt][nt][1] = 0.0;
+        }
     const uint32_t a_run = smem_u32(s_run);
 
     const long long v_begin = P.plane_start[P.plane_first];
@@ -219,15 +216,15 @@ __global__ void __launch_bounds__(GRID_WARPS * 32, 2) k_grid(const __grid_consta
 #pragma unroll
         for (int mt = 0; mt < MT; ++mt)
 #pragma unroll
-            for (int nt = 0; nt < MT; ++nt)
-                if (has[mt][nt]) tile_load2<GT>(a_tile[mt][nt] + cur_off, c_re[mt][nt], c_im[mt][nt]);
+            for (int nt = 0; nt < NT; ++nt)
+                if (has[mt][nt]) tile_load<GT>(a_tile[mt][nt] + cur_off, c[mt][nt]);
     };
     auto run_store = [&]() {
 #pragma unroll
         for (int mt = 0; mt < MT; ++mt)
 #pragma unroll
-            for (int nt = 0; nt < MT; ++nt)
-                if (has[mt][nt]) tile_store2<GT>(a_tile[mt][nt] + cur_off, c_re[mt][nt], c_im[mt][nt]);
+            for (int nt = 0; nt < NT; ++nt)
+                if (has[mt][nt]) tile_store<GT>(a_tile[mt][nt] + cur_off, c[mt][nt]);
     };
     // tile -> HBM, once per (tile, chunk)
     auto flush_tile = [&](u64 tkey) {
@@ -354,8 +351,9 @@ __global__ void __launch_bounds__(GRID_WARPS * 32, 2) k_grid(const __grid_consta
                 }
 #pragma unroll
                 for (int a = 0; a < S; ++a) {
-                    s_ku[a * KS + lane] = fu[a];
-                    s_kw[a * KS + lane] = make_double2(cur.vr * fv[a], cur.vi * fv[a]);
+                    s_ka[a * KS + lane] = fv[a];
+                    s_kb[(2 * a) * KS + lane] = cur.vr * fu[a];
+                    s_kb[(2 * a + 1) * KS + lane] = cur.vi * fu[a];
                 }
             }
             __syncwarp();
@@ -381,24 +379,21 @@ __global__ void __launch_bounds__(GRID_WARPS * 32, 2) k_grid(const __grid_consta
                 }
                 for (int jj = j; jj < end; jj += 4) {
                     const bool live = jj + q < end;
-                    double2 av[MT];
-                    double bv[MT];
+                    double av[MT], bv[NT];
 #pragma unroll
                     for (int mt = 0; mt < MT; ++mt) {
-                        av[mt] = make_double2(0.0, 0.0);
-                        bv[mt] = 0.0;
-                        if (live && row_ok[mt]) {
-                            av[mt] = lds_d2(a_kw[mt] + (uint32_t)jj * 16u);
-                            bv[mt] = lds_d(a_ku[mt] + (uint32_t)jj * 8u);
-                        }
+                        av[mt] = 0.0;
+                        if (live && row_ok[mt]) av[mt] = lds_d(a_ka[mt] + (uint32_t)jj * 8u);
+                    }
+#pragma unroll
+                    for (int nt = 0; nt < NT; ++nt) {
+                        bv[nt] = 0.0;
+                        if (live && col_ok[nt]) bv[nt] = lds_d(a_kb[nt] + (uint32_t)jj * 8u);
                     }
 #pragma unroll
                     for (int mt = 0; mt < MT; ++mt)
 #pragma unroll
-                        for (int nt = 0; nt < MT; ++nt) {
-                            dmma884(c_re[mt][nt], av[mt].x, bv[nt]);
-                            dmma884(c_im[mt][nt], av[mt].y, bv[nt]);
-                        }
+                        for (int nt = 0; nt < NT; ++nt) dmma884(c[mt][nt], av[mt], bv[nt]);
                 }
                 d = dn;
             }
