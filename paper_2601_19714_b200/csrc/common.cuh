@@ -59,8 +59,10 @@ struct rick_plan_s {
     unsigned long long *items, *items_a, *items_b;
     unsigned long long* sorted_items;      // points at items / items_a / items_b after the sort
     int idx_bits, key_bits;                // item layout of the last rick_grid / rick_image
-    uint32_t* hist; size_t hist_cap;
-    uint32_t* scan_tmp; size_t scan_cap;
+    // onesweep radix passes: digit histograms + tickets, digit bases, look-back status words
+    unsigned int* os_small;
+    unsigned long long* os_gbase;
+    unsigned long long* os_status; size_t os_status_cap;
     int64_t* plane_start;    // [n_planes_total + 1] offsets into the sorted order
     int64_t plane_start_cap;
     // row occupancy: row_occ[pg][row] = 1 when some visibility of global

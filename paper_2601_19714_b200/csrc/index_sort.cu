@@ -88,6 +88,14 @@ __global__ void k_wrange_finish(const DevCounters* c, const double* __restrict__
     out[g] = w;
 }
 
+// Radix passes over the key bits (<= 8-bit digits), shared by a1 (histograms) and a2 (passes).
+#define RS_MAXPASS 8
+struct RadixPlan {
+    int npass;
+    int shift[RS_MAXPASS];          // of the KEY (the item shift is idx_bits + shift)
+    unsigned int mask[RS_MAXPASS];
+};
+
 // ------------------------------------------------------------------------------------------
 // a1: one thread per visibility k = r*C + c.  Writes the sort item (key << idx_bits) | k.
 // ------------------------------------------------------------------------------------------
@@ -96,8 +104,14 @@ k_index_key(const double* __restrict__ uvw, const float* __restrict__ wgt,
             const double* __restrict__ chan_scale, const WRange* __restrict__ wrange,
             unsigned int M, unsigned int C, int N, int Nw, int h, int log2B, int T, int cube,
             double inv_du, int idx_bits, unsigned long long key_dropped,
-            unsigned long long* __restrict__ items, DevCounters* cnt)
+            unsigned long long* __restrict__ items, DevCounters* cnt, RadixPlan rp,
+            unsigned int* __restrict__ ghist)
 {
+    // digit histograms of ALL radix passes (they do not depend on the order of the items), so that
+    // every pass is one read + one write of the items (k_radix_onesweep)
+    __shared__ unsigned int s_h[RS_MAXPASS][256];
+    for (int i = threadIdx.x; i < RS_MAXPASS * 256; i += blockDim.x) (&s_h[0][0])[i] = 0u;
+    __syncthreads();
     // grid-stride: statistics stay in registers, one set of atomics per block (same-address
     // atomics per warp made this kernel atomic-bound)
     unsigned int on = 0, off = 0;
@@ -132,6 +146,14 @@ k_index_key(const double* __restrict__ uvw, const float* __restrict__ wgt,
             off++;
         }
         items[k] = (key << idx_bits) | (unsigned long long)k;
+#pragma unroll
+        for (int ps = 0; ps < RS_MAXPASS; ++ps)
+            if (ps < rp.npass) atomicAdd(&s_h[ps][(unsigned int)(key >> rp.shift[ps]) & rp.mask[ps]], 1u);
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < rp.npass * 256; i += blockDim.x) {
+        const unsigned int v = (&s_h[0][0])[i];
+        if (v) atomicAdd(&ghist[i], v);
     }
     // block-reduced statistics
     __shared__ unsigned int s_on[8], s_off[8];
@@ -166,56 +188,65 @@ k_index_key(const double* __restrict__ uvw, const float* __restrict__ wgt,
 // ------------------------------------------------------------------------------------------
 // a2: LSD radix sort of the 64-bit items over their key bits, <= 8-bit digits, stable.  The
 // visibility index sits in the low idx_bits of an item and is never a digit: stability keeps
-// equal keys in index order, so the sorted low parts ARE the permutation.
+// equal keys in index order, so the sorted low parts ARE the permutation.  The digit histograms of
+// all passes come from a1 (k_index_key); each pass is then ONE kernel that reads and writes the
+// items once (k_radix_onesweep).
 // ------------------------------------------------------------------------------------------
 #define RS_THREADS 256
 #define RS_ITEMS 16
 #define RS_TILE (RS_THREADS * RS_ITEMS)
 typedef unsigned long long u64;
 
-__global__ void __launch_bounds__(RS_THREADS)
-k_radix_hist(const u64* __restrict__ items, unsigned int M, int shift, uint32_t mask, int nbins,
-             uint32_t* __restrict__ hist, unsigned int nblocks)
+// exclusive scan over the digits of each pass: gbase[ps][d] = number of items whose digit of pass ps is < d
+__global__ void __launch_bounds__(256) k_digit_bases(const unsigned int* __restrict__ ghist, int npass,
+                                                     unsigned long long* __restrict__ gbase)
 {
-    __shared__ uint32_t hs[256];
-    hs[threadIdx.x] = 0;
-    __syncthreads();
-    const unsigned long long base = (unsigned long long)blockIdx.x * RS_TILE;
-    u64 it[RS_ITEMS];
-#pragma unroll
-    for (int i = 0; i < RS_ITEMS; ++i) {
-        const unsigned long long idx = base + (unsigned)i * RS_THREADS + threadIdx.x;
-        it[i] = idx < M ? items[idx] : ~0ull;
+    __shared__ unsigned long long ws[8];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (int ps = 0; ps < npass; ++ps) {
+        const unsigned long long v = ghist[ps * 256 + threadIdx.x];
+        unsigned long long x = v;
+        for (int o = 1; o < 32; o <<= 1) {
+            const unsigned long long y = __shfl_up_sync(0xffffffffu, x, o);
+            if (lane >= o) x += y;
+        }
+        if (lane == 31) ws[warp] = x;
+        __syncthreads();
+        unsigned long long off = 0;
+        for (int w = 0; w < warp; ++w) off += ws[w];
+        gbase[ps * 256 + threadIdx.x] = off + x - v;
+        __syncthreads();
     }
-#pragma unroll
-    for (int i = 0; i < RS_ITEMS; ++i) {
-        const unsigned long long idx = base + (unsigned)i * RS_THREADS + threadIdx.x;
-        const bool valid = idx < M;
-        const uint32_t d = valid ? ((uint32_t)(it[i] >> shift) & mask) : 0xFFFFu;
-        const unsigned int m = __match_any_sync(0xffffffffu, d);
-        if (valid && (int)(threadIdx.x & 31) == __ffs(m) - 1) atomicAdd(&hs[d], (uint32_t)__popc(m));
-    }
-    __syncthreads();
-    if ((int)threadIdx.x < nbins) hist[(size_t)threadIdx.x * nblocks + blockIdx.x] = hs[threadIdx.x];
 }
 
-// One tile of RS_TILE items per block: stable rank of every item inside the tile (warp match +
-// per-warp digit counters), the tile is reordered by digit in shared memory, then written out
-// position by position -- consecutive threads write consecutive addresses of one digit's run, so
-// the stores coalesce (scattered 8-byte stores paid one L1 tag cycle per line: 32 per warp store).
+// One radix pass in one read + one write of the items ("onesweep"): the global digit bases are known
+// (k_digit_bases); a tile ranks its items by digit (stable: warp match + per-warp digit counters), publishes
+// its digit counts and finds the counts of all EARLIER tiles by decoupled look-back through `status`
+// (one 64-bit word per (tile, digit): flag << 62 | count; flag 1 = this tile's count, 2 = inclusive prefix
+// over tiles 0..this).  Tiles are taken in order from a ticket counter, so every predecessor of a running
+// tile is running or done and the look-back cannot deadlock.  The tile is then reordered by digit in shared
+// memory and written out position by position: consecutive threads write consecutive addresses of one
+// digit's run, so the stores coalesce.
+#define OS_AGG (1ull << 62)
+#define OS_INC (2ull << 62)
+#define OS_VAL ((1ull << 62) - 1ull)
 __global__ void __launch_bounds__(RS_THREADS, 3)
-k_radix_scatter(const u64* __restrict__ in, u64* __restrict__ out, unsigned int M, int shift,
-                uint32_t mask, int nbins, const uint32_t* __restrict__ hist_scanned, unsigned int nblocks)
+k_radix_onesweep(const u64* __restrict__ in, u64* __restrict__ out, unsigned int M, int shift, uint32_t mask,
+                 int nbins, const unsigned long long* __restrict__ gbase, volatile unsigned long long* status,
+                 unsigned int* __restrict__ ticket)
 {
     __shared__ uint32_t cnt[RS_THREADS / 32][256];
     __shared__ u64 buf[RS_TILE];
     __shared__ uint32_t dig_start[256];
     __shared__ long long gofs[256];
     __shared__ uint32_t wsum[RS_THREADS / 32];
+    __shared__ unsigned int s_tile;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (threadIdx.x == 0) s_tile = atomicAdd(ticket, 1u);
     for (int i = threadIdx.x; i < (RS_THREADS / 32) * 256; i += RS_THREADS) (&cnt[0][0])[i] = 0;
     __syncthreads();
-    const unsigned long long tile0 = (unsigned long long)blockIdx.x * RS_TILE;
+    const unsigned int tile = s_tile;
+    const unsigned long long tile0 = (unsigned long long)tile * RS_TILE;
     const unsigned long long base = tile0 + (unsigned)warp * (32 * RS_ITEMS);
     u64 it[RS_ITEMS];
     uint32_t rank[RS_ITEMS];
@@ -252,6 +283,28 @@ k_radix_scatter(const u64* __restrict__ in, u64* __restrict__ out, unsigned int 
             total += t;
         }
     }
+    // publish this tile's count of digit d, then sum the earlier tiles' (look-back)
+    volatile unsigned long long* st = status + (size_t)tile * 256 + threadIdx.x;
+    unsigned long long excl = 0;
+    if ((int)threadIdx.x < nbins) {
+        if (tile == 0) {
+            *st = OS_INC | (unsigned long long)total;
+        } else {
+            *st = OS_AGG | (unsigned long long)total;
+            const volatile unsigned long long* q = st - 256;
+            for (unsigned int back = tile; back > 0; --back, q -= 256) {
+                unsigned long long v;
+                unsigned int spins = 0;
+                while (((v = *q) >> 62) == 0ull) {
+                    __nanosleep(40);
+                    if (++spins > (1u << 24)) __trap();      // a lost predecessor: fail loudly, never hang
+                }
+                excl += v & OS_VAL;
+                if ((v >> 62) == 2ull) break;
+            }
+            *st = OS_INC | (excl + (unsigned long long)total);
+        }
+    }
     uint32_t x = total;
     for (int o = 1; o < 32; o <<= 1) {
         const uint32_t y = __shfl_up_sync(0xffffffffu, x, o);
@@ -265,7 +318,7 @@ k_radix_scatter(const u64* __restrict__ in, u64* __restrict__ out, unsigned int 
     const uint32_t start = woff + x - total;
     dig_start[threadIdx.x] = start;
     if ((int)threadIdx.x < nbins)
-        gofs[threadIdx.x] = (long long)hist_scanned[(size_t)threadIdx.x * nblocks + blockIdx.x] - (long long)start;
+        gofs[threadIdx.x] = (long long)(gbase[threadIdx.x] + excl) - (long long)start;
     __syncthreads();
 #pragma unroll
     for (int i = 0; i < RS_ITEMS; ++i) {
@@ -285,83 +338,6 @@ k_radix_scatter(const u64* __restrict__ in, u64* __restrict__ out, unsigned int 
             const uint32_t d = (uint32_t)(v >> shift) & mask;
             out[gofs[d] + (long long)pos] = v;
         }
-    }
-}
-
-// exclusive scan of a u32 array: (1) per-block sums, (2) scan of the sums, (3) apply
-#define SC_THREADS 1024
-#define SC_ITEMS 4
-#define SC_TILE (SC_THREADS * SC_ITEMS)
-
-__device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t* total)
-{
-    __shared__ uint32_t ws[32];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    uint32_t x = v;
-    for (int o = 1; o < 32; o <<= 1) {
-        uint32_t y = __shfl_up_sync(0xffffffffu, x, o);
-        if (lane >= o) x += y;
-    }
-    if (lane == 31) ws[warp] = x;
-    __syncthreads();
-    if (warp == 0) {
-        uint32_t s = ws[lane];
-        for (int o = 1; o < 32; o <<= 1) {
-            uint32_t y = __shfl_up_sync(0xffffffffu, s, o);
-            if (lane >= o) s += y;
-        }
-        ws[lane] = s;
-    }
-    __syncthreads();
-    const uint32_t warp_off = warp ? ws[warp - 1] : 0;
-    *total = ws[31];
-    const uint32_t r = warp_off + x - v;
-    __syncthreads();
-    return r;
-}
-
-__global__ void __launch_bounds__(SC_THREADS)
-k_scan_reduce(const uint32_t* __restrict__ a, size_t n, uint32_t* __restrict__ sums)
-{
-    const size_t base = (size_t)blockIdx.x * SC_TILE + (size_t)threadIdx.x * SC_ITEMS;
-    uint32_t s = 0;
-#pragma unroll
-    for (int i = 0; i < SC_ITEMS; ++i)
-        if (base + i < n) s += a[base + i];
-    uint32_t tot;
-    block_exclusive_scan(s, &tot);
-    if (threadIdx.x == 0) sums[blockIdx.x] = tot;
-}
-
-__global__ void __launch_bounds__(SC_THREADS) k_scan_top(uint32_t* __restrict__ sums, unsigned int nb)
-{
-    uint32_t carry = 0;
-    for (unsigned int b0 = 0; b0 < nb; b0 += SC_THREADS) {
-        const unsigned int i = b0 + threadIdx.x;
-        const uint32_t v = i < nb ? sums[i] : 0;
-        uint32_t tot;
-        const uint32_t e = block_exclusive_scan(v, &tot);
-        if (i < nb) sums[i] = carry + e;
-        carry += tot;
-    }
-}
-
-__global__ void __launch_bounds__(SC_THREADS)
-k_scan_apply(uint32_t* __restrict__ a, size_t n, const uint32_t* __restrict__ sums)
-{
-    const size_t base = (size_t)blockIdx.x * SC_TILE + (size_t)threadIdx.x * SC_ITEMS;
-    uint32_t v[SC_ITEMS], s = 0;
-#pragma unroll
-    for (int i = 0; i < SC_ITEMS; ++i) {
-        v[i] = base + i < n ? a[base + i] : 0;
-        s += v[i];
-    }
-    uint32_t tot;
-    uint32_t e = block_exclusive_scan(s, &tot) + sums[blockIdx.x];
-#pragma unroll
-    for (int i = 0; i < SC_ITEMS; ++i) {
-        if (base + i < n) a[base + i] = e;
-        e += v[i];
     }
 }
 
@@ -432,17 +408,6 @@ k_tile_occupancy(const u64* __restrict__ sitems, const long long* __restrict__ p
 }
 
 // ------------------------------------------------------------------------------------------
-static int ensure_u32(rick_plan_t* p, uint32_t** buf, size_t* cap, size_t need)
-{
-    if (*cap >= need) return RICK_OK;
-    if (*buf) cudaFree(*buf);
-    *buf = nullptr;
-    *cap = 0;
-    RICK_CUDA(p, cudaMalloc(buf, sizeof(uint32_t) * need));
-    *cap = need;
-    return RICK_OK;
-}
-
 int rick_index_sort(rick_plan_t* p, const double* uvw_m, const float* weights)
 {
     cudaStream_t st = p->stream;
@@ -462,44 +427,52 @@ int rick_index_sort(rick_plan_t* p, const double* uvw_m, const float* weights)
     p->sorted_items = p->items;
     if (M > 0) {
         const unsigned long long key_dropped = (1ull << p->key_bits) - 1ull;
+        // digits of the passes: the key bits split evenly over ceil(bits / 8) passes
+        RadixPlan rp;
+        memset(&rp, 0, sizeof(rp));
+        const int bits = p->key_bits;
+        rp.npass = (bits + 7) / 8;
+        int nb_bits[RS_MAXPASS];
+        for (int pass = 0, done = 0; pass < rp.npass; ++pass) {
+            nb_bits[pass] = (bits - done + (rp.npass - pass) - 1) / (rp.npass - pass);
+            rp.shift[pass] = done;
+            rp.mask[pass] = (1u << nb_bits[pass]) - 1u;
+            done += nb_bits[pass];
+        }
+        // scratch of the onesweep passes: ghist[8][256] u32 | ticket[8] u32, gbase[8][256] u64,
+        // status[npass][nblocks][256] u64 (cleared by every sort)
+        const unsigned int nblocks = (M + RS_TILE - 1) / RS_TILE;
+        const size_t n_status = (size_t)rp.npass * nblocks * 256;
+        if (!p->os_small) {
+            RICK_CUDA(p, cudaMalloc(&p->os_small, sizeof(unsigned int) * (RS_MAXPASS * 256 + RS_MAXPASS)));
+            RICK_CUDA(p, cudaMalloc(&p->os_gbase, sizeof(unsigned long long) * RS_MAXPASS * 256));
+        }
+        if (n_status > p->os_status_cap) {
+            if (p->os_status) cudaFree(p->os_status);
+            p->os_status = nullptr;
+            p->os_status_cap = 0;
+            RICK_CUDA(p, cudaMalloc(&p->os_status, sizeof(unsigned long long) * n_status));
+            p->os_status_cap = n_status;
+        }
+        RICK_CUDA(p, cudaMemsetAsync(p->os_small, 0, sizeof(unsigned int) * (RS_MAXPASS * 256 + RS_MAXPASS), st));
+        RICK_CUDA(p, cudaMemsetAsync(p->os_status, 0, sizeof(unsigned long long) * n_status, st));
         {
             unsigned int nb = (M + 255) / 256;
             if (nb > (unsigned)p->n_sm * 8u) nb = (unsigned)p->n_sm * 8u;
             RICK_KERNEL(p, RK_INDEX_KEY, k_index_key<<<nb, 256, 0, st>>>(uvw_m, weights, p->chan_scale, p->wrange, M,
                                                     (unsigned)p->C, p->N, p->Nw, p->h, p->log2B, p->T,
                                                     p->d.cube, p->inv_du, p->idx_bits, key_dropped, p->items,
-                                                    p->counters));
+                                                    p->counters, rp, p->os_small));
         }
-        const int bits = p->key_bits;
-        const int npass = (bits + 7) / 8;
-        const unsigned int nblocks = (M + RS_TILE - 1) / RS_TILE;
-        int rc = ensure_u32(p, &p->hist, &p->hist_cap, (size_t)256 * nblocks);
-        if (rc) return rc;
-        const size_t n_hist_max = (size_t)256 * nblocks;
-        const unsigned int nsb_max = (unsigned int)((n_hist_max + SC_TILE - 1) / SC_TILE);
-        rc = ensure_u32(p, &p->scan_tmp, &p->scan_cap, nsb_max);
-        if (rc) return rc;
-
+        RICK_KERNEL(p, RK_SCAN, k_digit_bases<<<1, 256, 0, st>>>(p->os_small, rp.npass, p->os_gbase));
         const u64* in = (const u64*)p->items;
         u64* bufs[2] = {(u64*)p->items_a, (u64*)p->items_b};
-        int shift = p->idx_bits;
-        int done = 0;
-        for (int pass = 0; pass < npass; ++pass) {
-            const int nb_bits = (bits - done + (npass - pass) - 1) / (npass - pass);
-            const int nbins = 1 << nb_bits;
-            const uint32_t mask = (uint32_t)(nbins - 1);
-            RICK_KERNEL(p, RK_RADIX_HIST, k_radix_hist<<<nblocks, RS_THREADS, 0, st>>>(in, M, shift, mask, nbins, p->hist, nblocks));
-            const size_t n_hist = (size_t)nbins * nblocks;
-            const unsigned int nsb = (unsigned int)((n_hist + SC_TILE - 1) / SC_TILE);
-            RICK_KERNEL(p, RK_SCAN, k_scan_reduce<<<nsb, SC_THREADS, 0, st>>>(p->hist, n_hist, p->scan_tmp));
-            RICK_KERNEL(p, RK_SCAN, k_scan_top<<<1, SC_THREADS, 0, st>>>(p->scan_tmp, nsb));
-            RICK_KERNEL(p, RK_SCAN, k_scan_apply<<<nsb, SC_THREADS, 0, st>>>(p->hist, n_hist, p->scan_tmp));
+        for (int pass = 0; pass < rp.npass; ++pass) {
             u64* o = bufs[pass & 1];
-            RICK_KERNEL(p, RK_RADIX_SCATTER, k_radix_scatter<<<nblocks, RS_THREADS, 0, st>>>(in, o, M, shift, mask, nbins,
-                                                          p->hist, nblocks));
+            RICK_KERNEL(p, RK_RADIX_SCATTER, k_radix_onesweep<<<nblocks, RS_THREADS, 0, st>>>(
+                in, o, M, p->idx_bits + rp.shift[pass], rp.mask[pass], 1 << nb_bits[pass], p->os_gbase + pass * 256,
+                p->os_status + (size_t)pass * nblocks * 256, p->os_small + RS_MAXPASS * 256 + pass));
             in = o;
-            shift += nb_bits;
-            done += nb_bits;
         }
         p->sorted_items = (unsigned long long*)in;
     }
