@@ -96,6 +96,7 @@ struct rick_plan_s {
     // N = 4096 fp64 column kernels (fft_cols12.cu): TMA tensor map over the resident stack
     int cols12_ok;
     alignas(64) unsigned char cols12_tmap[128];
+    alignas(64) unsigned char cols12_tmap_sw[128];   // same view, 32-byte swizzle (k_cols12_wcorrect)
 
     // host-buffer staging for rick_image_host
     void* st_vis; size_t st_vis_cap;

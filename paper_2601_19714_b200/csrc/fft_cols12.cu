@@ -32,7 +32,7 @@ constexpr int C12_LOG2N = 12, C12_N = 1 << C12_LOG2N, C12_NT = C12_N / 16, C12_W
 constexpr int C12_THREADS = C12_NT * C12_WC, C12_STRIPS = C12_N / C12_WC;
 constexpr uint32_t C12_STAGE_BYTES = (uint32_t)C12_N * C12_WC * 16u;                        // 131072
 constexpr size_t C12_EX_BYTES = (size_t)C12_WC * (C12_N + C12_N / 16) * sizeof(double);     // 69632
-constexpr size_t C12_SMEM = C12_STAGE_BYTES + C12_EX_BYTES + 64;
+constexpr size_t C12_SMEM = C12_STAGE_BYTES + C12_EX_BYTES + 64 + 1024;   // + slack for the 1024-byte alignment
 
 struct Roles {
     int w, c, hh, t1, t2, t3;
@@ -107,49 +107,110 @@ k_cols12_fft(const __grid_constant__ CUtensorMap tmap, double2* __restrict__ sta
     }
 }
 
+// ---------------------------------------------------------------------------------------------------
 // a4 column pass fused with a5 (+ a6 when taper != nullptr).
+//
+// The CTA is two COLUMN GROUPS of 256 threads: group g (warps 8g .. 8g+7) owns column g of the strip,
+// thread role (w, hh) = (tg >> 4, tg & 15).  The groups share the TMA staging of the item but run out of
+// phase: group 1 may read the staging only after group 0 has (named barrier 3), and from there on each
+// group synchronises only with itself (named barrier 1 + g), so one group's shared-memory exchange runs
+// under the other group's butterflies (with one 512-thread lock step the item time was the SUM of its
+// fp64 time and its shared-memory time, profiles/r1b_ncu_full.md).  The staging is 32-byte swizzled by
+// the tensor map (16-byte chunk ^= bit 7 of the byte offset) so that a group's 16-byte reads at a
+// 32-byte pitch are bank-conflict free.  `full` = TMA landed; `empty` = all 16 warps have read the
+// staging, waited for by the one thread that issues the next load.
+struct RolesG {
+    int g, w, hh, wl, t1, t2;
+};
+__device__ __forceinline__ RolesG roles_g()
+{
+    RolesG r;
+    const int tg = threadIdx.x & 255;
+    r.g = threadIdx.x >> 8;
+    r.w = tg >> 4;
+    r.hh = tg & 15;
+    r.wl = (threadIdx.x >> 4) & 1;
+    r.t1 = r.w + 16 * r.hh;      // stage 1: rows t1 + 256 e
+    r.t2 = 16 * r.w + r.hh;      // stages 2 and 3; outputs X[t2 + 256 r]
+    return r;
+}
+
+__device__ __forceinline__ void strip_fft_g(double2 (&v)[16], const RolesG& R, const double2* __restrict__ stg,
+                                            double* __restrict__ ex, const double2* __restrict__ tw,
+                                            unsigned long long* full, unsigned long long* empty, uint32_t& parity,
+                                            bool issue_next, const CUtensorMap* tmap, int next_strip, int next_plane)
+{
+    if (R.g == 1) named_bar_sync(3, 512);        // group 0 has read the staging of this item
+    mbar_wait(full, parity);
+    // centring on input = rotation by N/2 = element e <- slot (e + 8) mod 16; swizzled chunk of column g
+    const int sw = R.g ^ ((R.hh >> 2) & 1);
+#pragma unroll
+    for (int e = 0; e < 16; ++e) v[e] = stg[(((e + 8) & 15) * 256 + R.w * 16 + R.hh) * 2 + sw];
+    if (R.g == 0) named_bar_arrive(3, 512);
+    __syncwarp();
+    if ((threadIdx.x & 31) == 0) mbar_arrive(empty);
+    if (threadIdx.x == 256 && issue_next) {
+        mbar_wait(empty, parity);
+        mbar_arrive_expect_tx(full, C12_STAGE_BYTES);
+        tma_load_5d(const_cast<double2*>(stg), tmap, full, 4 * next_strip, 0, 0, 0, next_plane);
+    }
+    parity ^= 1u;
+    bfly16<double, C12_LOG2N, 0>(v, R.t1, tw);
+    named_bar_sync(1 + R.g, 256);                // the group's reads of the previous item's exchange are done
+    xchg16_warp_grp(v, ex + (size_t)(threadIdx.x >> 5) * (2 * 16 * 17), R.wl, R.hh);
+    bfly16<double, C12_LOG2N, 4>(v, R.t2, tw);
+    named_bar_sync(1 + R.g, 256);                // every warp of the group is done with its private region
+    xchg16_grp(v, ex + (size_t)R.g * (C12_N + C12_N / 16), R.t2, 1 + R.g);
+    bfly16<double, C12_LOG2N, 8>(v, R.t2, tw);
+}
+
 __global__ void __launch_bounds__(C12_THREADS, 1)
 k_cols12_wcorrect(const __grid_constant__ CUtensorMap tmap, const double2* __restrict__ tw, int n_planes,
                   int z_first, double dl, const WRange* __restrict__ wr, double* __restrict__ image,
                   int accumulate, const double* __restrict__ taper, int strip_begin, int strip_end)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    double2* stg = reinterpret_cast<double2*>(smem_raw);
-    double* ex = reinterpret_cast<double*>(smem_raw + C12_STAGE_BYTES);
-    unsigned long long* bar = reinterpret_cast<unsigned long long*>(smem_raw + C12_STAGE_BYTES + C12_EX_BYTES);
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem_raw + C12_STAGE_BYTES + C12_EX_BYTES + 16);
-    const Roles R = roles();
+    // the swizzle pattern is a function of the shared-memory ADDRESS: staging on a 1024-byte boundary
+    unsigned char* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
+    double2* stg = reinterpret_cast<double2*>(smem);
+    double* ex = reinterpret_cast<double*>(smem + C12_STAGE_BYTES);
+    unsigned long long* full = reinterpret_cast<unsigned long long*>(smem + C12_STAGE_BYTES + C12_EX_BYTES);
+    unsigned long long* empty = full + 1;
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + C12_STAGE_BYTES + C12_EX_BYTES + 16);
+    const RolesG R = roles_g();
+    const int warp = threadIdx.x >> 5;
     if (threadIdx.x == 0) {
-        mbar_init(bar, 1);
+        mbar_init(full, 1);
+        mbar_init(empty, C12_THREADS / 32);
         mbar_fence_init();
     }
-    if (R.w == 0) tmem_alloc_all(tmem_slot);
+    if (warp == 0) tmem_alloc_all(tmem_slot);
     tmem_fence_before_sync();
     __syncthreads();
     tmem_fence_after_sync();
     const uint32_t tbase = *tmem_slot;
     // warps w, w+4, w+8, w+12 share the TMEM lanes 32 (w%4) ..; 128 columns each: S | step
-    const uint32_t tS = tbase + ((uint32_t)(32 * (R.w & 3)) << 16) + (uint32_t)((R.w >> 2) * 128);
+    const uint32_t tS = tbase + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)((warp >> 2) * 128);
     const uint32_t tStep = tS + 64;
 
     int strip = strip_begin + (int)blockIdx.x;
     if (threadIdx.x == 0 && strip < strip_end) {
-        mbar_arrive_expect_tx(bar, C12_STAGE_BYTES);
-        tma_load_5d(stg, &tmap, bar, 4 * strip, 0, 0, 0, n_planes - 1);
+        mbar_arrive_expect_tx(full, C12_STAGE_BYTES);
+        tma_load_5d(stg, &tmap, full, 4 * strip, 0, 0, 0, n_planes - 1);
     }
     uint32_t parity = 0;
     const double dw = wr->dw;
     const double w_first = wr->w_min + ((double)z_first + 0.5) * dw;
     for (; strip < strip_end; strip += gridDim.x) {
-        const int p = strip * C12_WC + R.c;
+        const int p = strip * C12_WC + R.g;
         const double l = (double)(p - C12_N / 2) * dl;
-        // step = exp(2 pi i dw (n-1)) of this thread's 16 pixels (rows t3 + 256 ((e+8)&15)) -> TMEM
+        // step = exp(2 pi i dw (n-1)) of this thread's 16 pixels (rows t2 + 256 ((e+8)&15)) -> TMEM
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
             double2 st[4];
 #pragma unroll
             for (int i = 0; i < 4; ++i) {
-                const int q = R.t3 + C12_NT * ((4 * k + i + 8) & 15);
+                const int q = R.t2 + C12_NT * ((4 * k + i + 8) & 15);
                 const double m = (double)(q - C12_N / 2) * dl;
                 const double r2 = l * l + m * m;
                 double xs = 0.0;
@@ -165,8 +226,8 @@ k_cols12_wcorrect(const __grid_constant__ CUtensorMap tmap, const double2* __res
         for (int plane = n_planes - 1; plane >= 0; --plane) {
             const bool more = plane > 0 || strip + (int)gridDim.x < strip_end;
             double2 v[16];
-            strip_fft(v, R, stg, ex, tw, bar, parity, more, &tmap, plane > 0 ? strip : strip + (int)gridDim.x,
-                      plane > 0 ? plane - 1 : n_planes - 1);
+            strip_fft_g(v, R, stg, ex, tw, full, empty, parity, more, &tmap, plane > 0 ? strip : strip + (int)gridDim.x,
+                        plane > 0 ? plane - 1 : n_planes - 1);
             // Horner in z: S <- P_z + step S
             if (plane == n_planes - 1) {
 #pragma unroll
@@ -210,7 +271,7 @@ k_cols12_wcorrect(const __grid_constant__ CUtensorMap tmap, const double2* __res
             unpack4(rs, s4);
 #pragma unroll
             for (int i = 0; i < 4; ++i) {
-                const int q = R.t3 + C12_NT * ((4 * k + i + 8) & 15);
+                const int q = R.t2 + C12_NT * ((4 * k + i + 8) & 15);
                 const double m = (double)(q - C12_N / 2) * dl;
                 const double r2 = l * l + m * m;
                 double val = 0.0;
@@ -230,7 +291,7 @@ k_cols12_wcorrect(const __grid_constant__ CUtensorMap tmap, const double2* __res
     }
     tmem_fence_before_sync();
     __syncthreads();
-    if (R.w == 0) tmem_dealloc_all(tbase);
+    if (warp == 0) tmem_dealloc_all(tbase);
 }
 
 }   // namespace
@@ -261,6 +322,14 @@ int rick_cols12_init(rick_plan_t* p)
     }
     RICK_CUDA(p, cudaFuncSetAttribute(k_cols12_fft, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C12_SMEM));
     RICK_CUDA(p, cudaFuncSetAttribute(k_cols12_wcorrect, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C12_SMEM));
+    static_assert(sizeof(CUtensorMap) <= sizeof(p->cols12_tmap_sw), "tensor map storage");
+    const CUresult r2 = enc(reinterpret_cast<CUtensorMap*>(p->cols12_tmap_sw), CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 5, p->stack,
+                            dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_32B,
+                            CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r2 != CUDA_SUCCESS) {
+        p->err = "cuTensorMapEncodeTiled (swizzled) failed";
+        return RICK_ERR_CUDA;
+    }
     p->cols12_ok = 1;
     return RICK_OK;
 }
@@ -281,7 +350,7 @@ int rick_cols12_wcorrect(rick_plan_t* p, int img, int z_first, int n_planes, dou
                          int fuse_taper, int strip_begin, int strip_end)
 {
     if (strip_end <= strip_begin) return RICK_OK;
-    const CUtensorMap tm = *reinterpret_cast<const CUtensorMap*>(p->cols12_tmap);
+    const CUtensorMap tm = *reinterpret_cast<const CUtensorMap*>(p->cols12_tmap_sw);
     const int n = strip_end - strip_begin;
     RICK_KERNEL(p, RK_COLS_WCORRECT, k_cols12_wcorrect<<<n < p->n_sm ? n : p->n_sm, C12_THREADS, C12_SMEM, p->stream>>>(
         tm, (const double2*)p->twiddle, n_planes, z_first, p->dl, p->wrange + img, image, accumulate,

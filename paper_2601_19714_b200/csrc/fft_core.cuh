@@ -305,3 +305,54 @@ __device__ __forceinline__ void xchg16_cta(double2 (&v)[16], double* __restrict_
         v[e].x = re[e];
     }
 }
+
+// ------------------------------------------------------------------------------------------
+// The same two exchanges for a CTA split into two COLUMN GROUPS of 256 threads (k_cols12_wcorrect):
+// a group owns one column of the strip, role (w, hh) = (tg >> 4, tg & 15), so a warp holds two
+// values of w (wl = lane >> 4) and all 16 hh.  Only group-wide named barriers (`bar_id`, 256
+// threads): the two groups run out of phase, one in its butterflies while the other exchanges.
+// ------------------------------------------------------------------------------------------
+
+// after stage 1: 16 x 16 transpose among the hh of one w, inside the warp.  wb: this warp's 2*16*17 doubles.
+__device__ __forceinline__ void xchg16_warp_grp(double2 (&v)[16], double* __restrict__ wb, const int wl, const int hh)
+{
+    double* b = wb + wl * (16 * 17);
+#pragma unroll
+    for (int r = 0; r < 16; ++r) b[hh * 17 + r] = v[r].x;
+    __syncwarp();
+    double re[16];
+#pragma unroll
+    for (int e = 0; e < 16; ++e) re[e] = b[e * 17 + hh];
+    __syncwarp();
+#pragma unroll
+    for (int r = 0; r < 16; ++r) b[hh * 17 + r] = v[r].y;
+    __syncwarp();
+#pragma unroll
+    for (int e = 0; e < 16; ++e) {
+        v[e].y = b[e * 17 + hh];
+        v[e].x = re[e];
+    }
+    __syncwarp();
+}
+
+// after stage 2, group-wide: writer role t2 leg r -> position pos0 + 16 r; reader element e <- position
+// t2 + 256 e.  gb: the group's 4096 + 256 doubles.
+__device__ __forceinline__ void xchg16_grp(double2 (&v)[16], double* __restrict__ gb, const int t2, const int bar_id)
+{
+    const int pos0 = ((t2 >> 4) << 8) + (t2 & 15);
+#pragma unroll
+    for (int r = 0; r < 16; ++r) gb[fft_pad(pos0 + r * 16)] = v[r].x;
+    asm volatile("bar.sync %0, 256;\n" ::"r"(bar_id) : "memory");
+    double re[16];
+#pragma unroll
+    for (int e = 0; e < 16; ++e) re[e] = gb[fft_pad(t2 + 256 * e)];
+    asm volatile("bar.sync %0, 256;\n" ::"r"(bar_id) : "memory");
+#pragma unroll
+    for (int r = 0; r < 16; ++r) gb[fft_pad(pos0 + r * 16)] = v[r].y;
+    asm volatile("bar.sync %0, 256;\n" ::"r"(bar_id) : "memory");
+#pragma unroll
+    for (int e = 0; e < 16; ++e) {
+        v[e].y = gb[fft_pad(t2 + 256 * e)];
+        v[e].x = re[e];
+    }
+}
