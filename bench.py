@@ -211,6 +211,18 @@ def main():
     e2e_ms = (time.perf_counter() - t0) * 1e3
     e2e = bu.aggregate_replicas(wl.n_vis * k_e2e, e2e_ms, device="cuda")
     h2d = hv.numel() * hv.element_size() + hu.numel() * 8 + (0 if hw is None else hw.numel() * 4)
+    # out-of-core visibilities (rick_image_stream_host): the same host buffers in 8 chunks of rows, the copy
+    # of chunk c+1 under index + sort + gridding of chunk c (whole stack resident, cube = 0 only)
+    if not wl.cube and not wl.plane_batch:
+        rpc = (wl.n_rows + 7) // 8
+        plan.rick_image_stream_host(hv, hu, hw, wl.freq_hz, hout[0], rpc)      # warm (grows the staging)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(k_e2e):
+            plan.rick_image_stream_host(hv, hu, hw, wl.freq_hz, hout[0], rpc)
+        torch.cuda.synchronize()
+        st_ms = (time.perf_counter() - t0) * 1e3 / k_e2e
+        stages["stream_host"] = {"ms_per_step": st_ms, "mvis_s": wl.n_vis / st_ms / 1e3, "rows_per_chunk": rpc, "chunks": 8}
     clocks = sampler.stop()
 
     cpu_baseline = None

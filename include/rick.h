@@ -127,6 +127,20 @@ int rick_image_host(rick_plan_t* p, const void* vis_host, int32_t vis_dtype, con
                     const float* weights_host, const double* chan_freq_hz, int32_t n_chan,
                     int64_t n_rows, double* image_out_host);
 
+/* Out-of-core visibilities: rick_image_host for a visibility set that need not fit device memory.
+ * The host arrays are as in rick_image_host; the visibilities (and weights) cross to the device in
+ * chunks of rows_per_chunk rows (>= 1; the last chunk may be shorter) through a two-slot plan-owned
+ * staging buffer, the copy of chunk c+1 overlapping index + sort + gridding of chunk c into the same
+ * resident stack (gridding is linear in the visibilities, Eq. 3; the single-node analogue of
+ * the I/O-compute overlap of PAPER.md:312).  uvw_m_host is copied whole first (24 B per row) and a0 runs
+ * over ALL rows, so planes, cells and statistics equal those of one rick_image call; only the summation
+ * order differs.  Per-chunk limits as rick_grid with R = rows_per_chunk.  Requires plane_batch == N_w
+ * and cube == 0 (RICK_ERR_STATE otherwise).  SYNCHRONISES the stream before returning.  The debug item
+ * accessor afterwards describes the last chunk only. */
+int rick_image_stream_host(rick_plan_t* p, const void* vis_host, int32_t vis_dtype, const double* uvw_m_host,
+                           const float* weights_host, const double* chan_freq_hz, int32_t n_chan,
+                           int64_t n_rows, int64_t rows_per_chunk, double* image_out_host);
+
 /* Copy of the plan's image ([N][N] double) into dst_device (cube = 0 only). */
 int rick_get_image(rick_plan_t* p, double* dst_device);
 

@@ -93,6 +93,9 @@ struct rick_plan_s {
     double prof_ms[32];                     // aggregated by rick_profile_read
     long long prof_cnt[32];
 
+    // chunked gridding (rick_image_stream_host): visibility chunk c uses staging half c & 1
+    cudaEvent_t ev_chunk_in[2], ev_chunk_free[2];
+
     // N = 4096 fp64 column kernels (fft_cols12.cu): TMA tensor map over the resident stack
     int cols12_ok;
     alignas(64) unsigned char cols12_tmap[128];
@@ -144,7 +147,13 @@ void rick_prof_end(rick_plan_t* p, cudaStream_t st);
 
 // stage entry points (each enqueues on p->stream)
 int rick_tables_build(rick_plan_t* p);                                   // tables.cu
-int rick_index_sort(rick_plan_t* p, const double* uvw_m, const float* weights);   // index_sort.cu
+// flags of rick_index_sort (chunked gridding, rick_image_stream_host): keep the w range and the statistics
+// counters of the plan (set up once over ALL rows by rick_wrange_all), OR the occupancy maps into the
+// existing ones instead of rebuilding them
+#define RICK_SORT_KEEP_RANGE 1
+#define RICK_SORT_OCC_ACCUM 2
+int rick_index_sort(rick_plan_t* p, const double* uvw_m, const float* weights, int flags = 0);   // index_sort.cu
+int rick_wrange_all(rick_plan_t* p, const double* uvw_m, int64_t n_rows);                         // index_sort.cu
 int rick_zero_dirty(rick_plan_t* p, int n_slots, cudaStream_t st);        // grid.cu: zero the dirty rows of slots 0..n_slots-1
 int rick_zero_sparse(rick_plan_t* p, int plane_first, int n_slots);     // grid.cu: stale rows whole, occupied rows by tile
 int rick_mark_dirty(rick_plan_t* p, int plane_first, int n_planes);      // grid.cu: dirty |= occupancy of the batch

@@ -408,21 +408,32 @@ k_tile_occupancy(const u64* __restrict__ sitems, const long long* __restrict__ p
 }
 
 // ------------------------------------------------------------------------------------------
-int rick_index_sort(rick_plan_t* p, const double* uvw_m, const float* weights)
+// a0 alone over n_rows rows: resets the statistics counters and leaves the w range in p->wrange
+int rick_wrange_all(rick_plan_t* p, const double* uvw_m, int64_t n_rows)
+{
+    cudaStream_t st = p->stream;
+    RICK_KERNEL(p, RK_RESET, k_counters_reset<<<1, 1, 0, st>>>(p->counters));
+    if (n_rows > 0) {
+        int nb = (int)((n_rows + 255) / 256);
+        if (nb > p->n_sm * 8) nb = p->n_sm * 8;
+        RICK_KERNEL(p, RK_WRANGE, k_wrange_rows<<<nb, 256, 0, st>>>(uvw_m, (long long)n_rows, p->counters));
+    }
+    RICK_KERNEL(p, RK_WRANGE, k_wrange_finish<<<(p->n_img + 127) / 128, 128, 0, st>>>(p->counters, p->chan_scale, p->C, p->d.cube,
+                                                          p->Nw, p->d.w_min, p->d.w_max,
+                                                          (long long)n_rows, p->wrange));
+    return RICK_OK;
+}
+
+int rick_index_sort(rick_plan_t* p, const double* uvw_m, const float* weights, int flags)
 {
     cudaStream_t st = p->stream;
     const unsigned int M = (unsigned int)p->M;
     const int n_planes_total = p->n_img * p->Nw;
 
-    RICK_KERNEL(p, RK_RESET, k_counters_reset<<<1, 1, 0, st>>>(p->counters));
-    if (p->R > 0) {
-        int nb = (int)((p->R + 255) / 256);
-        if (nb > p->n_sm * 8) nb = p->n_sm * 8;
-        RICK_KERNEL(p, RK_WRANGE, k_wrange_rows<<<nb, 256, 0, st>>>(uvw_m, (long long)p->R, p->counters));
+    if (!(flags & RICK_SORT_KEEP_RANGE)) {
+        const int rc = rick_wrange_all(p, uvw_m, p->R);
+        if (rc) return rc;
     }
-    RICK_KERNEL(p, RK_WRANGE, k_wrange_finish<<<(p->n_img + 127) / 128, 128, 0, st>>>(p->counters, p->chan_scale, p->C, p->d.cube,
-                                                          p->Nw, p->d.w_min, p->d.w_max,
-                                                          (long long)p->R, p->wrange));
 
     p->sorted_items = p->items;
     if (M > 0) {
@@ -479,13 +490,13 @@ int rick_index_sort(rick_plan_t* p, const double* uvw_m, const float* weights)
     RICK_KERNEL(p, RK_PLANE_STARTS, k_plane_starts<<<(n_planes_total + 1 + 127) / 128, 128, 0, st>>>(
         (const u64*)p->sorted_items, M, p->idx_bits, (unsigned long long)p->N * p->N, n_planes_total,
         (long long*)p->plane_start));
-    RICK_CUDA(p, cudaMemsetAsync(p->row_occ, 0, (size_t)n_planes_total * p->N, st));
+    if (!(flags & RICK_SORT_OCC_ACCUM)) RICK_CUDA(p, cudaMemsetAsync(p->row_occ, 0, (size_t)n_planes_total * p->N, st));
     if (M > 0) {
         const int n = n_planes_total * p->T;
         RICK_KERNEL(p, RK_ROW_OCC, k_row_occupancy<<<(n + 127) / 128, 128, 0, st>>>(
             (const u64*)p->sorted_items, M, p->idx_bits, p->N, p->B, p->T, p->h, n_planes_total, p->row_occ));
     }
-    RICK_CUDA(p, cudaMemsetAsync(p->tile_occ, 0, (size_t)n_planes_total * p->T * p->T, st));
+    if (!(flags & RICK_SORT_OCC_ACCUM)) RICK_CUDA(p, cudaMemsetAsync(p->tile_occ, 0, (size_t)n_planes_total * p->T * p->T, st));
     if (M > 0) {
         unsigned int nb = (M + 255) / 256;
         if (nb > (unsigned)p->n_sm * 8u) nb = (unsigned)p->n_sm * 8u;

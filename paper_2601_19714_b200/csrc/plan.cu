@@ -102,6 +102,10 @@ extern "C" int rick_plan_destroy(rick_plan_t* p)
     if (p->stream3) { cudaStreamSynchronize(p->stream3); cudaStreamDestroy(p->stream3); }
     if (p->ev_vis) cudaEventDestroy(p->ev_vis);
     if (p->ev_part) cudaEventDestroy(p->ev_part);
+    for (int i = 0; i < 2; ++i) {
+        if (p->ev_chunk_in[i]) cudaEventDestroy(p->ev_chunk_in[i]);
+        if (p->ev_chunk_free[i]) cudaEventDestroy(p->ev_chunk_free[i]);
+    }
     delete p;
     return RICK_OK;
 }
@@ -131,6 +135,10 @@ static int plan_init(rick_plan_t* p)
         RICK_CUDA(p, cudaStreamCreateWithFlags(&p->stream3, cudaStreamNonBlocking));
         RICK_CUDA(p, cudaEventCreateWithFlags(&p->ev_vis, cudaEventDisableTiming));
         RICK_CUDA(p, cudaEventCreateWithFlags(&p->ev_part, cudaEventDisableTiming));
+        for (int i = 0; i < 2; ++i) {
+            RICK_CUDA(p, cudaEventCreateWithFlags(&p->ev_chunk_in[i], cudaEventDisableTiming));
+            RICK_CUDA(p, cudaEventCreateWithFlags(&p->ev_chunk_free[i], cudaEventDisableTiming));
+        }
     }
     RICK_CUDA(p, cudaMalloc(&p->counters, sizeof(DevCounters)));
     RICK_CUDA(p, cudaMemsetAsync(p->counters, 0, sizeof(DevCounters), p->stream));
@@ -352,6 +360,43 @@ extern "C" int rick_gridcorrect(rick_plan_t* p)
     return RICK_OK;
 }
 
+// a4..a6 of one resident batch (planes z0 .. z0 + nb - 1 of image img): row pass, then either the fused
+// column pass + w-correction (N = 4096 fp64) or the generic column pass and correction.  host_out (cube = 0,
+// last batch only): the image leaves for HOST memory part by part on the copy stream while the next part
+// of the last pass is still running; *host_done says whether that happened.
+static int transform_and_correct(rick_plan_t* p, int img, int z0, int nb, double* dst, int last, double* host_out,
+                                 bool* host_done)
+{
+    int rc;
+    if (p->cols12_ok) {   // column pass fused with the w-correction: the transformed planes are never written
+        if ((rc = rick_fft_rows(p, img * p->Nw + z0, nb))) return rc;
+        const int strips = rick_cols12_strips();
+        if (host_out && last && !p->d.cube) {
+            // whole rounds of the persistent grid per part: 4 + 4 + 3 + rest rounds of n_sm strips
+            const int rounds[4] = {4, 4, 3, 1 << 20};
+            int s0 = 0;
+            for (int k = 0; k < 4 && s0 < strips; ++k) {
+                long long s1 = (long long)s0 + (long long)rounds[k] * p->n_sm;
+                if (s1 > strips) s1 = strips;
+                if ((rc = rick_cols12_wcorrect(p, img, z0, nb, dst, z0 > 0, last, s0, (int)s1))) return rc;
+                RICK_CUDA(p, cudaEventRecord(p->ev_part, p->stream));
+                RICK_CUDA(p, cudaStreamWaitEvent(p->stream3, p->ev_part, 0));
+                const size_t c0 = 2 * (size_t)s0, nc = 2 * (size_t)(s1 - s0);
+                RICK_CUDA(p, cudaMemcpy2DAsync(host_out + c0, sizeof(double) * p->N, dst + c0, sizeof(double) * p->N,
+                                               sizeof(double) * nc, (size_t)p->N, cudaMemcpyDeviceToHost, p->stream3));
+                s0 = (int)s1;
+            }
+            *host_done = true;
+        } else {
+            if ((rc = rick_cols12_wcorrect(p, img, z0, nb, dst, z0 > 0, last, 0, strips))) return rc;
+        }
+    } else {
+        if ((rc = rick_fft_planes(p, img * p->Nw + z0, nb))) return rc;
+        if ((rc = rick_wcorrect(p, img, z0, nb, dst, z0 > 0, last))) return rc;
+    }
+    return RICK_OK;
+}
+
 // a0..a6.  vis_ready (may be null): event the gridder must wait for (visibilities still being copied
 // by rick_image_host).  host_out (may be null; cube = 0 only): the image goes to HOST memory, part by
 // part on the copy stream while the next part of the last pass is still running.
@@ -377,32 +422,7 @@ static int image_impl(rick_plan_t* p, const void* vis, int32_t vis_dtype, const 
             if ((rc = rick_zero_sparse(p, img * p->Nw + z0, nb))) return rc;
             if ((rc = rick_mark_dirty(p, img * p->Nw + z0, nb))) return rc;
             if ((rc = rick_grid_planes(p, vis, vis_dtype, uvw_m, weights, img * p->Nw + z0, nb))) return rc;
-            if (p->cols12_ok) {   // column pass fused with the w-correction: the transformed planes are never written
-                if ((rc = rick_fft_rows(p, img * p->Nw + z0, nb))) return rc;
-                const int strips = rick_cols12_strips();
-                if (host_out && last && !p->d.cube) {
-                    // whole rounds of the persistent grid per part: 4 + 4 + 3 + rest rounds of n_sm strips
-                    const int rounds[4] = {4, 4, 3, 1 << 20};
-                    int s0 = 0;
-                    for (int k = 0; k < 4 && s0 < strips; ++k) {
-                        long long s1 = (long long)s0 + (long long)rounds[k] * p->n_sm;
-                        if (s1 > strips) s1 = strips;
-                        if ((rc = rick_cols12_wcorrect(p, img, z0, nb, dst, z0 > 0, last, s0, (int)s1))) return rc;
-                        RICK_CUDA(p, cudaEventRecord(p->ev_part, p->stream));
-                        RICK_CUDA(p, cudaStreamWaitEvent(p->stream3, p->ev_part, 0));
-                        const size_t c0 = 2 * (size_t)s0, nc = 2 * (size_t)(s1 - s0);
-                        RICK_CUDA(p, cudaMemcpy2DAsync(host_out + c0, sizeof(double) * p->N, dst + c0, sizeof(double) * p->N,
-                                                       sizeof(double) * nc, (size_t)p->N, cudaMemcpyDeviceToHost, p->stream3));
-                        s0 = (int)s1;
-                    }
-                    host_done = true;
-                } else {
-                    if ((rc = rick_cols12_wcorrect(p, img, z0, nb, dst, z0 > 0, last, 0, strips))) return rc;
-                }
-            } else {
-                if ((rc = rick_fft_planes(p, img * p->Nw + z0, nb))) return rc;
-                if ((rc = rick_wcorrect(p, img, z0, nb, dst, z0 > 0, last))) return rc;
-            }
+            if ((rc = transform_and_correct(p, img, z0, nb, dst, last, host_out, &host_done))) return rc;
         }
     }
     if (!p->d.cube) {
@@ -470,6 +490,81 @@ extern "C" int rick_image_host(rick_plan_t* p, const void* vis_host, int32_t vis
     rc = image_impl(p, p->st_vis, vis_dtype, p->st_uvw, weights_host ? p->st_wgt : nullptr, chan_freq_hz,
                     n_chan, n_rows, p->d.cube ? p->st_img : nullptr, M ? p->ev_vis : nullptr, image_out_host);
     if (rc) return rc;
+    RICK_CUDA(p, cudaStreamSynchronize(p->stream));
+    RICK_CUDA(p, cudaStreamSynchronize(p->stream3));
+    return RICK_OK;
+}
+
+
+// Out-of-core visibilities (the single-node analogue of the I/O-compute overlap the
+// paper plans).  The visibilities stay in HOST memory and cross to the device in chunks of
+// rows_per_chunk rows through a two-slot staging buffer: chunk c + 1 is copied on the copy stream while
+// chunk c is indexed, sorted and gridded INTO the same resident stack (gridding is linear in the
+// visibilities, Eq. 3).  a0 runs once over all rows first (uvw is 24 B per row and is copied whole), so
+// every chunk sees the same w range and lands on the same planes as in one rick_image call; the occupancy
+// maps are the union over the chunks.  a4..a6 run once at the end.
+extern "C" int rick_image_stream_host(rick_plan_t* p, const void* vis_host, int32_t vis_dtype, const double* uvw_m_host,
+                                      const float* weights_host, const double* chan_freq_hz, int32_t n_chan,
+                                      int64_t n_rows, int64_t rows_per_chunk, double* image_out_host)
+{
+    if (!p) return RICK_ERR_INVALID;
+    p->err.clear();
+    if (!image_out_host) { p->err = "null image_out_host"; return RICK_ERR_INVALID; }
+    if (p->batch != p->Nw || p->d.cube) { p->err = "chunked gridding needs the whole stack resident and cube = 0"; return RICK_ERR_STATE; }
+    if (rows_per_chunk < 1) { p->err = "rows_per_chunk < 1"; return RICK_ERR_INVALID; }
+    if (n_rows < 0) { p->err = "negative n_rows"; return RICK_ERR_INVALID; }
+    if (rows_per_chunk > n_rows) rows_per_chunk = n_rows > 0 ? n_rows : 1;
+    // the 32-bit index / 64-bit item limits apply to ONE chunk, not to the whole set
+    int rc = check_inputs(p, vis_host, vis_dtype, uvw_m_host, chan_freq_hz, n_chan, n_rows > 0 ? rows_per_chunk : 0);
+    if (rc) return rc;
+    const size_t C = (size_t)n_chan, vsz = vis_dtype == RICK_VIS_C128 ? 16 : 8;
+    const size_t chunk_vis = (size_t)rows_per_chunk * C * vsz, chunk_wgt = (size_t)rows_per_chunk * C * sizeof(float);
+    const size_t NN = (size_t)p->N * p->N;
+    if ((rc = ensure_bytes(p, &p->st_vis, &p->st_vis_cap, 2 * chunk_vis))) return rc;
+    if ((rc = ensure_bytes(p, &p->st_uvw, &p->st_uvw_cap, sizeof(double) * 3 * (size_t)n_rows))) return rc;
+    if (weights_host && (rc = ensure_bytes(p, &p->st_wgt, &p->st_wgt_cap, 2 * chunk_wgt))) return rc;
+    p->state = 0;
+    if ((rc = prepare(p, chan_freq_hz, n_chan, rows_per_chunk))) return rc;      // sort scratch for ONE chunk
+    const int n_planes_total = p->Nw;
+    if (n_rows > 0)
+        RICK_CUDA(p, cudaMemcpyAsync(p->st_uvw, uvw_m_host, sizeof(double) * 3 * (size_t)n_rows, cudaMemcpyHostToDevice, p->stream));
+    // the copy stream may touch the staging only after everything enqueued so far (earlier calls) is done
+    RICK_CUDA(p, cudaEventRecord(p->ev_fork, p->stream));
+    RICK_CUDA(p, cudaStreamWaitEvent(p->stream3, p->ev_fork, 0));
+    if ((rc = rick_wrange_all(p, p->st_uvw, n_rows))) return rc;                 // a0 over ALL rows
+    if ((rc = rick_zero_dirty(p, p->batch, p->stream))) return rc;               // the whole stack is zero again
+    RICK_CUDA(p, cudaMemsetAsync(p->row_occ, 0, (size_t)n_planes_total * p->N, p->stream));
+    RICK_CUDA(p, cudaMemsetAsync(p->tile_occ, 0, (size_t)n_planes_total * p->T * p->T, p->stream));
+    int c = 0;
+    for (int64_t r0 = 0; r0 < n_rows; r0 += rows_per_chunk, ++c) {
+        const int64_t nr = n_rows - r0 < rows_per_chunk ? n_rows - r0 : rows_per_chunk;
+        const int b = c & 1;
+        const size_t off = (size_t)r0 * C;
+        unsigned char* dv = reinterpret_cast<unsigned char*>(p->st_vis) + (size_t)b * chunk_vis;
+        float* dw = weights_host ? reinterpret_cast<float*>(reinterpret_cast<unsigned char*>(p->st_wgt) + (size_t)b * chunk_wgt) : nullptr;
+        if (c >= 2) RICK_CUDA(p, cudaStreamWaitEvent(p->stream3, p->ev_chunk_free[b], 0));
+        RICK_CUDA(p, cudaMemcpyAsync(dv, reinterpret_cast<const unsigned char*>(vis_host) + off * vsz, (size_t)nr * C * vsz,
+                                     cudaMemcpyHostToDevice, p->stream3));
+        if (dw)
+            RICK_CUDA(p, cudaMemcpyAsync(dw, weights_host + off, (size_t)nr * C * sizeof(float), cudaMemcpyHostToDevice, p->stream3));
+        RICK_CUDA(p, cudaEventRecord(p->ev_chunk_in[b], p->stream3));
+        p->R = nr;
+        p->M = nr * (int64_t)n_chan;
+        const double* du = p->st_uvw + 3 * (size_t)r0;
+        if (dw) RICK_CUDA(p, cudaStreamWaitEvent(p->stream, p->ev_chunk_in[b], 0));   // the index step sums the weights
+        if ((rc = rick_index_sort(p, du, dw, RICK_SORT_KEEP_RANGE | RICK_SORT_OCC_ACCUM))) return rc;
+        if (!dw) RICK_CUDA(p, cudaStreamWaitEvent(p->stream, p->ev_chunk_in[b], 0));
+        if ((rc = rick_mark_dirty(p, 0, p->Nw))) return rc;
+        if ((rc = rick_grid_planes(p, dv, vis_dtype, du, dw, 0, p->Nw))) return rc;
+        RICK_CUDA(p, cudaEventRecord(p->ev_chunk_free[b], p->stream));
+    }
+    p->R = n_rows;
+    p->M = n_rows * (int64_t)n_chan;
+    bool host_done = false;
+    if ((rc = transform_and_correct(p, 0, 0, p->Nw, p->image, 1, image_out_host, &host_done))) return rc;
+    p->state = 4;
+    if (!host_done)
+        RICK_CUDA(p, cudaMemcpyAsync(image_out_host, p->image, sizeof(double) * NN, cudaMemcpyDeviceToHost, p->stream));
     RICK_CUDA(p, cudaStreamSynchronize(p->stream));
     RICK_CUDA(p, cudaStreamSynchronize(p->stream3));
     return RICK_OK;

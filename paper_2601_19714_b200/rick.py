@@ -23,6 +23,7 @@ RICK_VIS_C64, RICK_VIS_C128 = 0, 1
 
 EXPORTS = ["rick_plan", "rick_plan_destroy", "rick_grid", "rick_fft_wplanes",
            "rick_wcorrect_accumulate", "rick_gridcorrect", "rick_image", "rick_image_host",
+           "rick_image_stream_host",
            "rick_get_image", "rick_get_stats", "rick_last_error", "rick_debug_items",
            "rick_debug_planes", "rick_version", "rick_profile",
            "rick_profile_read", "rick_kernel_name"]
@@ -68,6 +69,7 @@ def load_library():
     L.rick_gridcorrect.argtypes = [vp]
     L.rick_image.argtypes = [vp, vp, i32, vp, vp, C.POINTER(C.c_double), i32, i64, vp]
     L.rick_image_host.argtypes = [vp, vp, i32, vp, vp, C.POINTER(C.c_double), i32, i64, vp]
+    L.rick_image_stream_host.argtypes = [vp, vp, i32, vp, vp, C.POINTER(C.c_double), i32, i64, i64, vp]
     L.rick_get_image.argtypes = [vp, vp]
     L.rick_get_stats.argtypes = [vp, C.POINTER(Stats)]
     L.rick_last_error.argtypes = [vp]
@@ -175,6 +177,20 @@ class Plan:
             self._h, C.c_void_p(vis.data_ptr()), self._vis_dtype(vis), C.c_void_p(uvw_m.data_ptr()),
             None if weights is None else C.c_void_p(weights.data_ptr()),
             freq.ctypes.data_as(C.POINTER(C.c_double)), n_chan, n_rows, C.c_void_p(image_out.data_ptr())))
+        return image_out
+
+    def rick_image_stream_host(self, vis, uvw_m, weights, chan_freq_hz, image_out, rows_per_chunk: int):
+        """Out-of-core visibilities: all buffers HOST; the visibilities cross in chunks of rows; synchronises."""
+        freq = np.ascontiguousarray(chan_freq_hz, dtype=np.float64)
+        n_chan, n_rows = int(freq.shape[0]), int(uvw_m.shape[0])
+        for t in (vis, uvw_m, image_out) + (() if weights is None else (weights,)):
+            assert (not t.is_cuda) and t.is_contiguous()
+        self._n_vis = n_rows * n_chan
+        self._check(self._lib.rick_image_stream_host(
+            self._h, C.c_void_p(vis.data_ptr()), self._vis_dtype(vis), C.c_void_p(uvw_m.data_ptr()),
+            None if weights is None else C.c_void_p(weights.data_ptr()),
+            freq.ctypes.data_as(C.POINTER(C.c_double)), n_chan, n_rows, int(rows_per_chunk),
+            C.c_void_p(image_out.data_ptr())))
         return image_out
 
     def rick_get_image(self) -> torch.Tensor:

@@ -35,7 +35,7 @@ def test_library_exports_every_declared_symbol():
 def test_binding_has_same_names():
     from paper_2601_19714_b200 import rick
     for n in ["rick_grid", "rick_fft_wplanes", "rick_wcorrect_accumulate", "rick_gridcorrect",
-              "rick_image", "rick_image_host", "rick_get_image", "rick_get_stats"]:
+              "rick_image", "rick_image_host", "rick_image_stream_host", "rick_get_image", "rick_get_stats"]:
         assert hasattr(rick.Plan, n)
 
 
