@@ -226,21 +226,34 @@ __global__ void __launch_bounds__(GRID_WARPS * 32, 2) k_grid(const __grid_consta
             for (int nt = 0; nt < NT; ++nt)
                 if (has[mt][nt]) tile_store<GT>(a_tile[mt][nt] + cur_off, c[mt][nt]);
     };
-    // tile -> HBM, once per (tile, chunk)
+    // tile -> HBM, once per (tile, chunk): the TH x TH cells scanned linearly, four cells per lane in flight
+    const float inv_TH = 1.0f / (float)TH;
+    const int n_cells = TH * TH;
     auto flush_tile = [&](u64 tkey) {
         __syncwarp();
         const unsigned int pz = (unsigned int)(tkey / TT), rem = (unsigned int)(tkey - (u64)pz * TT);
         const int tv = (int)(rem / (unsigned)T), tu = (int)(rem - (unsigned)tv * (unsigned)T);
         cell* plane = reinterpret_cast<cell*>(P.stack) + (size_t)(pz - (unsigned)P.plane_first) * N * N;
         const long long g0 = (long long)(tv * B - h) * N + (tu * B - h);     // may be < 0 on the grid edge
-        for (int row = 0; row < TH; ++row) {
-            for (int col = lane; col < TH; col += 32) {
-                cell v = tile[row * TWp + col];
-                if (v.x != 0 || v.y != 0) {
-                    red_add(plane + (g0 + (long long)row * N + col), v);
-                    tile[row * TWp + col] = zero;
-                }
+        for (int i0 = lane; i0 < n_cells; i0 += 128) {
+            cell v[4];
+            int t[4];
+            long long gofs[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const int i = i0 + 32 * u;
+                const int row = __float2int_rd(((float)i + 0.5f) * inv_TH), col = i - row * TH;   // exact: i < 2^11
+                t[u] = row * TWp + col;
+                gofs[u] = g0 + (long long)row * N + col;
+                v[u] = zero;
+                if (i < n_cells) v[u] = tile[t[u]];
             }
+#pragma unroll
+            for (int u = 0; u < 4; ++u)
+                if (v[u].x != 0 || v[u].y != 0) {
+                    red_add(plane + gofs[u], v[u]);
+                    tile[t[u]] = zero;
+                }
         }
         __syncwarp();
     };
@@ -248,9 +261,13 @@ __global__ void __launch_bounds__(GRID_WARPS * 32, 2) k_grid(const __grid_consta
     // inputs of one visibility, loaded one batch ahead of their use
     struct VisIn {
         u64 key;
-        double um, vm, s, vr, vi;
+        double um, vm, s, vr, vi;      // vr, vi: raw value as loaded (complex128), else see raw
+        float2 raw;                    // complex64 as loaded
+        float om;                      // weight as loaded
     };
     auto load_item = [&](long long ks, long long c_end) -> u64 { return ks < c_end ? P.sitems[ks] : NOKEY; };
+    // loads only: nothing here depends on a loaded value, so the whole batch of loads stays in flight
+    // while the previous batch is accumulated (conversions and the weight product happen in finish_vis)
     auto load_vis = [&](u64 item, VisIn& in) {
         in.key = NOKEY;
         if (item == NOKEY) return;
@@ -265,12 +282,18 @@ __global__ void __launch_bounds__(GRID_WARPS * 32, 2) k_grid(const __grid_consta
             in.vr = v.x;
             in.vi = v.y;
         } else {
-            const float2 v = reinterpret_cast<const float2*>(P.vis)[idx];
-            in.vr = (double)v.x;
-            in.vi = (double)v.y;
+            in.raw = reinterpret_cast<const float2*>(P.vis)[idx];
+        }
+        in.om = 1.0f;
+        if (P.wgt) in.om = P.wgt[idx];
+    };
+    auto finish_vis = [&](VisIn& in) {
+        if (!P.vis_c128) {
+            in.vr = (double)in.raw.x;
+            in.vi = (double)in.raw.y;
         }
         if (P.wgt) {
-            const double om = (double)P.wgt[idx];
+            const double om = (double)in.om;
             in.vr *= om;
             in.vi *= om;
         }
@@ -317,6 +340,7 @@ __global__ void __launch_bounds__(GRID_WARPS * 32, 2) k_grid(const __grid_consta
                 s_run[r] = d;
             }
             if (valid) {
+                finish_vis(cur);
                 const double xu = __dmul_rn(__dmul_rn(cur.um, cur.s), P.inv_du);
                 const double xv = __dmul_rn(__dmul_rn(cur.vm, cur.s), P.inv_du);
                 const int iu = (int)floor(__dadd_rn(xu, shift));
