@@ -47,22 +47,32 @@ k_fft_rows(typename cplx_of<T>::type* __restrict__ stack,
     // Persistent CTAs walk the list of occupied row groups.
     const int rl = threadIdx.x / K::NT, t = threadIdx.x - rl * K::NT;
     C* sm = reinterpret_cast<C*>(smem_raw) + (size_t)rl * (K::N + K::N / 16);
-    __shared__ unsigned char s_to[K::RPC][K::N / 8];
+    __shared__ unsigned char s_to[2][K::RPC][K::N / 8];
     const int Tn = K::N >> log2B;
     const unsigned int n_work = *count;
-    for (unsigned int w = blockIdx.x; w < n_work; w += gridDim.x) {
-        const size_t grp = list[w];
+    // only the tiles some footprint reaches hold gridded data (tile_occ); whatever else the row holds
+    // (rick_image leaves the previous transform there) is not read and counts as zero.  The flags of the
+    // NEXT group are fetched (list entry, then flag bytes) while this group is transformed: at most two
+    // bytes per thread (RPC * Tn = THREADS * 16 / B, B >= 8), parked in registers across the transform.
+    auto flag_addr = [&](size_t grp, int i) -> const unsigned char* {
+        const int a = i / Tn, ti = i - a * Tn;
+        const size_t R = grp * K::RPC + a;          // slot-major row
+        const size_t slot = R / K::N;
+        const int row = (int)(R - slot * K::N);
+        return tocc + (slot * Tn + (size_t)(row >> log2B)) * Tn + ti;
+    };
+    const int n_flags = K::RPC * Tn;
+    unsigned int w = blockIdx.x;
+    size_t grp = w < n_work ? list[w] : 0;
+    if (w < n_work)
+        for (int i = threadIdx.x; i < n_flags; i += K::THREADS) (&s_to[0][0][0])[(i / Tn) * (K::N / 8) + (i % Tn)] = *flag_addr(grp, i);
+    __syncthreads();
+    for (int it = 0; w < n_work; w += gridDim.x, ++it) {
+        const int cur = it & 1;
+        const unsigned int w_next = w + gridDim.x;
+        const bool has_next = w_next < n_work;
+        const size_t grp_next = has_next ? list[w_next] : 0;
         C* g = stack + (grp * K::RPC + rl) * K::N;
-        // only the tiles some footprint reaches hold gridded data (tile_occ); whatever else the row holds
-        // (rick_image leaves the previous transform there) is not read and counts as zero
-        for (int i = threadIdx.x; i < K::RPC * Tn; i += K::THREADS) {
-            const int a = i / Tn, ti = i - a * Tn;
-            const size_t R = grp * K::RPC + a;          // slot-major row
-            const size_t slot = R / K::N;
-            const int row = (int)(R - slot * K::N);
-            s_to[a][ti] = tocc[(slot * Tn + (size_t)(row >> log2B)) * Tn + ti];
-        }
-        __syncthreads();
         C v[16];
 #pragma unroll
         for (int e = 0; e < 16; ++e) {
@@ -70,12 +80,25 @@ k_fft_rows(typename cplx_of<T>::type* __restrict__ stack,
             C x;
             x.x = 0;
             x.y = 0;
-            if (s_to[rl][i >> log2B]) x = g[i];
+            if (s_to[cur][rl][i >> log2B]) x = g[i];
             v[e] = x;
+        }
+        unsigned char f0 = 0, f1 = 0;
+        if (has_next) {
+            if ((int)threadIdx.x < n_flags) f0 = *flag_addr(grp_next, threadIdx.x);
+            if ((int)threadIdx.x + K::THREADS < n_flags) f1 = *flag_addr(grp_next, threadIdx.x + K::THREADS);
         }
         fft_thread<T, LOG2N>(v, t, sm, 1, 0, tw);
 #pragma unroll
         for (int e = 0; e < 16; ++e) g[t + K::NT * ((e + 8) & 15)] = v[e];
+        if (has_next) {
+            unsigned char* nx = &s_to[cur ^ 1][0][0];
+            const int i0 = threadIdx.x, i1 = threadIdx.x + K::THREADS;
+            if (i0 < n_flags) nx[(i0 / Tn) * (K::N / 8) + (i0 % Tn)] = f0;
+            if (i1 < n_flags) nx[(i1 / Tn) * (K::N / 8) + (i1 % Tn)] = f1;
+        }
+        __syncthreads();
+        grp = grp_next;
     }
 }
 
