@@ -193,7 +193,12 @@ k_index_key(const double* __restrict__ uvw, const float* __restrict__ wgt,
 // items once (k_radix_onesweep).
 // ------------------------------------------------------------------------------------------
 #define RS_THREADS 256
-#define RS_ITEMS 16
+#ifndef RS_ITEMS
+#define RS_ITEMS 12      // items per thread; 12 x 256 threads x 4 CTAs per SM measured best on B200 (0.59 vs 0.62 ms at 16 x 3)
+#endif
+#ifndef RS_MINB
+#define RS_MINB 4
+#endif
 #define RS_TILE (RS_THREADS * RS_ITEMS)
 typedef unsigned long long u64;
 
@@ -230,7 +235,10 @@ __global__ void __launch_bounds__(256) k_digit_bases(const unsigned int* __restr
 #define OS_AGG (1ull << 62)
 #define OS_INC (2ull << 62)
 #define OS_VAL ((1ull << 62) - 1ull)
-__global__ void __launch_bounds__(RS_THREADS, 3)
+#ifndef OS_LB
+#define OS_LB 8u
+#endif
+__global__ void __launch_bounds__(RS_THREADS, RS_MINB)
 k_radix_onesweep(const u64* __restrict__ in, u64* __restrict__ out, unsigned int M, int shift, uint32_t mask,
                  int nbins, const unsigned long long* __restrict__ gbase, volatile unsigned long long* status,
                  unsigned int* __restrict__ ticket)
@@ -260,7 +268,16 @@ k_radix_onesweep(const u64* __restrict__ in, u64* __restrict__ out, unsigned int
         const unsigned long long idx = base + (unsigned)i * 32 + lane;
         const bool valid = idx < M;
         const uint32_t d = (uint32_t)(it[i] >> shift) & mask;
-        const unsigned int m = __match_any_sync(0xffffffffu, valid ? d : 0xFFFFu);
+        // lanes with the same digit: eight ballots, one per digit bit (MATCH.ANY costs several times that on
+        // sm_100: it was 39 % of this kernel's stall samples, profiles/r1d_ncu_full.md)
+        unsigned int m = __ballot_sync(0xffffffffu, valid);
+        if (!valid) m = ~m;
+#pragma unroll
+        for (int b = 0; b < 8; ++b) {
+            const bool bit = (d >> b) & 1u;
+            const unsigned int bal = __ballot_sync(0xffffffffu, bit);
+            m &= bit ? bal : ~bal;
+        }
         const int leader = __ffs(m) - 1;
         uint32_t old = 0;
         if (valid && lane == leader) {
@@ -291,16 +308,30 @@ k_radix_onesweep(const u64* __restrict__ in, u64* __restrict__ out, unsigned int
             *st = OS_INC | (unsigned long long)total;
         } else {
             *st = OS_AGG | (unsigned long long)total;
+            // look-back over the preceding tiles, OS_LB status words in flight at a time (a single dependent
+            // read per step made every tile wait on a chain of L2 round trips)
             const volatile unsigned long long* q = st - 256;
-            for (unsigned int back = tile; back > 0; --back, q -= 256) {
-                unsigned long long v;
-                unsigned int spins = 0;
-                while (((v = *q) >> 62) == 0ull) {
-                    __nanosleep(40);
-                    if (++spins > (1u << 24)) __trap();      // a lost predecessor: fail loudly, never hang
+            bool done = false;
+            for (unsigned int back = tile; back > 0 && !done;) {
+                const unsigned int n = back < OS_LB ? back : OS_LB;
+                unsigned long long v[OS_LB];
+#pragma unroll
+                for (unsigned int j = 0; j < OS_LB; ++j) v[j] = j < n ? q[-256 * (long long)j] : 0ull;
+#pragma unroll
+                for (unsigned int j = 0; j < OS_LB; ++j) {
+                    if (j < n && !done) {
+                        unsigned int spins = 0;
+                        while ((v[j] >> 62) == 0ull) {
+                            __nanosleep(40);
+                            if (++spins > (1u << 24)) __trap();      // a lost predecessor: fail loudly, never hang
+                            v[j] = q[-256 * (long long)j];
+                        }
+                        excl += v[j] & OS_VAL;
+                        if ((v[j] >> 62) == 2ull) done = true;
+                    }
                 }
-                excl += v & OS_VAL;
-                if ((v >> 62) == 2ull) break;
+                back -= n;
+                q -= 256 * (long long)n;
             }
             *st = OS_INC | (excl + (unsigned long long)total);
         }
