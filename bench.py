@@ -115,7 +115,7 @@ def main():
     wl = make_workload(args, "cuda")
     vis, uvw, wgt = rick.to_device(wl)
     plan = rick.plan_from_workload(wl)
-    image = torch.empty((wl.n, wl.n), dtype=torch.float64, device="cuda")
+    image = torch.empty((wl.n_chan, wl.n, wl.n) if wl.cube else (wl.n, wl.n), dtype=torch.float64, device="cuda")
     E = 8 if wl.grid_prec == "f32" else 16
     stack_bytes = wl.n * wl.n * wl.n_wplanes * E
     image_bytes = wl.n * wl.n * 8

@@ -162,6 +162,9 @@ class Plan:
             shape = (n_chan, self.n, self.n) if self.cube else (self.n, self.n)
             image_out = torch.empty(shape, dtype=torch.float64, device=vis.device)
         assert image_out.dtype == torch.float64 and image_out.is_cuda and image_out.is_contiguous()
+        need = (n_chan if self.cube else 1) * self.n * self.n
+        if image_out.numel() != need:      # the C ABI cannot see the buffer's size: check it here
+            raise ValueError(f"image_out has {image_out.numel()} elements, this plan writes {need}")
         self._check(self._lib.rick_image(self._h, _dev_ptr(vis), self._vis_dtype(vis), _dev_ptr(uvw_m),
                                          _dev_ptr(weights), fp, n_chan, n_rows, _dev_ptr(image_out)))
         return image_out
@@ -173,6 +176,9 @@ class Plan:
         for t in (vis, uvw_m, image_out) + (() if weights is None else (weights,)):
             assert (not t.is_cuda) and t.is_contiguous()
         self._n_vis = n_rows * n_chan
+        need = (n_chan if self.cube else 1) * self.n * self.n
+        if image_out.numel() != need or image_out.dtype != torch.float64:
+            raise ValueError(f"image_out must hold {need} float64 values")
         self._check(self._lib.rick_image_host(
             self._h, C.c_void_p(vis.data_ptr()), self._vis_dtype(vis), C.c_void_p(uvw_m.data_ptr()),
             None if weights is None else C.c_void_p(weights.data_ptr()),
@@ -186,6 +192,8 @@ class Plan:
         for t in (vis, uvw_m, image_out) + (() if weights is None else (weights,)):
             assert (not t.is_cuda) and t.is_contiguous()
         self._n_vis = n_rows * n_chan
+        if image_out.numel() != self.n * self.n or image_out.dtype != torch.float64:
+            raise ValueError(f"image_out must hold {self.n * self.n} float64 values")
         self._check(self._lib.rick_image_stream_host(
             self._h, C.c_void_p(vis.data_ptr()), self._vis_dtype(vis), C.c_void_p(uvw_m.data_ptr()),
             None if weights is None else C.c_void_p(weights.data_ptr()),

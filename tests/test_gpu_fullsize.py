@@ -67,9 +67,19 @@ def test_cfg2_full_meerkat_whole_image_keys_perm():
     assert wl.n_vis == 16515072 and wl.n == 4096 and wl.n_wplanes == 32
     plan, img, st = _gpu_image(wl)
     keys, perm = plan.debug_keys(), plan.debug_perm()
+    # the host-buffer entry bench.py's e2e leg times: at this size it grids the set in two chunks
+    # (rick_image_stream_host), so the image agrees up to summation order and the statistics exactly
+    import torch
+    hv = torch.from_numpy(np.ascontiguousarray(wl.vis)).pin_memory()
+    hu = torch.from_numpy(np.ascontiguousarray(wl.uvw_m)).pin_memory()
+    hout = torch.full((wl.n, wl.n), float("nan"), dtype=torch.float64).pin_memory()
+    plan.rick_image_host(hv, hu, None, wl.freq_hz, hout)
+    st_host = plan.rick_get_stats()
     plan.destroy()
     o = oracle.image(wl.uvw_m, wl.freq_hz, wl.vis, None, wl.n, wl.n_wplanes, wl.support, wl.pixel_rad)
     _stats_equal(st, o["stats"])
+    _stats_equal(st_host, o["stats"])
+    assert _report("cfg2 full, host entry", hout.numpy(), o["image"]) <= TOL64
     idx = oracle.index(wl.uvw_m, wl.freq_hz, wl.n, wl.n_wplanes, wl.support, wl.pixel_rad, 16)
     assert np.array_equal(keys, idx["key"])                        # bit-exact
     assert np.array_equal(perm, oracle.sort(idx["key"]))           # bit-exact, stable
