@@ -159,7 +159,9 @@ const char* rick_last_error(const rick_plan_t* p);
  * of *key_bits bits for a dropped visibility.  sorted = 0: in visibility order (item k describes
  * visibility k); sorted = 1: after the stable sort by key -- the low parts are then the permutation. */
 const uint64_t* rick_debug_items(rick_plan_t* p, int32_t sorted, int32_t* idx_bits, int32_t* key_bits);
-void*           rick_debug_planes(rick_plan_t* p); /* [N_w][N][N] complex of grid_prec      */
+void*           rick_debug_planes(rick_plan_t* p); /* [N_w][N][N] complex of grid_prec; meaningful after the
+                                                    * STAGED calls only: rick_image leaves the stack
+                                                    * untransformed (N = 4096 fp64) or row-permuted (N >= 8192) */
 
 /* Per-kernel timing with CUDA events on the plan's stream (for roofline reporting).
  * rick_profile(p, 1) clears the records and brackets every later kernel launch with a

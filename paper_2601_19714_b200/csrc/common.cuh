@@ -45,6 +45,7 @@ struct rick_plan_s {
 
     // tables
     void* twiddle;           // [N] complex of grid_prec: e^{+2 pi i k/N}
+    void* twiddle2;          // [N/16] e^{+2 pi i k/(N/16)}: the long-column two-pass transform (N >= 8192), else null
     double* taper;           // [N] c((p-N/2)/N)
     double kb_poly[15 * (RICK_KB_DEG + 1)];   // host: [S][DEG+1], tap a on d = (a-h) - s/2, s in [-1,1]
 
@@ -163,13 +164,18 @@ int rick_grid_planes(rick_plan_t* p, const void* vis, int vis_dtype, const doubl
 int rick_fft_planes(rick_plan_t* p, int plane_first, int n_planes);      // fft.cu: rows then columns (in place)
 int rick_fft_rows(rick_plan_t* p, int plane_first, int n_planes);        // fft.cu: occupied rows only
 int rick_fft_cols(rick_plan_t* p, int n_planes);                         // fft.cu (generic strided pass)
+// fft.cu: column pass of rick_image for long columns (N >= 8192) as two passes at full line width; leaves the
+// rows of every plane PERMUTED: memory row 16 (q mod N/16) + q / (N/16) holds pixel row q (rick_cols2_perm)
+int rick_fft_cols2(rick_plan_t* p, int n_planes);
+int rick_cols2_perm(const rick_plan_t* p);   // log2(N/16) when rick_fft_cols2 applies to this plan, else 0
 int rick_cols12_init(rick_plan_t* p);                                    // fft_cols12.cu
 int rick_cols12_fft(rick_plan_t* p, int n_planes);                       // fft_cols12.cu
 int rick_cols12_wcorrect(rick_plan_t* p, int img, int z_first, int n_planes, double* image,
                          int accumulate, int fuse_taper, int strip_begin, int strip_end);   // fft_cols12.cu
 int rick_cols12_strips(void);                                            // fft_cols12.cu
+// row_perm: 0 = planes in natural row order; else log2(N/16), the row order rick_fft_cols2 leaves
 int rick_wcorrect(rick_plan_t* p, int img, int z_first, int n_planes, double* image,
-                  int accumulate, int fuse_taper);                     // wcorrect.cu
+                  int accumulate, int fuse_taper, int row_perm = 0);   // wcorrect.cu
 int rick_taper_divide(rick_plan_t* p, double* image);                    // wcorrect.cu
 
 // ordered (monotone) encoding of doubles for atomicMin/atomicMax on u64

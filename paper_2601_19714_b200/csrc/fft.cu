@@ -176,6 +176,110 @@ static int launch_fft(rick_plan_t* p, int plane_first, int n_planes, int which) 
     return RICK_OK;
 }
 
+
+// ------------------------------------------------------------------------------------------
+// Long columns (N >= 8192: a column is 128 KB and one SM can hold a single one, so the strided pass above
+// touches HBM in 16-byte pieces with nothing in flight while it transforms: 1.8 TB/s at N = 8192 fp64,
+// 1.1 TB/s at N = 16384 fp32).  rick_image transforms them in TWO passes at full line width instead
+// ("four-step", N = 16 N2, n = n1 + 16 n2, m = m2 + N2 m1):
+//     X[m2 + N2 m1] = sum_n1 W16^(n1 m1) [ W_N^(n1 m2) sum_n2 x[n1 + 16 n2] W_N2^(n2 m2) ]
+//   pass A (k_fft_cols_a): for each n1 the N2-point transform over rows n1 + 16 n2 of a strip of 8 columns
+//     (128-byte pieces in fp64, the same in-register Stockham core as the row pass), times W_N^(n1 m2), stored at
+//     row n1 + 16 m2;
+//   pass B (k_fft_cols_b): for each m2 one THREAD transforms the 16 consecutive rows 16 m2 + n1 of its column
+//     in registers (no exchange at all; a warp moves 512 contiguous bytes per row).
+// Six transfers of the stack instead of four, all at the copy rate.  The centring is the rotation by N2/2
+// in n2 (pass A input, e -> (e+8) mod 16) and by 8 in m1 (pass B output); pass B stores in place, so memory
+// row 16 m2 + s holds pixel row q = m2 + N2 s: the correction pass reads rows through that permutation
+// (rick_cols2_perm) and no pass ever un-permutes the planes.  The staged API keeps the single-pass kernel
+// (its planes are in natural order).
+template <typename T, int LOG2N> struct Col2Cfg {
+    static constexpr int N = 1 << LOG2N, LOG2N2 = LOG2N - 4, N2 = N / 16, NT2 = N2 / 16;
+    static constexpr int W = 8;      // 128-byte (fp64) / 64-byte (fp32) row pieces; 16 fp32 columns measured no faster
+    static constexpr int THREADS = NT2 * W;
+    static constexpr size_t SMEM = (size_t)W * (N2 + N2 / 16) * 2 * sizeof(T);
+};
+
+template <typename T, int LOG2N>
+__global__ void __launch_bounds__(Col2Cfg<T, LOG2N>::THREADS, 512 / Col2Cfg<T, LOG2N>::THREADS)
+k_fft_cols_a(typename cplx_of<T>::type* __restrict__ stack, const typename cplx_of<T>::type* __restrict__ tw2,
+             const typename cplx_of<T>::type* __restrict__ twN)
+{
+    typedef typename cplx_of<T>::type C;
+    typedef Col2Cfg<T, LOG2N> K;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    C* sm = reinterpret_cast<C*>(smem_raw);
+    constexpr int STRIPS = K::N / K::W;
+    const int n1 = blockIdx.x & 15;                    // the 16 CTAs of a strip are launched together
+    const unsigned int rest = blockIdx.x >> 4;
+    const int strip = (int)(rest % STRIPS), plane = (int)(rest / STRIPS);
+    const int c = threadIdx.x % K::W, t = threadIdx.x / K::W;
+    C* g = stack + (size_t)plane * K::N * K::N + (size_t)n1 * K::N + (size_t)strip * K::W + c;
+    C v[16];
+#pragma unroll
+    for (int e = 0; e < 16; ++e) v[e] = g[(size_t)16 * (t + K::NT2 * ((e + 8) & 15)) * K::N];
+    fft_thread<T, K::LOG2N2>(v, t, sm, K::W, c, tw2);
+#pragma unroll
+    for (int e = 0; e < 16; ++e) {
+        const int m2 = t + K::NT2 * e;
+        C x = v[e];
+        if (n1) x = cmul(x, twN[n1 * m2]);
+        g[(size_t)16 * m2 * K::N] = x;
+    }
+}
+
+template <typename T, int LOG2N>
+__global__ void __launch_bounds__(256)
+k_fft_cols_b(typename cplx_of<T>::type* __restrict__ stack, size_t n_threads)
+{
+    typedef typename cplx_of<T>::type C;
+    constexpr int N = 1 << LOG2N, N2 = N / 16;
+    const size_t gid = (size_t)blockIdx.x * 256 + threadIdx.x;       // (plane, m2, column), column fastest
+    if (gid >= n_threads) return;
+    const int p = (int)(gid & (size_t)(N - 1));
+    const size_t rest = gid >> LOG2N;
+    const int m2 = (int)(rest & (size_t)(N2 - 1));
+    const size_t plane = rest >> (LOG2N - 4);
+    C* g = stack + plane * N * N + (size_t)(16 * m2) * N + p;
+    C b[16];
+#pragma unroll
+    for (int n1 = 0; n1 < 16; ++n1) b[n1] = g[(size_t)n1 * N];
+    fft16<T>(b);
+#pragma unroll
+    for (int m1 = 0; m1 < 16; ++m1) g[(size_t)((m1 + 8) & 15) * N] = b[leg_reg<16>(m1)];
+}
+
+template <typename T, int LOG2N> static int launch_cols2(rick_plan_t* p, int n_planes)
+{
+    typedef typename cplx_of<T>::type C;
+    typedef Col2Cfg<T, LOG2N> K;
+    const int rcd = rick_all_dirty(p, n_planes);       // both passes write every row of the slots
+    if (rcd) return rcd;
+    RICK_CUDA(p, cudaFuncSetAttribute(k_fft_cols_a<T, LOG2N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)K::SMEM));
+    const unsigned int blocks_a = (unsigned int)((size_t)n_planes * (K::N / K::W) * 16);
+    RICK_KERNEL(p, RK_FFT_COLS, k_fft_cols_a<T, LOG2N><<<blocks_a, K::THREADS, K::SMEM, p->stream>>>(
+        (C*)p->stack, (const C*)p->twiddle2, (const C*)p->twiddle));
+    const size_t n_threads = (size_t)n_planes * K::N2 * K::N;
+    RICK_KERNEL(p, RK_FFT_COLS, k_fft_cols_b<T, LOG2N><<<(unsigned int)((n_threads + 255) / 256), 256, 0, p->stream>>>(
+        (C*)p->stack, n_threads));
+    return RICK_OK;
+}
+
+int rick_cols2_perm(const rick_plan_t* p) { return p->log2N >= 13 ? p->log2N - 4 : 0; }
+
+int rick_fft_cols2(rick_plan_t* p, int n_planes)
+{
+    if (n_planes <= 0) return RICK_OK;
+    if (p->f32) {
+        if (p->log2N == 13) return launch_cols2<float, 13>(p, n_planes);
+        if (p->log2N == 14) return launch_cols2<float, 14>(p, n_planes);
+    } else if (p->log2N == 13) {
+        return launch_cols2<double, 13>(p, n_planes);
+    }
+    p->err = "two-pass column transform: grid edge not supported";
+    return RICK_ERR_INVALID;
+}
+
 static int fft_dispatch(rick_plan_t* p, int plane_first, int n_planes, int which)
 {
     if (n_planes <= 0) return RICK_OK;

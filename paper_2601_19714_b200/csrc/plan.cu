@@ -87,7 +87,7 @@ extern "C" int rick_plan_destroy(rick_plan_t* p)
 {
     if (!p) return RICK_OK;
     cudaStreamSynchronize(p->stream);
-    free_dev(p->twiddle); free_dev(p->taper); free_dev(p->stack); free_dev(p->image);
+    free_dev(p->twiddle); free_dev(p->twiddle2); free_dev(p->taper); free_dev(p->stack); free_dev(p->image);
     free_dev(p->items); free_dev(p->items_a); free_dev(p->items_b);
     free_dev(p->os_small); free_dev(p->os_gbase); free_dev(p->os_status); free_dev(p->plane_start); free_dev(p->chan_scale);
     free_dev(p->row_occ); free_dev(p->row_dirty); free_dev(p->tile_occ); free_dev(p->row_list);
@@ -391,8 +391,14 @@ static int transform_and_correct(rick_plan_t* p, int img, int z0, int nb, double
             if ((rc = rick_cols12_wcorrect(p, img, z0, nb, dst, z0 > 0, last, 0, strips))) return rc;
         }
     } else {
-        if ((rc = rick_fft_planes(p, img * p->Nw + z0, nb))) return rc;
-        if ((rc = rick_wcorrect(p, img, z0, nb, dst, z0 > 0, last))) return rc;
+        const int perm = rick_cols2_perm(p);
+        if (perm) {       // long columns: two passes at full line width, rows left permuted for the correction
+            if ((rc = rick_fft_rows(p, img * p->Nw + z0, nb))) return rc;
+            if ((rc = rick_fft_cols2(p, nb))) return rc;
+        } else {
+            if ((rc = rick_fft_planes(p, img * p->Nw + z0, nb))) return rc;
+        }
+        if ((rc = rick_wcorrect(p, img, z0, nb, dst, z0 > 0, last, perm))) return rc;
     }
     return RICK_OK;
 }

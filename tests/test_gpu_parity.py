@@ -371,3 +371,25 @@ def test_stream_host_weights_fused_4096():
         assert st["n_gridded"] == o["stats"]["n_gridded"]
         assert abs(st["sum_w"] - o["stats"]["sum_w"]) <= 1e-9 * abs(o["stats"]["sum_w"])
     plan.destroy()
+
+
+@pytest.mark.parametrize("prec,pb,tol", [("f64", 0, TOL64), ("f64", 2, TOL64), ("f32", 0, TOL32)])
+def test_long_columns_two_pass(prec, pb, tol):
+    """N = 8192: rick_image transforms the columns in two passes (N = 16 x 512) and leaves the rows of the
+    planes permuted for the correction pass; whole image against the oracle, all planes resident and in
+    ragged batches 2 + 1 (accumulate path), fp64 and fp32 grid.  (N = 16384 fp32: tests/test_gpu_fullsize.py.)"""
+    rick = _rick()
+    wl = synth.make_config(3, n_times=4, n_wplanes=3, n_src=6)
+    assert wl.n == 8192
+    wl.grid_prec = prec
+    o = _oracle(wl)
+    plan = rick.plan_from_workload(wl, plane_batch=pb)
+    vis, uvw, wgt = rick.to_device(wl)
+    img = plan.rick_image(vis, uvw, wgt, wl.freq_hz).cpu().numpy()
+    img2 = plan.rick_image(vis, uvw, wgt, wl.freq_hz).cpu().numpy()        # all rows dirty after the first call
+    st = plan.rick_get_stats()
+    plan.destroy()
+    e = _rel(img, o["image"])
+    print(f"N=8192 two-pass columns {prec} plane_batch={pb}: rel L2 {e:.2e}")
+    assert e <= tol and _rel(img2, o["image"]) <= tol
+    assert st["n_gridded"] == o["stats"]["n_gridded"]
