@@ -156,7 +156,9 @@ int rick_tables_build(rick_plan_t* p);                                   // tabl
 int rick_index_sort(rick_plan_t* p, const double* uvw_m, const float* weights, int flags = 0);   // index_sort.cu
 int rick_wrange_all(rick_plan_t* p, const double* uvw_m, int64_t n_rows);                         // index_sort.cu
 int rick_zero_dirty(rick_plan_t* p, int n_slots, cudaStream_t st);        // grid.cu: zero the dirty rows of slots 0..n_slots-1
-int rick_zero_sparse(rick_plan_t* p, int plane_first, int n_slots);     // grid.cu: stale rows whole, occupied rows by tile
+// grid.cu: occupied rows by tile; stale rows whole unless keep_stale (the two-pass column transform never reads
+// a row that is not occupied, so rick_image leaves such rows dirty instead of clearing them)
+int rick_zero_sparse(rick_plan_t* p, int plane_first, int n_slots, int keep_stale = 0);
 int rick_mark_dirty(rick_plan_t* p, int plane_first, int n_planes);      // grid.cu: dirty |= occupancy of the batch
 int rick_all_dirty(rick_plan_t* p, int n_slots);                         // grid.cu: after an in-place column pass
 int rick_grid_planes(rick_plan_t* p, const void* vis, int vis_dtype, const double* uvw_m,
@@ -166,7 +168,7 @@ int rick_fft_rows(rick_plan_t* p, int plane_first, int n_planes);        // fft.
 int rick_fft_cols(rick_plan_t* p, int n_planes);                         // fft.cu (generic strided pass)
 // fft.cu: column pass of rick_image for long columns (N >= 8192) as two passes at full line width; leaves the
 // rows of every plane PERMUTED: memory row 16 (q mod N/16) + q / (N/16) holds pixel row q (rick_cols2_perm)
-int rick_fft_cols2(rick_plan_t* p, int n_planes);
+int rick_fft_cols2(rick_plan_t* p, int plane_first, int n_planes);
 int rick_cols2_perm(const rick_plan_t* p);   // log2(N/16) when rick_fft_cols2 applies to this plan, else 0
 int rick_cols12_init(rick_plan_t* p);                                    // fft_cols12.cu
 int rick_cols12_fft(rick_plan_t* p, int n_planes);                       // fft_cols12.cu

@@ -203,7 +203,7 @@ template <typename T, int LOG2N> struct Col2Cfg {
 template <typename T, int LOG2N>
 __global__ void __launch_bounds__(Col2Cfg<T, LOG2N>::THREADS, 512 / Col2Cfg<T, LOG2N>::THREADS)
 k_fft_cols_a(typename cplx_of<T>::type* __restrict__ stack, const typename cplx_of<T>::type* __restrict__ tw2,
-             const typename cplx_of<T>::type* __restrict__ twN)
+             const typename cplx_of<T>::type* __restrict__ twN, const unsigned char* __restrict__ occ)
 {
     typedef typename cplx_of<T>::type C;
     typedef Col2Cfg<T, LOG2N> K;
@@ -215,9 +215,19 @@ k_fft_cols_a(typename cplx_of<T>::type* __restrict__ stack, const typename cplx_
     const int strip = (int)(rest % STRIPS), plane = (int)(rest / STRIPS);
     const int c = threadIdx.x % K::W, t = threadIdx.x / K::W;
     C* g = stack + (size_t)plane * K::N * K::N + (size_t)n1 * K::N + (size_t)strip * K::W + c;
+    // rows no footprint reaches were never transformed by the row pass and count as zero: they are not read
+    // (and rick_image does not clear them, rick_zero_sparse keep_stale); the pass writes every row
+    const unsigned char* oc = occ + (size_t)plane * K::N + n1;
     C v[16];
 #pragma unroll
-    for (int e = 0; e < 16; ++e) v[e] = g[(size_t)16 * (t + K::NT2 * ((e + 8) & 15)) * K::N];
+    for (int e = 0; e < 16; ++e) {
+        const int n2 = t + K::NT2 * ((e + 8) & 15);
+        C x;
+        x.x = 0;
+        x.y = 0;
+        if (oc[16 * n2]) x = g[(size_t)16 * n2 * K::N];
+        v[e] = x;
+    }
     fft_thread<T, K::LOG2N2>(v, t, sm, K::W, c, tw2);
 #pragma unroll
     for (int e = 0; e < 16; ++e) {
@@ -249,7 +259,7 @@ k_fft_cols_b(typename cplx_of<T>::type* __restrict__ stack, size_t n_threads)
     for (int m1 = 0; m1 < 16; ++m1) g[(size_t)((m1 + 8) & 15) * N] = b[leg_reg<16>(m1)];
 }
 
-template <typename T, int LOG2N> static int launch_cols2(rick_plan_t* p, int n_planes)
+template <typename T, int LOG2N> static int launch_cols2(rick_plan_t* p, int plane_first, int n_planes)
 {
     typedef typename cplx_of<T>::type C;
     typedef Col2Cfg<T, LOG2N> K;
@@ -258,7 +268,7 @@ template <typename T, int LOG2N> static int launch_cols2(rick_plan_t* p, int n_p
     RICK_CUDA(p, cudaFuncSetAttribute(k_fft_cols_a<T, LOG2N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)K::SMEM));
     const unsigned int blocks_a = (unsigned int)((size_t)n_planes * (K::N / K::W) * 16);
     RICK_KERNEL(p, RK_FFT_COLS, k_fft_cols_a<T, LOG2N><<<blocks_a, K::THREADS, K::SMEM, p->stream>>>(
-        (C*)p->stack, (const C*)p->twiddle2, (const C*)p->twiddle));
+        (C*)p->stack, (const C*)p->twiddle2, (const C*)p->twiddle, p->row_occ + (size_t)plane_first * p->N));
     const size_t n_threads = (size_t)n_planes * K::N2 * K::N;
     RICK_KERNEL(p, RK_FFT_COLS, k_fft_cols_b<T, LOG2N><<<(unsigned int)((n_threads + 255) / 256), 256, 0, p->stream>>>(
         (C*)p->stack, n_threads));
@@ -267,14 +277,14 @@ template <typename T, int LOG2N> static int launch_cols2(rick_plan_t* p, int n_p
 
 int rick_cols2_perm(const rick_plan_t* p) { return p->log2N >= 13 ? p->log2N - 4 : 0; }
 
-int rick_fft_cols2(rick_plan_t* p, int n_planes)
+int rick_fft_cols2(rick_plan_t* p, int plane_first, int n_planes)
 {
     if (n_planes <= 0) return RICK_OK;
     if (p->f32) {
-        if (p->log2N == 13) return launch_cols2<float, 13>(p, n_planes);
-        if (p->log2N == 14) return launch_cols2<float, 14>(p, n_planes);
+        if (p->log2N == 13) return launch_cols2<float, 13>(p, plane_first, n_planes);
+        if (p->log2N == 14) return launch_cols2<float, 14>(p, plane_first, n_planes);
     } else if (p->log2N == 13) {
-        return launch_cols2<double, 13>(p, n_planes);
+        return launch_cols2<double, 13>(p, plane_first, n_planes);
     }
     p->err = "two-pass column transform: grid edge not supported";
     return RICK_ERR_INVALID;

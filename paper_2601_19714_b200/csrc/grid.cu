@@ -462,7 +462,7 @@ __global__ void __launch_bounds__(256) k_zero_dirty_rows(uint4* __restrict__ sta
 __global__ void __launch_bounds__(256) k_zero_sparse(uint4* __restrict__ stack, unsigned char* __restrict__ dirty,
                                                      const unsigned char* __restrict__ occ,
                                                      const unsigned char* __restrict__ tocc, size_t n_rows, int N,
-                                                     int log2B, int T, size_t row16, int unit16)
+                                                     int log2B, int T, size_t row16, int unit16, int keep_stale)
 {
     const uint4 z = make_uint4(0, 0, 0, 0);
     const int lane = threadIdx.x & 31;
@@ -472,6 +472,7 @@ __global__ void __launch_bounds__(256) k_zero_sparse(uint4* __restrict__ stack, 
         if (!dirty[r]) continue;
         uint4* dst = stack + r * row16;
         if (!occ[r]) {
+            if (keep_stale) continue;      // nobody reads this row before it is written again; it stays dirty
             for (size_t i = lane; i < row16; i += 32) dst[i] = z;
             __syncwarp();
             if (lane == 0) dirty[r] = 0;
@@ -509,14 +510,14 @@ int rick_zero_dirty(rick_plan_t* p, int n_slots, cudaStream_t st)
 }
 
 // slots 0..n_slots-1 are about to receive global planes plane_first.. (occupancy of the current sort)
-int rick_zero_sparse(rick_plan_t* p, int plane_first, int n_slots)
+int rick_zero_sparse(rick_plan_t* p, int plane_first, int n_slots, int keep_stale)
 {
     const size_t cell = p->f32 ? 8 : 16;
     const size_t row16 = p->plane_bytes / 16 / (size_t)p->N;
     const int unit16 = (int)((size_t)p->B * cell / 16);
     RICK_KERNEL(p, RK_ZERO, k_zero_sparse<<<p->n_sm * 8, 256, 0, p->stream>>>(
         reinterpret_cast<uint4*>(p->stack), p->row_dirty, p->row_occ + (size_t)plane_first * p->N,
-        p->tile_occ + (size_t)plane_first * p->T * p->T, (size_t)n_slots * p->N, p->N, p->log2B, p->T, row16, unit16));
+        p->tile_occ + (size_t)plane_first * p->T * p->T, (size_t)n_slots * p->N, p->N, p->log2B, p->T, row16, unit16, keep_stale));
     return RICK_OK;
 }
 

@@ -394,7 +394,7 @@ static int transform_and_correct(rick_plan_t* p, int img, int z0, int nb, double
         const int perm = rick_cols2_perm(p);
         if (perm) {       // long columns: two passes at full line width, rows left permuted for the correction
             if ((rc = rick_fft_rows(p, img * p->Nw + z0, nb))) return rc;
-            if ((rc = rick_fft_cols2(p, nb))) return rc;
+            if ((rc = rick_fft_cols2(p, img * p->Nw + z0, nb))) return rc;
         } else {
             if ((rc = rick_fft_planes(p, img * p->Nw + z0, nb))) return rc;
         }
@@ -425,7 +425,8 @@ static int image_impl(rick_plan_t* p, const void* vis, int32_t vis_dtype, const 
         for (int z0 = 0; z0 < p->Nw; z0 += p->batch) {
             const int nb = p->Nw - z0 < p->batch ? p->Nw - z0 : p->batch;
             const int last = z0 + nb >= p->Nw;
-            if ((rc = rick_zero_sparse(p, img * p->Nw + z0, nb))) return rc;
+            // (the two-pass column transform reads occupied rows only: stale rows need no clearing)
+            if ((rc = rick_zero_sparse(p, img * p->Nw + z0, nb, !p->cols12_ok && rick_cols2_perm(p) != 0))) return rc;
             if ((rc = rick_mark_dirty(p, img * p->Nw + z0, nb))) return rc;
             if ((rc = rick_grid_planes(p, vis, vis_dtype, uvw_m, weights, img * p->Nw + z0, nb))) return rc;
             if ((rc = transform_and_correct(p, img, z0, nb, dst, last, host_out, &host_done))) return rc;
