@@ -193,6 +193,9 @@ static int launch_fft(rick_plan_t* p, int plane_first, int n_planes, int which) 
 // row 16 m2 + s holds pixel row q = m2 + N2 s: the correction pass reads rows through that permutation
 // (rick_cols2_perm) and no pass ever un-permutes the planes.  The staged API keeps the single-pass kernel
 // (its planes are in natural order).
+#ifndef C2_MINB
+#define C2_MINB 512
+#endif
 template <typename T, int LOG2N> struct Col2Cfg {
     static constexpr int N = 1 << LOG2N, LOG2N2 = LOG2N - 4, N2 = N / 16, NT2 = N2 / 16;
     static constexpr int W = 8;      // 128-byte (fp64) / 64-byte (fp32) row pieces; 16 fp32 columns measured no faster
@@ -201,7 +204,7 @@ template <typename T, int LOG2N> struct Col2Cfg {
 };
 
 template <typename T, int LOG2N>
-__global__ void __launch_bounds__(Col2Cfg<T, LOG2N>::THREADS, 512 / Col2Cfg<T, LOG2N>::THREADS)
+__global__ void __launch_bounds__(Col2Cfg<T, LOG2N>::THREADS, C2_MINB / Col2Cfg<T, LOG2N>::THREADS)
 k_fft_cols_a(typename cplx_of<T>::type* __restrict__ stack, const typename cplx_of<T>::type* __restrict__ tw2,
              const typename cplx_of<T>::type* __restrict__ twN, const unsigned char* __restrict__ occ)
 {
@@ -229,12 +232,18 @@ k_fft_cols_a(typename cplx_of<T>::type* __restrict__ stack, const typename cplx_
         v[e] = x;
     }
     fft_thread<T, K::LOG2N2>(v, t, sm, K::W, c, tw2);
+    // four outputs at a time: their twiddle loads are not hoisted above the transform (register budget)
 #pragma unroll
-    for (int e = 0; e < 16; ++e) {
-        const int m2 = t + K::NT2 * e;
-        C x = v[e];
-        if (n1) x = cmul(x, twN[n1 * m2]);
-        g[(size_t)16 * m2 * K::N] = x;
+    for (int e0 = 0; e0 < 16; e0 += 4) {
+        asm volatile("" ::: "memory");
+        C w[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) w[i] = twN[n1 * (t + K::NT2 * (e0 + i))];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const int m2 = t + K::NT2 * (e0 + i);
+            g[(size_t)16 * m2 * K::N] = cmul(v[e0 + i], w[i]);      // twN[0] = 1 when n1 = 0
+        }
     }
 }
 
