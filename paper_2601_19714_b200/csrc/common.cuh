@@ -98,6 +98,9 @@ struct rick_plan_s {
     cudaEvent_t ev_chunk_in[2], ev_chunk_free[2];
 
     // N = 4096 fp64 column kernels (fft_cols12.cu): TMA tensor map over the resident stack
+    // cube plans with all planes of an image resident keep img_batch images' stacks resident (slots = batch *
+    // img_batch) so that zero-fill, gridder and row pass run once per group of images, not once per channel
+    int img_batch, slots;
     int cols12_ok;
     alignas(64) unsigned char cols12_tmap[128];
     alignas(64) unsigned char cols12_tmap_sw[128];   // same view, 32-byte swizzle (k_cols12_wcorrect)
@@ -173,11 +176,11 @@ int rick_cols2_perm(const rick_plan_t* p);   // log2(N/16) when rick_fft_cols2 a
 int rick_cols12_init(rick_plan_t* p);                                    // fft_cols12.cu
 int rick_cols12_fft(rick_plan_t* p, int n_planes);                       // fft_cols12.cu
 int rick_cols12_wcorrect(rick_plan_t* p, int img, int z_first, int n_planes, double* image,
-                         int accumulate, int fuse_taper, int strip_begin, int strip_end);   // fft_cols12.cu
+                         int accumulate, int fuse_taper, int strip_begin, int strip_end, int slot_first = 0);   // fft_cols12.cu
 int rick_cols12_strips(void);                                            // fft_cols12.cu
 // row_perm: 0 = planes in natural row order; else log2(N/16), the row order rick_fft_cols2 leaves
 int rick_wcorrect(rick_plan_t* p, int img, int z_first, int n_planes, double* image,
-                  int accumulate, int fuse_taper, int row_perm = 0);   // wcorrect.cu
+                  int accumulate, int fuse_taper, int row_perm = 0, int slot_first = 0);   // wcorrect.cu
 int rick_taper_divide(rick_plan_t* p, double* image);                    // wcorrect.cu
 
 // ordered (monotone) encoding of doubles for atomicMin/atomicMax on u64

@@ -167,7 +167,7 @@ __device__ __forceinline__ void strip_fft_g(double2 (&v)[16], const RolesG& R, c
 __global__ void __launch_bounds__(C12_THREADS, 1)
 k_cols12_wcorrect(const __grid_constant__ CUtensorMap tmap, const double2* __restrict__ tw, int n_planes,
                   int z_first, double dl, const WRange* __restrict__ wr, double* __restrict__ image,
-                  int accumulate, const double* __restrict__ taper, int strip_begin, int strip_end)
+                  int accumulate, const double* __restrict__ taper, int strip_begin, int strip_end, int slot_first)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     // the swizzle pattern is a function of the shared-memory ADDRESS: staging on a 1024-byte boundary
@@ -196,7 +196,7 @@ k_cols12_wcorrect(const __grid_constant__ CUtensorMap tmap, const double2* __res
     int strip = strip_begin + (int)blockIdx.x;
     if (threadIdx.x == 0 && strip < strip_end) {
         mbar_arrive_expect_tx(full, C12_STAGE_BYTES);
-        tma_load_5d(stg, &tmap, full, 4 * strip, 0, 0, 0, n_planes - 1);
+        tma_load_5d(stg, &tmap, full, 4 * strip, 0, 0, 0, slot_first + n_planes - 1);
     }
     uint32_t parity = 0;
     const double dw = wr->dw;
@@ -227,7 +227,7 @@ k_cols12_wcorrect(const __grid_constant__ CUtensorMap tmap, const double2* __res
             const bool more = plane > 0 || strip + (int)gridDim.x < strip_end;
             double2 v[16];
             strip_fft_g(v, R, stg, ex, tw, full, empty, parity, more, &tmap, plane > 0 ? strip : strip + (int)gridDim.x,
-                        plane > 0 ? plane - 1 : n_planes - 1);
+                        slot_first + (plane > 0 ? plane - 1 : n_planes - 1));
             // Horner in z: S <- P_z + step S
             if (plane == n_planes - 1) {
 #pragma unroll
@@ -309,7 +309,7 @@ int rick_cols12_init(rick_plan_t* p)
     static_assert(sizeof(CUtensorMap) <= sizeof(p->cols12_tmap), "tensor map storage");
     const cuuint64_t rowB = (cuuint64_t)C12_N * 16;
     // dims: (re/im/column pair as doubles, hh, w, e, plane) with row = w + 16 hh + 256 e
-    const cuuint64_t dims[5] = {(cuuint64_t)2 * C12_N, 16, 16, 16, (cuuint64_t)p->batch};
+    const cuuint64_t dims[5] = {(cuuint64_t)2 * C12_N, 16, 16, 16, (cuuint64_t)p->slots};
     const cuuint64_t strides[4] = {16 * rowB, rowB, 256 * rowB, (cuuint64_t)C12_N * rowB};
     const cuuint32_t box[5] = {4, 16, 16, 16, 1};
     const cuuint32_t es[5] = {1, 1, 1, 1, 1};
@@ -347,14 +347,14 @@ int rick_cols12_fft(rick_plan_t* p, int n_planes)
 // number of rounds of the persistent grid) so that the device -> host copy of one part runs under the
 // next part's kernel.
 int rick_cols12_wcorrect(rick_plan_t* p, int img, int z_first, int n_planes, double* image, int accumulate,
-                         int fuse_taper, int strip_begin, int strip_end)
+                         int fuse_taper, int strip_begin, int strip_end, int slot_first)
 {
     if (strip_end <= strip_begin) return RICK_OK;
     const CUtensorMap tm = *reinterpret_cast<const CUtensorMap*>(p->cols12_tmap_sw);
     const int n = strip_end - strip_begin;
     RICK_KERNEL(p, RK_COLS_WCORRECT, k_cols12_wcorrect<<<n < p->n_sm ? n : p->n_sm, C12_THREADS, C12_SMEM, p->stream>>>(
         tm, (const double2*)p->twiddle, n_planes, z_first, p->dl, p->wrange + img, image, accumulate,
-        fuse_taper ? p->taper : nullptr, strip_begin, strip_end));
+        fuse_taper ? p->taper : nullptr, strip_begin, strip_end, slot_first));
     return RICK_OK;
 }
 

@@ -117,12 +117,12 @@ static int plan_init(rick_plan_t* p)
     RICK_CUDA(p, cudaDeviceGetAttribute(&p->n_sm, cudaDevAttrMultiProcessorCount, dev));
     const size_t cell = p->f32 ? 8 : 16;
     p->plane_bytes = (size_t)p->N * p->N * cell;
-    RICK_CUDA(p, cudaMalloc(&p->stack, p->plane_bytes * (size_t)p->batch));
+    RICK_CUDA(p, cudaMalloc(&p->stack, p->plane_bytes * (size_t)p->slots));
     // the resident stack starts all-zero and no row is dirty: from here on only rows that were written
     // are ever cleared again (rick_zero_dirty)
-    RICK_CUDA(p, cudaMemsetAsync(p->stack, 0, p->plane_bytes * (size_t)p->batch, p->stream));
-    RICK_CUDA(p, cudaMalloc(&p->row_dirty, (size_t)p->batch * p->N));
-    RICK_CUDA(p, cudaMemsetAsync(p->row_dirty, 0, (size_t)p->batch * p->N, p->stream));
+    RICK_CUDA(p, cudaMemsetAsync(p->stack, 0, p->plane_bytes * (size_t)p->slots, p->stream));
+    RICK_CUDA(p, cudaMalloc(&p->row_dirty, (size_t)p->slots * p->N));
+    RICK_CUDA(p, cudaMemsetAsync(p->row_dirty, 0, (size_t)p->slots * p->N, p->stream));
     RICK_CUDA(p, cudaMalloc(&p->image, sizeof(double) * (size_t)p->N * p->N));
     RICK_CUDA(p, cudaMallocHost(&p->h_scale, sizeof(double) * RICK_MAX_CHAN));
     RICK_CUDA(p, cudaEventCreateWithFlags(&p->ev_scale, cudaEventDisableTiming));
@@ -185,6 +185,14 @@ extern "C" int rick_plan(rick_plan_t** out, const rick_plan_desc* d, void* cuda_
     while ((1 << p->log2B) < B) p->log2B++;
     p->f32 = d->grid_prec == RICK_GRID_F32;
     p->batch = d->plane_batch ? d->plane_batch : d->n_wplanes;
+    // cube with every plane of an image resident: keep up to 8 images' stacks (at most 48 GB) resident
+    p->img_batch = 1;
+    if (d->cube && p->batch == p->Nw) {
+        const double img_bytes = (double)d->n * d->n * (p->f32 ? 8.0 : 16.0) * (double)p->Nw;
+        int k = (int)(48.0e9 / img_bytes);
+        p->img_batch = k < 1 ? 1 : (k > 8 ? 8 : k);
+    }
+    p->slots = p->batch * p->img_batch;
     p->beta = d->kb_beta > 0.0 ? d->kb_beta : 2.34 * (double)d->support;
     p->dl = d->pixel_rad;
     p->inv_du = (double)d->n * d->pixel_rad;
@@ -420,6 +428,30 @@ static int image_impl(rick_plan_t* p, const void* vis, int32_t vis_dtype, const 
     if (vis_ready) RICK_CUDA(p, cudaStreamWaitEvent(p->stream, vis_ready, 0));
     const size_t NN = (size_t)p->N * p->N;
     bool host_done = false;
+    if (p->d.cube && p->img_batch > 1) {
+        // groups of img_batch images: one zero-fill, one gridder launch and one row pass per group (a
+        // channel's 5e5 visibilities are too few to fill the machine), the column pass + correction per image
+        const int perm = rick_cols2_perm(p);
+        for (int img0 = 0; img0 < p->n_img; img0 += p->img_batch) {
+            const int kk = p->n_img - img0 < p->img_batch ? p->n_img - img0 : p->img_batch;
+            const int pf = img0 * p->Nw, ns = kk * p->Nw;
+            if ((rc = rick_zero_sparse(p, pf, ns, !p->cols12_ok && perm != 0))) return rc;
+            if ((rc = rick_mark_dirty(p, pf, ns))) return rc;
+            if ((rc = rick_grid_planes(p, vis, vis_dtype, uvw_m, weights, pf, ns))) return rc;
+            if ((rc = rick_fft_rows(p, pf, ns))) return rc;
+            if (!p->cols12_ok) {
+                if (perm) rc = rick_fft_cols2(p, pf, ns);
+                else rc = rick_fft_cols(p, ns);
+                if (rc) return rc;
+            }
+            for (int j = 0; j < kk; ++j) {
+                double* dst = image_out + (size_t)(img0 + j) * NN;
+                if (p->cols12_ok) rc = rick_cols12_wcorrect(p, img0 + j, 0, p->Nw, dst, 0, 1, 0, rick_cols12_strips(), j * p->Nw);
+                else rc = rick_wcorrect(p, img0 + j, 0, p->Nw, dst, 0, 1, perm, j * p->Nw);
+                if (rc) return rc;
+            }
+        }
+    } else
     for (int img = 0; img < p->n_img; ++img) {
         double* dst = p->d.cube ? image_out + (size_t)img * NN : p->image;
         for (int z0 = 0; z0 < p->Nw; z0 += p->batch) {

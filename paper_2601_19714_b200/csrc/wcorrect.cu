@@ -73,17 +73,17 @@ k_taper_divide(double* __restrict__ image, int N, const double* __restrict__ tap
 }
 
 int rick_wcorrect(rick_plan_t* p, int img, int z_first, int n_planes, double* image, int accumulate,
-                  int fuse_taper, int row_perm)
+                  int fuse_taper, int row_perm, int slot_first)
 {
     const size_t NN = (size_t)p->N * p->N;
     const unsigned int blocks = (unsigned int)((NN + 255) / 256);
     const double* tp = fuse_taper ? p->taper : nullptr;
     if (p->f32) {
         RICK_KERNEL(p, RK_WCORRECT, k_wcorrect<float2><<<blocks, 256, 0, p->stream>>>(
-            (const float2*)p->stack, n_planes, z_first, p->N, p->dl, p->wrange + img, image, accumulate, tp, row_perm));
+            (const float2*)p->stack + (size_t)slot_first * p->N * p->N, n_planes, z_first, p->N, p->dl, p->wrange + img, image, accumulate, tp, row_perm));
     } else {
         RICK_KERNEL(p, RK_WCORRECT, k_wcorrect<double2><<<blocks, 256, 0, p->stream>>>(
-            (const double2*)p->stack, n_planes, z_first, p->N, p->dl, p->wrange + img, image, accumulate, tp, row_perm));
+            (const double2*)p->stack + (size_t)slot_first * p->N * p->N, n_planes, z_first, p->N, p->dl, p->wrange + img, image, accumulate, tp, row_perm));
     }
     return RICK_OK;
 }
