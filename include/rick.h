@@ -161,7 +161,8 @@ const char* rick_last_error(const rick_plan_t* p);
 const uint64_t* rick_debug_items(rick_plan_t* p, int32_t sorted, int32_t* idx_bits, int32_t* key_bits);
 void*           rick_debug_planes(rick_plan_t* p); /* [N_w][N][N] complex of grid_prec; meaningful after the
                                                     * STAGED calls only: rick_image leaves the stack
-                                                    * untransformed (N = 4096 fp64) or row-permuted (N >= 8192) */
+                                                    * half-transformed (rows only at N = 4096 fp64, rows + the
+                                                    * first column pass at N >= 8192) */
 
 /* Per-kernel timing with CUDA events on the plan's stream (for roofline reporting).
  * rick_profile(p, 1) clears the records and brackets every later kernel launch with a

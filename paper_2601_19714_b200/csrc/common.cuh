@@ -169,18 +169,21 @@ int rick_grid_planes(rick_plan_t* p, const void* vis, int vis_dtype, const doubl
 int rick_fft_planes(rick_plan_t* p, int plane_first, int n_planes);      // fft.cu: rows then columns (in place)
 int rick_fft_rows(rick_plan_t* p, int plane_first, int n_planes);        // fft.cu: occupied rows only
 int rick_fft_cols(rick_plan_t* p, int n_planes);                         // fft.cu (generic strided pass)
-// fft.cu: column pass of rick_image for long columns (N >= 8192) as two passes at full line width; leaves the
-// rows of every plane PERMUTED: memory row 16 (q mod N/16) + q / (N/16) holds pixel row q (rick_cols2_perm)
+// fft.cu: column pass of rick_image for long columns (N >= 8192, rick_cols2_perm != 0) in two passes at full line
+// width: rick_fft_cols2 = pass A (strided N/16-point transforms + twiddles, in place; reads occupied rows only,
+// writes every row), rick_cols2_wcorrect = pass B (16-point transforms in registers) fused with a5 (+ a6):
+// the transformed planes are never written
 int rick_fft_cols2(rick_plan_t* p, int plane_first, int n_planes);
-int rick_cols2_perm(const rick_plan_t* p);   // log2(N/16) when rick_fft_cols2 applies to this plan, else 0
+int rick_cols2_perm(const rick_plan_t* p);   // log2(N/16) when the two-pass transform applies to this plan, else 0
+int rick_cols2_wcorrect(rick_plan_t* p, int img, int z_first, int n_planes, double* image, int accumulate,
+                        int fuse_taper, int slot_first = 0);
 int rick_cols12_init(rick_plan_t* p);                                    // fft_cols12.cu
 int rick_cols12_fft(rick_plan_t* p, int n_planes);                       // fft_cols12.cu
 int rick_cols12_wcorrect(rick_plan_t* p, int img, int z_first, int n_planes, double* image,
                          int accumulate, int fuse_taper, int strip_begin, int strip_end, int slot_first = 0);   // fft_cols12.cu
 int rick_cols12_strips(void);                                            // fft_cols12.cu
-// row_perm: 0 = planes in natural row order; else log2(N/16), the row order rick_fft_cols2 leaves
 int rick_wcorrect(rick_plan_t* p, int img, int z_first, int n_planes, double* image,
-                  int accumulate, int fuse_taper, int row_perm = 0, int slot_first = 0);   // wcorrect.cu
+                  int accumulate, int fuse_taper, int slot_first = 0);   // wcorrect.cu
 int rick_taper_divide(rick_plan_t* p, double* image);                    // wcorrect.cu
 
 // ordered (monotone) encoding of doubles for atomicMin/atomicMax on u64

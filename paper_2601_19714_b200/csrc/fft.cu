@@ -186,13 +186,12 @@ static int launch_fft(rick_plan_t* p, int plane_first, int n_planes, int which) 
 //   pass A (k_fft_cols_a): for each n1 the N2-point transform over rows n1 + 16 n2 of a strip of 8 columns
 //     (128-byte pieces in fp64, the same in-register Stockham core as the row pass), times W_N^(n1 m2), stored at
 //     row n1 + 16 m2;
-//   pass B (k_fft_cols_b): for each m2 one THREAD transforms the 16 consecutive rows 16 m2 + n1 of its column
-//     in registers (no exchange at all; a warp moves 512 contiguous bytes per row).
-// Six transfers of the stack instead of four, all at the copy rate.  The centring is the rotation by N2/2
-// in n2 (pass A input, e -> (e+8) mod 16) and by 8 in m1 (pass B output); pass B stores in place, so memory
-// row 16 m2 + s holds pixel row q = m2 + N2 s: the correction pass reads rows through that permutation
-// (rick_cols2_perm) and no pass ever un-permutes the planes.  The staged API keeps the single-pass kernel
-// (its planes are in natural order).
+//   pass B (k_cols_b_wcorrect, below): for each m2 one THREAD transforms the 16 consecutive rows 16 m2 + n1 of
+//     its column in registers (no exchange at all; lanes run along the columns), fused with the w-correction.
+// Pass A reads and writes the stack once more than a single pass would, at full line width; pass B replaces
+// the read of the correction pass.  The centring is the rotation by N2/2 in n2 (pass A input, e -> (e+8) mod
+// 16) and by 8 in m1 (pass B output).  The staged API keeps the single-pass kernel (its planes are complete
+// transforms in natural order).
 #ifndef C2_MINB
 #define C2_MINB 512
 #endif
@@ -247,40 +246,16 @@ k_fft_cols_a(typename cplx_of<T>::type* __restrict__ stack, const typename cplx_
     }
 }
 
-template <typename T, int LOG2N>
-__global__ void __launch_bounds__(256)
-k_fft_cols_b(typename cplx_of<T>::type* __restrict__ stack, size_t n_threads)
-{
-    typedef typename cplx_of<T>::type C;
-    constexpr int N = 1 << LOG2N, N2 = N / 16;
-    const size_t gid = (size_t)blockIdx.x * 256 + threadIdx.x;       // (plane, m2, column), column fastest
-    if (gid >= n_threads) return;
-    const int p = (int)(gid & (size_t)(N - 1));
-    const size_t rest = gid >> LOG2N;
-    const int m2 = (int)(rest & (size_t)(N2 - 1));
-    const size_t plane = rest >> (LOG2N - 4);
-    C* g = stack + plane * N * N + (size_t)(16 * m2) * N + p;
-    C b[16];
-#pragma unroll
-    for (int n1 = 0; n1 < 16; ++n1) b[n1] = g[(size_t)n1 * N];
-    fft16<T>(b);
-#pragma unroll
-    for (int m1 = 0; m1 < 16; ++m1) g[(size_t)((m1 + 8) & 15) * N] = b[leg_reg<16>(m1)];
-}
-
 template <typename T, int LOG2N> static int launch_cols2(rick_plan_t* p, int plane_first, int n_planes)
 {
     typedef typename cplx_of<T>::type C;
     typedef Col2Cfg<T, LOG2N> K;
-    const int rcd = rick_all_dirty(p, n_planes);       // both passes write every row of the slots
+    const int rcd = rick_all_dirty(p, n_planes);       // the pass writes every row of the slots
     if (rcd) return rcd;
     RICK_CUDA(p, cudaFuncSetAttribute(k_fft_cols_a<T, LOG2N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)K::SMEM));
     const unsigned int blocks_a = (unsigned int)((size_t)n_planes * (K::N / K::W) * 16);
     RICK_KERNEL(p, RK_FFT_COLS, k_fft_cols_a<T, LOG2N><<<blocks_a, K::THREADS, K::SMEM, p->stream>>>(
         (C*)p->stack, (const C*)p->twiddle2, (const C*)p->twiddle, p->row_occ + (size_t)plane_first * p->N));
-    const size_t n_threads = (size_t)n_planes * K::N2 * K::N;
-    RICK_KERNEL(p, RK_FFT_COLS, k_fft_cols_b<T, LOG2N><<<(unsigned int)((n_threads + 255) / 256), 256, 0, p->stream>>>(
-        (C*)p->stack, n_threads));
     return RICK_OK;
 }
 
@@ -333,3 +308,103 @@ static int fft_dispatch(rick_plan_t* p, int plane_first, int n_planes, int which
 int rick_fft_planes(rick_plan_t* p, int plane_first, int n_planes) { return fft_dispatch(p, plane_first, n_planes, 3); }
 int rick_fft_rows(rick_plan_t* p, int plane_first, int n_planes) { return fft_dispatch(p, plane_first, n_planes, 1); }
 int rick_fft_cols(rick_plan_t* p, int n_planes) { return fft_dispatch(p, 0, n_planes, 2); }
+
+// ------------------------------------------------------------------------------------------
+// Pass B of the long-column transform FUSED with a5 (+ a6): the 16-point transforms of pass B need no
+// exchange, so a thread can keep transforming the same 16 rows of its column plane after plane and sum the
+// planes with Horner's rule in z (S <- P_z + step S, step = exp(2 pi i dw (n-1)); Eq. 2) --
+// the transformed planes are never written and never read back: two transfers of the stack less.
+// Two threads (h = 0, 1) share one (column p, block m2): both transform the 16 rows, each keeps the 8
+// outputs of its half (pixel rows q = m2 + N2 (8 h + i)) -- 8 x (S, step) complex doubles fit the
+// register file next to the transform, 16 do not.  A warp = 16 consecutive columns x 2 halves.
+template <typename T, int LOG2N>
+__global__ void __launch_bounds__(256, 2)
+k_cols_b_wcorrect(const typename cplx_of<T>::type* __restrict__ stack, int n_planes, int z_first, double dl,
+                  const WRange* __restrict__ wr, double* __restrict__ image, int accumulate,
+                  const double* __restrict__ taper)
+{
+    typedef typename cplx_of<T>::type C;
+    constexpr int N = 1 << LOG2N, N2 = N / 16;
+    const size_t gid = (size_t)blockIdx.x * 256 + threadIdx.x;       // < N * N2 * 2 by construction of the grid
+    const int pl = (int)(gid & 15), h = (int)((gid >> 4) & 1);
+    const size_t rest = gid >> 5;
+    const int p = (int)(rest % (N / 16)) * 16 + pl, m2 = (int)(rest / (N / 16));
+    const double dw = wr->dw;
+    const double l = (double)(p - N / 2) * dl;
+    double2 S[8], st[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        const int q = m2 + N2 * (8 * h + i);
+        const double m = (double)(q - N / 2) * dl;
+        const double r2 = l * l + m * m;
+        double xs = 0.0;
+        if (r2 < 1.0) xs = dw * (-r2 / (1.0 + sqrt(1.0 - r2)));
+        xs -= rint(xs);
+        sincospi(2.0 * xs, &st[i].y, &st[i].x);
+        S[i].x = 0.0;
+        S[i].y = 0.0;
+    }
+    const C* g = stack + (size_t)(16 * m2) * N + p;
+    for (int plane = n_planes - 1; plane >= 0; --plane) {
+        const C* gp = g + (size_t)plane * N * N;
+        C b[16];
+#pragma unroll
+        for (int n1 = 0; n1 < 16; ++n1) b[n1] = gp[(size_t)n1 * N];
+        fft16<T>(b);
+        // memory slot s = (m1 + 8) & 15 holds pixel row m2 + N2 s: half h keeps outputs m1 = 8 (1 - h) + i
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            const C lo = b[leg_reg<16>(i)], hi = b[leg_reg<16>(8 + i)];
+            const double xr = (double)(h ? lo.x : hi.x), xi = (double)(h ? lo.y : hi.y);
+            const double2 s = S[i];
+            S[i].x = fma(st[i].x, s.x, fma(-st[i].y, s.y, xr));
+            S[i].y = fma(st[i].x, s.y, fma(st[i].y, s.x, xi));
+        }
+    }
+    const double w_first = wr->w_min + ((double)z_first + 0.5) * dw;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        const int q = m2 + N2 * (8 * h + i);
+        const double m = (double)(q - N / 2) * dl;
+        const double r2 = l * l + m * m;
+        double val = 0.0;
+        if (r2 < 1.0) {
+            double x0 = w_first * (-r2 / (1.0 + sqrt(1.0 - r2)));
+            x0 -= rint(x0);
+            double pr, pi;
+            sincospi(2.0 * x0, &pi, &pr);
+            val = pr * S[i].x - pi * S[i].y;
+        }
+        const size_t pix = (size_t)q * N + p;
+        if (accumulate) val += image[pix];
+        if (taper) val /= (taper[p] * taper[q]);
+        image[pix] = val;
+    }
+}
+
+template <typename T, int LOG2N>
+static int launch_cols_b_wcorrect(rick_plan_t* p, int img, int z_first, int n_planes, double* image, int accumulate,
+                                  int fuse_taper, int slot_first)
+{
+    typedef typename cplx_of<T>::type C;
+    constexpr int N = 1 << LOG2N;
+    const size_t n_threads = (size_t)N * (N / 16) * 2;
+    RICK_KERNEL(p, RK_WCORRECT, k_cols_b_wcorrect<T, LOG2N><<<(unsigned int)(n_threads / 256), 256, 0, p->stream>>>(
+        (const C*)p->stack + (size_t)slot_first * N * N, n_planes, z_first, p->dl, p->wrange + img, image, accumulate,
+        fuse_taper ? p->taper : nullptr));
+    return RICK_OK;
+}
+
+int rick_cols2_wcorrect(rick_plan_t* p, int img, int z_first, int n_planes, double* image, int accumulate,
+                        int fuse_taper, int slot_first)
+{
+    if (n_planes <= 0) return RICK_OK;
+    if (p->f32) {
+        if (p->log2N == 13) return launch_cols_b_wcorrect<float, 13>(p, img, z_first, n_planes, image, accumulate, fuse_taper, slot_first);
+        if (p->log2N == 14) return launch_cols_b_wcorrect<float, 14>(p, img, z_first, n_planes, image, accumulate, fuse_taper, slot_first);
+    } else if (p->log2N == 13) {
+        return launch_cols_b_wcorrect<double, 13>(p, img, z_first, n_planes, image, accumulate, fuse_taper, slot_first);
+    }
+    p->err = "two-pass column transform: grid edge not supported";
+    return RICK_ERR_INVALID;
+}

@@ -400,13 +400,14 @@ static int transform_and_correct(rick_plan_t* p, int img, int z0, int nb, double
         }
     } else {
         const int perm = rick_cols2_perm(p);
-        if (perm) {       // long columns: two passes at full line width, rows left permuted for the correction
+        if (perm) {       // long columns: pass A at full line width, pass B fused with the correction
             if ((rc = rick_fft_rows(p, img * p->Nw + z0, nb))) return rc;
             if ((rc = rick_fft_cols2(p, img * p->Nw + z0, nb))) return rc;
+            if ((rc = rick_cols2_wcorrect(p, img, z0, nb, dst, z0 > 0, last))) return rc;
         } else {
             if ((rc = rick_fft_planes(p, img * p->Nw + z0, nb))) return rc;
+            if ((rc = rick_wcorrect(p, img, z0, nb, dst, z0 > 0, last))) return rc;
         }
-        if ((rc = rick_wcorrect(p, img, z0, nb, dst, z0 > 0, last, perm))) return rc;
     }
     return RICK_OK;
 }
@@ -447,7 +448,8 @@ static int image_impl(rick_plan_t* p, const void* vis, int32_t vis_dtype, const 
             for (int j = 0; j < kk; ++j) {
                 double* dst = image_out + (size_t)(img0 + j) * NN;
                 if (p->cols12_ok) rc = rick_cols12_wcorrect(p, img0 + j, 0, p->Nw, dst, 0, 1, 0, rick_cols12_strips(), j * p->Nw);
-                else rc = rick_wcorrect(p, img0 + j, 0, p->Nw, dst, 0, 1, perm, j * p->Nw);
+                else if (perm) rc = rick_cols2_wcorrect(p, img0 + j, 0, p->Nw, dst, 0, 1, j * p->Nw);
+                else rc = rick_wcorrect(p, img0 + j, 0, p->Nw, dst, 0, 1, j * p->Nw);
                 if (rc) return rc;
             }
         }

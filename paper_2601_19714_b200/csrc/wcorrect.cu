@@ -15,7 +15,7 @@ template <typename C>
 __global__ void __launch_bounds__(256)
 k_wcorrect(const C* __restrict__ stack, int n_planes, int z_first, int N, double dl,
            const WRange* __restrict__ wr, double* __restrict__ image, int accumulate,
-           const double* __restrict__ taper, int row_perm)
+           const double* __restrict__ taper)
 {
     const size_t NN = (size_t)N * N;
     const size_t pix = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -33,9 +33,7 @@ k_wcorrect(const C* __restrict__ stack, int n_planes, int z_first, int N, double
         double pr, pi, sr, si;
         sincospi(2.0 * x0, &pi, &pr);
         sincospi(2.0 * xs, &si, &sr);
-        // after the two-pass column transform (fft.cu) pixel row q sits in memory row 16 (q mod N2) + q / N2
-        const size_t row = row_perm ? (((size_t)(q & ((1 << row_perm) - 1)) << 4) | (size_t)(q >> row_perm)) : (size_t)q;
-        const C* g = stack + row * N + p;
+        const C* g = stack + pix;
         int z = 0;
         for (; z + 4 <= n_planes; z += 4) {
             const C a0 = g[(size_t)(z + 0) * NN], a1 = g[(size_t)(z + 1) * NN];
@@ -73,17 +71,17 @@ k_taper_divide(double* __restrict__ image, int N, const double* __restrict__ tap
 }
 
 int rick_wcorrect(rick_plan_t* p, int img, int z_first, int n_planes, double* image, int accumulate,
-                  int fuse_taper, int row_perm, int slot_first)
+                  int fuse_taper, int slot_first)
 {
     const size_t NN = (size_t)p->N * p->N;
     const unsigned int blocks = (unsigned int)((NN + 255) / 256);
     const double* tp = fuse_taper ? p->taper : nullptr;
     if (p->f32) {
         RICK_KERNEL(p, RK_WCORRECT, k_wcorrect<float2><<<blocks, 256, 0, p->stream>>>(
-            (const float2*)p->stack + (size_t)slot_first * p->N * p->N, n_planes, z_first, p->N, p->dl, p->wrange + img, image, accumulate, tp, row_perm));
+            (const float2*)p->stack + (size_t)slot_first * p->N * p->N, n_planes, z_first, p->N, p->dl, p->wrange + img, image, accumulate, tp));
     } else {
         RICK_KERNEL(p, RK_WCORRECT, k_wcorrect<double2><<<blocks, 256, 0, p->stream>>>(
-            (const double2*)p->stack + (size_t)slot_first * p->N * p->N, n_planes, z_first, p->N, p->dl, p->wrange + img, image, accumulate, tp, row_perm));
+            (const double2*)p->stack + (size_t)slot_first * p->N * p->N, n_planes, z_first, p->N, p->dl, p->wrange + img, image, accumulate, tp));
     }
     return RICK_OK;
 }

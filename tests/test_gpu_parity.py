@@ -375,9 +375,9 @@ def test_stream_host_weights_fused_4096():
 
 @pytest.mark.parametrize("prec,pb,tol", [("f64", 0, TOL64), ("f64", 2, TOL64), ("f32", 0, TOL32)])
 def test_long_columns_two_pass(prec, pb, tol):
-    """N = 8192: rick_image transforms the columns in two passes (N = 16 x 512) and leaves the rows of the
-    planes permuted for the correction pass; whole image against the oracle, all planes resident and in
-    ragged batches 2 + 1 (accumulate path), fp64 and fp32 grid.  (N = 16384 fp32: tests/test_gpu_fullsize.py.)"""
+    """N = 8192: rick_image transforms the columns in two passes (N = 16 x 512), the second one fused with
+    the w-correction; whole image against the oracle, all planes resident and in ragged batches 2 + 1
+    (accumulate path), fp64 and fp32 grid.  (N = 16384 fp32: tests/test_gpu_fullsize.py.)"""
     rick = _rick()
     wl = synth.make_config(3, n_times=4, n_wplanes=3, n_src=6)
     assert wl.n == 8192
