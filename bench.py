@@ -30,6 +30,8 @@ def make_workload(args, device):
     kw = {}
     if args.small:
         kw = dict(n_times=32, n=1024, n_wplanes=8)
+    if args.grid:
+        kw["n"] = args.grid          # e.g. --config 2 --grid 8192: the paper's 8192^2 x 32-plane shape (context only)
     return synth.make_config(args.config, device=device, **kw)
 
 
@@ -63,6 +65,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=2)
     ap.add_argument("--small", action="store_true", help="scaled-down workload (debug only)")
+    ap.add_argument("--grid", type=int, default=0, help="override the grid edge N of the config (context runs only)")
     ap.add_argument("--cpu-frac", type=int, default=4, help="oracle sample: 1/frac of the workload")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
@@ -177,7 +180,7 @@ def main():
     # dram__bytes_read.sum + dram__bytes_write.sum per launch, from profiles/r1e_ncu_full.md (configs[1] only;
     # the row pass transforms occupied rows only, so its traffic is below its dense algorithmic bytes)
     traffic_ncu = {}
-    if args.config == 2 and not args.small:
+    if args.config == 2 and not args.small and not args.grid:
         traffic_ncu = {"fft_rows": 4.628e9, "fft_cols_wcorrect": 8.936e9, "grid": 0.781e9}
     if dom in alg_bytes:
         avg_ms = prof[dom][0] / prof[dom][1]
@@ -240,7 +243,7 @@ def main():
                 "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": "f64" if wl.grid_prec == "f64" else "f32",
                 "data": "synthetic",
-                "config": {"workload": WORKLOAD if not args.small and args.config == 2 else wl.name,
+                "config": {"workload": WORKLOAD if not args.small and not args.grid and args.config == 2 else wl.name,
                            "n_vis": wl.n_vis, "grid": wl.n, "w_planes": wl.n_wplanes, "support": wl.support,
                            "parallelism": f"replicas x{world}" if world > 1 else "single GPU",
                            "l2": "inputs larger than L2 (stack %.2f GB, visibilities %.0f MB); no flush needed"
