@@ -169,12 +169,12 @@ int rick_grid_planes(rick_plan_t* p, const void* vis, int vis_dtype, const doubl
 int rick_fft_planes(rick_plan_t* p, int plane_first, int n_planes);      // fft.cu: rows then columns (in place)
 int rick_fft_rows(rick_plan_t* p, int plane_first, int n_planes);        // fft.cu: occupied rows only
 int rick_fft_cols(rick_plan_t* p, int n_planes);                         // fft.cu (generic strided pass)
-// fft.cu: column pass of rick_image for long columns (N >= 8192, rick_cols2_perm != 0) in two passes at full line
+// fft.cu: column pass of rick_image for long columns (N >= 8192, rick_cols2_on) in two passes at full line
 // width: rick_fft_cols2 = pass A (strided N/16-point transforms + twiddles, in place; reads occupied rows only,
 // writes every row), rick_cols2_wcorrect = pass B (16-point transforms in registers) fused with a5 (+ a6):
 // the transformed planes are never written
 int rick_fft_cols2(rick_plan_t* p, int plane_first, int n_planes);
-int rick_cols2_perm(const rick_plan_t* p);   // log2(N/16) when the two-pass transform applies to this plan, else 0
+int rick_cols2_on(const rick_plan_t* p);     // 1 when the two-pass transform applies to this plan (N >= 8192)
 int rick_cols2_wcorrect(rick_plan_t* p, int img, int z_first, int n_planes, double* image, int accumulate,
                         int fuse_taper, int slot_first = 0);
 int rick_cols12_init(rick_plan_t* p);                                    // fft_cols12.cu

@@ -259,7 +259,7 @@ template <typename T, int LOG2N> static int launch_cols2(rick_plan_t* p, int pla
     return RICK_OK;
 }
 
-int rick_cols2_perm(const rick_plan_t* p) { return p->log2N >= 13 ? p->log2N - 4 : 0; }
+int rick_cols2_on(const rick_plan_t* p) { return p->log2N >= 13; }
 
 int rick_fft_cols2(rick_plan_t* p, int plane_first, int n_planes)
 {

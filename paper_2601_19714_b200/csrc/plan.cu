@@ -399,8 +399,8 @@ static int transform_and_correct(rick_plan_t* p, int img, int z0, int nb, double
             if ((rc = rick_cols12_wcorrect(p, img, z0, nb, dst, z0 > 0, last, 0, strips))) return rc;
         }
     } else {
-        const int perm = rick_cols2_perm(p);
-        if (perm) {       // long columns: pass A at full line width, pass B fused with the correction
+        const int two_pass = rick_cols2_on(p);
+        if (two_pass) {       // long columns: pass A at full line width, pass B fused with the correction
             if ((rc = rick_fft_rows(p, img * p->Nw + z0, nb))) return rc;
             if ((rc = rick_fft_cols2(p, img * p->Nw + z0, nb))) return rc;
             if ((rc = rick_cols2_wcorrect(p, img, z0, nb, dst, z0 > 0, last))) return rc;
@@ -432,23 +432,23 @@ static int image_impl(rick_plan_t* p, const void* vis, int32_t vis_dtype, const 
     if (p->d.cube && p->img_batch > 1) {
         // groups of img_batch images: one zero-fill, one gridder launch and one row pass per group (a
         // channel's 5e5 visibilities are too few to fill the machine), the column pass + correction per image
-        const int perm = rick_cols2_perm(p);
+        const int two_pass = rick_cols2_on(p);
         for (int img0 = 0; img0 < p->n_img; img0 += p->img_batch) {
             const int kk = p->n_img - img0 < p->img_batch ? p->n_img - img0 : p->img_batch;
             const int pf = img0 * p->Nw, ns = kk * p->Nw;
-            if ((rc = rick_zero_sparse(p, pf, ns, !p->cols12_ok && perm != 0))) return rc;
+            if ((rc = rick_zero_sparse(p, pf, ns, !p->cols12_ok && two_pass))) return rc;
             if ((rc = rick_mark_dirty(p, pf, ns))) return rc;
             if ((rc = rick_grid_planes(p, vis, vis_dtype, uvw_m, weights, pf, ns))) return rc;
             if ((rc = rick_fft_rows(p, pf, ns))) return rc;
             if (!p->cols12_ok) {
-                if (perm) rc = rick_fft_cols2(p, pf, ns);
+                if (two_pass) rc = rick_fft_cols2(p, pf, ns);
                 else rc = rick_fft_cols(p, ns);
                 if (rc) return rc;
             }
             for (int j = 0; j < kk; ++j) {
                 double* dst = image_out + (size_t)(img0 + j) * NN;
                 if (p->cols12_ok) rc = rick_cols12_wcorrect(p, img0 + j, 0, p->Nw, dst, 0, 1, 0, rick_cols12_strips(), j * p->Nw);
-                else if (perm) rc = rick_cols2_wcorrect(p, img0 + j, 0, p->Nw, dst, 0, 1, j * p->Nw);
+                else if (two_pass) rc = rick_cols2_wcorrect(p, img0 + j, 0, p->Nw, dst, 0, 1, j * p->Nw);
                 else rc = rick_wcorrect(p, img0 + j, 0, p->Nw, dst, 0, 1, j * p->Nw);
                 if (rc) return rc;
             }
@@ -460,7 +460,7 @@ static int image_impl(rick_plan_t* p, const void* vis, int32_t vis_dtype, const 
             const int nb = p->Nw - z0 < p->batch ? p->Nw - z0 : p->batch;
             const int last = z0 + nb >= p->Nw;
             // (the two-pass column transform reads occupied rows only: stale rows need no clearing)
-            if ((rc = rick_zero_sparse(p, img * p->Nw + z0, nb, !p->cols12_ok && rick_cols2_perm(p) != 0))) return rc;
+            if ((rc = rick_zero_sparse(p, img * p->Nw + z0, nb, !p->cols12_ok && rick_cols2_on(p)))) return rc;
             if ((rc = rick_mark_dirty(p, img * p->Nw + z0, nb))) return rc;
             if ((rc = rick_grid_planes(p, vis, vis_dtype, uvw_m, weights, img * p->Nw + z0, nb))) return rc;
             if ((rc = transform_and_correct(p, img, z0, nb, dst, last, host_out, &host_done))) return rc;

@@ -129,7 +129,7 @@ int rick_tables_build(rick_plan_t* p)
     } else {
         RICK_KERNEL(p, RK_TABLES, k_twiddle<double2><<<(N + 255) / 256, 256, 0, p->stream>>>((double2*)p->twiddle, N));
     }
-    if (rick_cols2_perm(p)) {      // table of the length-N/16 sub-transforms of the two-pass column pass
+    if (rick_cols2_on(p)) {      // table of the length-N/16 sub-transforms of the two-pass column pass
         const int N2 = N / 16;
         RICK_CUDA(p, cudaMalloc(&p->twiddle2, (p->f32 ? sizeof(float2) : sizeof(double2)) * (size_t)N2));
         if (p->f32) {
