@@ -393,3 +393,53 @@ def test_long_columns_two_pass(prec, pb, tol):
     print(f"N=8192 two-pass columns {prec} plane_batch={pb}: rel L2 {e:.2e}")
     assert e <= tol and _rel(img2, o["image"]) <= tol
     assert st["n_gridded"] == o["stats"]["n_gridded"]
+
+
+def test_randomized_parameter_sweep():
+    """Seeded sweep over what the fixed cases do not combine: support 3..11, sort tile 8/16/32, grid edge
+    64..2048, fp64 / fp32 grid, cube, ragged plane batches, weights, complex64 / complex128, and the chunked
+    host entry -- every case against the oracle (twice through the same plan: stale rows, dirty flags).
+    fp32 grid with S = 11 is left out: the taper is not clamped (R12) and at S = 11 its corner value
+    (~1e-8 of the centre) amplifies the fp32 rounding of the planes to ~3e-4 of the image norm."""
+    import torch
+    rick = _rick()
+    rng = np.random.default_rng(20260119)
+    for case in range(16):
+        cfg = int(rng.choice([1, 2, 3, 5]))
+        n = int(rng.choice([64, 128, 256, 512, 1024, 2048]))
+        if cfg in (2, 5) and n < 256:
+            n = 256
+        nw = int(rng.integers(1, 8))
+        prec = str(rng.choice(["f64", "f64", "f32"]))
+        S = int(rng.choice([3, 5, 7, 9, 11] if prec == "f64" else [3, 5, 7, 9]))
+        B = int(rng.choice([0, 8, 16, 32]))
+        if B > n:
+            B = 0
+        cube = 1 if cfg == 5 else 0
+        pb = 0 if (cube and rng.random() < 0.7) else int(rng.integers(0, nw + 1))
+        wl = synth.make_config(cfg, n_times=int(rng.integers(1, 6)), n=n,
+                               n_chan=int(rng.integers(1, 5)) if cfg != 1 else None, n_wplanes=nw, n_src=4,
+                               with_weights=bool(rng.random() < 0.4), seed=int(rng.integers(1, 1 << 30)))
+        wl.support, wl.grid_prec, wl.plane_batch = S, prec, pb
+        if rng.random() < 0.3 and wl.vis.dtype == np.complex64:
+            wl.vis = wl.vis.astype(np.complex128)
+        desc = f"cfg{cfg} N={n} Nw={nw} S={S} B={B} {prec} cube={cube} batch={pb} {wl.vis.dtype} M={wl.n_vis}"
+        o = oracle.image(wl.uvw_m, wl.freq_hz, wl.vis, wl.weights, wl.n, wl.n_wplanes, S, wl.pixel_rad,
+                         B=(B or 16), cube=cube)
+        plan = rick.plan_from_workload(wl, tile=B)
+        vis, uvw, wgt = rick.to_device(wl)
+        outs = [plan.rick_image(vis, uvw, wgt, wl.freq_hz).cpu().numpy() for _ in range(2)]
+        st = plan.rick_get_stats()
+        if not cube and pb in (0, nw):
+            hv = torch.from_numpy(np.ascontiguousarray(wl.vis)).pin_memory()
+            hu = torch.from_numpy(wl.uvw_m).pin_memory()
+            hw = None if wl.weights is None else torch.from_numpy(wl.weights).pin_memory()
+            ho = torch.empty((n, n), dtype=torch.float64).pin_memory()
+            plan.rick_image_stream_host(hv, hu, hw, wl.freq_hz, ho, max(1, wl.n_rows // 3 + 1))
+            outs.append(ho.numpy().copy())
+        plan.destroy()
+        tol = TOL64 if prec == "f64" else TOL32
+        errs = [_rel(x.reshape(o["image"].shape), o["image"]) for x in outs]
+        print(desc, " ".join(f"{e:.1e}" for e in errs))
+        assert all(e <= tol for e in errs), desc
+        assert st["n_gridded"] == o["stats"]["n_gridded"], desc
