@@ -10,16 +10,16 @@
 // owns a PRIVATE shared-memory accumulation tile of (B+S-1)^2 cells -- the tile plus the kernel
 // halo, the single-GPU analogue of the paper's ghost region.  Per batch of 32 visibilities every
 // lane evaluates the 2S kernel values of its own visibility and stages them in shared memory
-// (the v-axis values already multiplied by w V); then the warp walks the 32 visibilities one by one
-// with its lanes spread over the footprint, each lane owning two horizontally adjacent cells.
-//   * Run accumulation: consecutive visibilities of the SAME centre cell have the same footprint,
-//     so their contributions are summed in REGISTERS (4 DFMA per lane per visibility, operands by
-//     two broadcast LDS.128); the shared-memory tile is read-modified-written once per run, when
-//     the centre cell changes (core-dense uv coverage: 5.5 visibilities per run in config 2).
-//     Before, every visibility paid the 2 x 49-cell RMW and the gridder ran at the shared-memory
-//     bandwidth.
+// (the u-axis values already multiplied by w V); then the warp walks the batch run by run.
+//   * Run accumulation: consecutive visibilities of the SAME centre cell (reading R22; 5.5 per run in
+//     config 2) share one footprint, and their sum is sum_k g_v(k) (x) [g_u(k) wV_re(k), g_u(k) wV_im(k)]:
+//     an (S x K)(K x 2S) product over the K visibilities of the run.  The warp accumulates it as rank-4
+//     updates with the fp64 mma.sync m8n8k4 (fragment rows = footprint rows, fragment columns =
+//     (footprint column, re | im): a lane's two accumulators are the (re, im) of one cell).  The
+//     accumulators are loaded from the tile when a run starts and stored back when it ends: the
+//     shared-memory tile is read-modified-written once per run, not once per visibility.
 //   * When the tile changes, the tile is flushed to HBM with fire-and-forget RED atomics
-//     (non-zero cells only) and re-zeroed.
+//     (non-zero cells only, scanned linearly with four cells per lane in flight) and re-zeroed.
 //
 // Kernel values.  d_a = (a-h) - delta with delta = x_u - (i_u - N/2) in [-1/2, 1/2): tap a sees g
 // only on one unit interval, where it is a degree-KB_DEG polynomial f_a(s), s = 2 delta, to < 2e-16
