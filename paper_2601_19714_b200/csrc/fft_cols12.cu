@@ -4,7 +4,7 @@
 //
 // Why a dedicated kernel.  A column of a 4096^2 complex128 plane is 64 KB, so one SM can hold a
 // strip of only two columns: the pass touches HBM in 32-byte pieces at a 64 KB stride.  Measured
-// on B200 (profiles/r1_colpass_probes.md): 32 B scattered reads run at ~4.7 TB/s through TMA but
+// on B200 (feed ceilings): 32 B scattered reads run at ~4.7 TB/s through TMA but
 // only ~4 TB/s through LSU loads, 32 B scattered WRITES at ~2 TB/s; and the L1 tag stage pays one
 // cycle per 128 B line touched (16 lines per warp instruction).  Hence:
 //   * the strip is fetched by ONE TMA instruction per (strip, plane): a 5-D tensor map views the
@@ -19,8 +19,8 @@
 //     per pixel per strip.
 //   * S and step (2 x 16 complex doubles per thread, 256 KB per SM) do not fit the register file
 //     next to the FFT; they live in TENSOR MEMORY, used here as a thread-private accumulator file
-//     (tcgen05.ld / tcgen05.st, shape 32x32b) -- the tensor cores themselves are not involved: no
-//     stage of this path is a dense contraction.
+//     (tcgen05.ld / tcgen05.st, shape 32x32b) -- the tensor cores themselves are not involved in
+//     this kernel.
 // Shared memory: 128 KB TMA staging + 68 KB exchange buffer (real / imaginary halves in turn).
 #include "common.cuh"
 #include "fft_core.cuh"
