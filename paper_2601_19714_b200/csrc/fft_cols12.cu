@@ -156,12 +156,15 @@ __device__ __forceinline__ void strip_fft_g(double2 (&v)[16], const RolesG& R, c
     }
     parity ^= 1u;
     bfly16<double, C12_LOG2N, 0>(v, R.t1, tw);
+    // the base twiddles of stages 2 and 3 are fetched before the exchanges they follow
+    const double2 w1_s2 = tw[bfly16_tw_index<C12_LOG2N, 4>(R.t2)];
     named_bar_sync(1 + R.g, 256);                // the group's reads of the previous item's exchange are done
     xchg16_warp_grp(v, ex + (size_t)(threadIdx.x >> 5) * (2 * 16 * 17), R.wl, R.hh);
-    bfly16<double, C12_LOG2N, 4>(v, R.t2, tw);
+    bfly16<double, C12_LOG2N, 4>(v, R.t2, tw, &w1_s2);
+    const double2 w1_s3 = tw[bfly16_tw_index<C12_LOG2N, 8>(R.t2)];
     named_bar_sync(1 + R.g, 256);                // every warp of the group is done with its private region
     xchg16_grp(v, ex + (size_t)R.g * (C12_N + C12_N / 16), R.t2, 1 + R.g);
-    bfly16<double, C12_LOG2N, 8>(v, R.t2, tw);
+    bfly16<double, C12_LOG2N, 8>(v, R.t2, tw, &w1_s3);
 }
 
 __global__ void __launch_bounds__(C12_THREADS, 1)
@@ -238,6 +241,7 @@ k_cols12_wcorrect(const __grid_constant__ CUtensorMap tmap, const double2* __res
                     tmem_st16(tS + 16 * k, r);
                 }
             } else {
+                tmem_wait_st();      // the previous plane's stores of S (their latency ran under this item's transform)
 #pragma unroll
                 for (int k = 0; k < 4; ++k) {
                     uint32_t rs[16], rt[16];
@@ -259,9 +263,9 @@ k_cols12_wcorrect(const __grid_constant__ CUtensorMap tmap, const double2* __res
                     tmem_st16(tS + 16 * k, rs);
                 }
             }
-            tmem_wait_st();
         }
         // I = Re(exp(2 pi i w_first (n-1)) S)  [+ previous batches]  [/ taper]
+        tmem_wait_st();
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
             uint32_t rs[16];

@@ -221,15 +221,23 @@ __device__ __forceinline__ void fft_thread(typename cplx_of<T>::type (&v)[16], c
 
 // twiddle (NS = 2^LOG2NS butterflies already combined) + radix-16 butterfly over v[e] = x[t + (N/16) e];
 // on exit v[r] = leg r in natural order.
+// index of the thread's base twiddle w1 of the stage with NS = 2^LOG2NS butterflies combined
+template <int LOG2N, int LOG2NS> __device__ __forceinline__ int bfly16_tw_index(const int t)
+{
+    constexpr int N = 1 << LOG2N, NS = 1 << LOG2NS;
+    return (t & (NS - 1)) * (N / (NS * 16));
+}
+
 template <typename T, int LOG2N, int LOG2NS>
 __device__ __forceinline__ void bfly16(typename cplx_of<T>::type (&v)[16], const int t,
-                                       const typename cplx_of<T>::type* __restrict__ tw)
+                                       const typename cplx_of<T>::type* __restrict__ tw,
+                                       const typename cplx_of<T>::type* w1_pre = nullptr)
 {
     typedef typename cplx_of<T>::type C;
-    constexpr int N = 1 << LOG2N, NS = 1 << LOG2NS;
     if constexpr (LOG2NS > 0) {
-        const int jm = t & (NS - 1);
-        const C w1 = tw[jm * (N / (NS * 16))];
+        // w1_pre: the base twiddle already fetched by the caller (before an exchange, whose barriers the
+        // load cannot be hoisted over)
+        const C w1 = w1_pre ? *w1_pre : tw[bfly16_tw_index<LOG2N, LOG2NS>(t)];
         v[1] = cmul(v[1], w1);
         const C w2 = cmul(w1, w1);
         const C w3 = cmul(w2, w1);
