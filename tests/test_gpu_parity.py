@@ -338,6 +338,12 @@ def test_stream_host_chunks(cfg1):
     plan.rick_image_stream_host(torch.from_numpy(few.vis).pin_memory(), torch.from_numpy(few.uvw_m).pin_memory(), None,
                                 few.freq_hz, out, 1)
     assert _rel(out.numpy(), of["image"]) <= TOL64
+    # an empty set gives an all-zero image and zero counts
+    ev = torch.empty((0, wl.n_chan), dtype=torch.complex128)
+    eu = torch.empty((0, 3), dtype=torch.float64)
+    out.fill_(float("nan"))
+    plan.rick_image_stream_host(ev, eu, None, wl.freq_hz, out, 5)
+    assert float(out.abs().max()) == 0.0 and plan.rick_get_stats()["n_gridded"] == 0
     # refused where the whole stack is not resident, and for a bad chunk size
     p2 = rick.Plan(256, 8, 7, wl.pixel_rad, plane_batch=2)
     with pytest.raises(rick.RickError) as ex:
