@@ -78,8 +78,10 @@ typedef struct {
 } rick_stats;
 
 /* Create a plan: validates `d`, allocates the plane stack
- * (min(plane_batch, N_w) * N*N complex of grid_prec), the image (N*N double, or the
- * caller's cube slice by slice), tables (FFT twiddles, taper, kernel coefficients)
+ * (min(plane_batch, N_w) * N*N complex of grid_prec; with cube = 1 and every plane of an
+ * image resident, the stacks of up to 8 channel images at once, 48 GB at most, so that one
+ * zero-fill, gridder launch and row pass serve a group of channels), the image (N*N double,
+ * or the caller's cube slice by slice), tables (FFT twiddles, taper, kernel coefficients)
  * -- the tables are computed by kernels on `cuda_stream` (a cudaStream_t, may be 0).
  * Returns RICK_ERR_INVALID (bad descriptor), RICK_ERR_CUDA (no device / CUDA
  * failure), RICK_ERR_OOM.  *out is NULL on failure. */
