@@ -452,6 +452,13 @@ static int image_impl(rick_plan_t* p, const void* vis, int32_t vis_dtype, const 
                 else rc = rick_wcorrect(p, img0 + j, 0, p->Nw, dst, 0, 1, j * p->Nw);
                 if (rc) return rc;
             }
+            if (host_out) {      // this group's images leave for the host while the next group is imaged
+                RICK_CUDA(p, cudaEventRecord(p->ev_part, p->stream));
+                RICK_CUDA(p, cudaStreamWaitEvent(p->stream3, p->ev_part, 0));
+                RICK_CUDA(p, cudaMemcpyAsync(host_out + (size_t)img0 * NN, image_out + (size_t)img0 * NN,
+                                             sizeof(double) * NN * (size_t)kk, cudaMemcpyDeviceToHost, p->stream3));
+                host_done = true;
+            }
         }
     } else
     for (int img = 0; img < p->n_img; ++img) {
