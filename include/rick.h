@@ -125,7 +125,7 @@ int rick_image(rick_plan_t* p, const void* vis, int32_t vis_dtype, const double*
 /* Same as rick_image with every buffer in HOST memory (pinned memory makes the copies
  * asynchronous): copies the inputs to plan-owned device staging, runs a0..a6, copies
  * the image back to image_out_host and SYNCHRONISES the stream before returning.  Sets of 2^22 or more
- * visibilities on a plan with plane_batch == N_w and cube == 0 are processed as
+ * visibilities on a plan with N <= 4096, plane_batch == N_w and cube == 0 are processed as
  * rick_image_stream_host with two chunks (same image up to summation order, same statistics). */
 int rick_image_host(rick_plan_t* p, const void* vis_host, int32_t vis_dtype, const double* uvw_m_host,
                     const float* weights_host, const double* chan_freq_hz, int32_t n_chan,
