@@ -176,7 +176,7 @@ int rick_fft_cols(rick_plan_t* p, int n_planes);                         // fft.
 int rick_fft_cols2(rick_plan_t* p, int plane_first, int n_planes);
 int rick_cols2_on(const rick_plan_t* p);     // 1 when the two-pass transform applies to this plan (N >= 8192)
 int rick_cols2_wcorrect(rick_plan_t* p, int img, int z_first, int n_planes, double* image, int accumulate,
-                        int fuse_taper, int slot_first = 0);
+                        int fuse_taper, int slot_first = 0, int col_begin = 0, int col_end = -1);   // columns [col_begin, col_end), multiples of 16; -1 = N
 int rick_cols12_init(rick_plan_t* p);                                    // fft_cols12.cu
 int rick_cols12_fft(rick_plan_t* p, int n_planes);                       // fft_cols12.cu
 int rick_cols12_wcorrect(rick_plan_t* p, int img, int z_first, int n_planes, double* image,

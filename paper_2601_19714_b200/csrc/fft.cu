@@ -321,14 +321,15 @@ template <typename T, int LOG2N>
 __global__ void __launch_bounds__(256, 2)
 k_cols_b_wcorrect(const typename cplx_of<T>::type* __restrict__ stack, int n_planes, int z_first, double dl,
                   const WRange* __restrict__ wr, double* __restrict__ image, int accumulate,
-                  const double* __restrict__ taper)
+                  const double* __restrict__ taper, int col_begin, int n_col16)
 {
     typedef typename cplx_of<T>::type C;
     constexpr int N = 1 << LOG2N, N2 = N / 16;
-    const size_t gid = (size_t)blockIdx.x * 256 + threadIdx.x;       // < N * N2 * 2 by construction of the grid
+    // columns col_begin .. col_begin + 16 n_col16 - 1 only (the host-buffer entry launches the pass in parts)
+    const size_t gid = (size_t)blockIdx.x * 256 + threadIdx.x;       // < 16 n_col16 * N2 * 2 by construction of the grid
     const int pl = (int)(gid & 15), h = (int)((gid >> 4) & 1);
     const size_t rest = gid >> 5;
-    const int p = (int)(rest % (N / 16)) * 16 + pl, m2 = (int)(rest / (N / 16));
+    const int p = col_begin + (int)(rest % (size_t)n_col16) * 16 + pl, m2 = (int)(rest / (size_t)n_col16);
     const double dw = wr->dw;
     const double l = (double)(p - N / 2) * dl;
     double2 S[8], st[8];
@@ -384,26 +385,29 @@ k_cols_b_wcorrect(const typename cplx_of<T>::type* __restrict__ stack, int n_pla
 
 template <typename T, int LOG2N>
 static int launch_cols_b_wcorrect(rick_plan_t* p, int img, int z_first, int n_planes, double* image, int accumulate,
-                                  int fuse_taper, int slot_first)
+                                  int fuse_taper, int slot_first, int col_begin, int col_end)
 {
     typedef typename cplx_of<T>::type C;
     constexpr int N = 1 << LOG2N;
-    const size_t n_threads = (size_t)N * (N / 16) * 2;
+    const int n_col16 = (col_end - col_begin) / 16;                   // both multiples of 16
+    if (n_col16 <= 0) return RICK_OK;
+    const size_t n_threads = (size_t)n_col16 * 16 * (N / 16) * 2;     // a multiple of 256
     RICK_KERNEL(p, RK_WCORRECT, k_cols_b_wcorrect<T, LOG2N><<<(unsigned int)(n_threads / 256), 256, 0, p->stream>>>(
         (const C*)p->stack + (size_t)slot_first * N * N, n_planes, z_first, p->dl, p->wrange + img, image, accumulate,
-        fuse_taper ? p->taper : nullptr));
+        fuse_taper ? p->taper : nullptr, col_begin, n_col16));
     return RICK_OK;
 }
 
 int rick_cols2_wcorrect(rick_plan_t* p, int img, int z_first, int n_planes, double* image, int accumulate,
-                        int fuse_taper, int slot_first)
+                        int fuse_taper, int slot_first, int col_begin, int col_end)
 {
     if (n_planes <= 0) return RICK_OK;
+    if (col_end < 0) col_end = p->N;
     if (p->f32) {
-        if (p->log2N == 13) return launch_cols_b_wcorrect<float, 13>(p, img, z_first, n_planes, image, accumulate, fuse_taper, slot_first);
-        if (p->log2N == 14) return launch_cols_b_wcorrect<float, 14>(p, img, z_first, n_planes, image, accumulate, fuse_taper, slot_first);
+        if (p->log2N == 13) return launch_cols_b_wcorrect<float, 13>(p, img, z_first, n_planes, image, accumulate, fuse_taper, slot_first, col_begin, col_end);
+        if (p->log2N == 14) return launch_cols_b_wcorrect<float, 14>(p, img, z_first, n_planes, image, accumulate, fuse_taper, slot_first, col_begin, col_end);
     } else if (p->log2N == 13) {
-        return launch_cols_b_wcorrect<double, 13>(p, img, z_first, n_planes, image, accumulate, fuse_taper, slot_first);
+        return launch_cols_b_wcorrect<double, 13>(p, img, z_first, n_planes, image, accumulate, fuse_taper, slot_first, col_begin, col_end);
     }
     p->err = "two-pass column transform: grid edge not supported";
     return RICK_ERR_INVALID;

@@ -403,7 +403,20 @@ static int transform_and_correct(rick_plan_t* p, int img, int z0, int nb, double
         if (two_pass) {       // long columns: pass A at full line width, pass B fused with the correction
             if ((rc = rick_fft_rows(p, img * p->Nw + z0, nb))) return rc;
             if ((rc = rick_fft_cols2(p, img * p->Nw + z0, nb))) return rc;
-            if ((rc = rick_cols2_wcorrect(p, img, z0, nb, dst, z0 > 0, last))) return rc;
+            if (host_out && last && !p->d.cube) {
+                // four column ranges: the image columns of one part cross to the host under the next part
+                const int step = p->N / 4;
+                for (int c0 = 0; c0 < p->N; c0 += step) {
+                    if ((rc = rick_cols2_wcorrect(p, img, z0, nb, dst, z0 > 0, last, 0, c0, c0 + step))) return rc;
+                    RICK_CUDA(p, cudaEventRecord(p->ev_part, p->stream));
+                    RICK_CUDA(p, cudaStreamWaitEvent(p->stream3, p->ev_part, 0));
+                    RICK_CUDA(p, cudaMemcpy2DAsync(host_out + c0, sizeof(double) * p->N, dst + c0, sizeof(double) * p->N,
+                                                   sizeof(double) * (size_t)step, (size_t)p->N, cudaMemcpyDeviceToHost, p->stream3));
+                }
+                *host_done = true;
+            } else {
+                if ((rc = rick_cols2_wcorrect(p, img, z0, nb, dst, z0 > 0, last))) return rc;
+            }
         } else {
             if ((rc = rick_fft_planes(p, img * p->Nw + z0, nb))) return rc;
             if ((rc = rick_wcorrect(p, img, z0, nb, dst, z0 > 0, last))) return rc;

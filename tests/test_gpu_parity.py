@@ -394,10 +394,16 @@ def test_long_columns_two_pass(prec, pb, tol):
     img = plan.rick_image(vis, uvw, wgt, wl.freq_hz).cpu().numpy()
     img2 = plan.rick_image(vis, uvw, wgt, wl.freq_hz).cpu().numpy()        # all rows dirty after the first call
     st = plan.rick_get_stats()
+    # host-buffer entry: the last pass runs in four column ranges, each copied out under the next
+    import torch
+    hv = torch.from_numpy(np.ascontiguousarray(wl.vis)).pin_memory()
+    hu = torch.from_numpy(wl.uvw_m).pin_memory()
+    hout = torch.full((wl.n, wl.n), float("nan"), dtype=torch.float64).pin_memory()
+    plan.rick_image_host(hv, hu, None, wl.freq_hz, hout)
     plan.destroy()
     e = _rel(img, o["image"])
-    print(f"N=8192 two-pass columns {prec} plane_batch={pb}: rel L2 {e:.2e}")
-    assert e <= tol and _rel(img2, o["image"]) <= tol
+    print(f"N=8192 two-pass columns {prec} plane_batch={pb}: rel L2 {e:.2e}, host entry {_rel(hout.numpy(), o['image']):.2e}")
+    assert e <= tol and _rel(img2, o["image"]) <= tol and _rel(hout.numpy(), o["image"]) <= tol
     assert st["n_gridded"] == o["stats"]["n_gridded"]
 
 
