@@ -182,11 +182,11 @@ def main():
     alg_bytes = {"fft_rows": 2 * stack_bytes, "fft_cols": 2 * stack_bytes, "zero": stack_bytes,
                  "wcorrect": stack_bytes + image_bytes, "fft_cols_wcorrect": stack_bytes + image_bytes}
     dom = max((k for k in prof if prof[k][1]), key=lambda k: prof[k][0])
-    # dram__bytes_read.sum + dram__bytes_write.sum per launch, from profiles/r1e_ncu_full.md (configs[1] only;
+    # dram__bytes_read.sum + dram__bytes_write.sum per launch, from profiles/r1f_ncu_full.md (configs[1] only;
     # the row pass transforms occupied rows only, so its traffic is below its dense algorithmic bytes)
     traffic_ncu = {}
     if args.config == 2 and not args.small and not args.grid:
-        traffic_ncu = {"fft_rows": 4.628e9, "fft_cols_wcorrect": 8.936e9, "grid": 0.781e9}
+        traffic_ncu = {"fft_rows": 4.629e9, "fft_cols_wcorrect": 8.925e9, "grid": 0.781e9}
     if dom in alg_bytes:
         avg_ms = prof[dom][0] / prof[dom][1]
         ach = alg_bytes[dom] / (avg_ms * 1e-3) / 1e9
