@@ -117,7 +117,14 @@ static int plan_init(rick_plan_t* p)
     RICK_CUDA(p, cudaDeviceGetAttribute(&p->n_sm, cudaDevAttrMultiProcessorCount, dev));
     const size_t cell = p->f32 ? 8 : 16;
     p->plane_bytes = (size_t)p->N * p->N * cell;
-    RICK_CUDA(p, cudaMalloc(&p->stack, p->plane_bytes * (size_t)p->slots));
+    if (p->img_batch > 1 && cudaMalloc(&p->stack, p->plane_bytes * (size_t)p->slots) != cudaSuccess) {
+        // no room for a group of images: fall back to one image's stack at a time
+        cudaGetLastError();
+        p->stack = nullptr;
+        p->img_batch = 1;
+        p->slots = p->batch;
+    }
+    if (!p->stack) RICK_CUDA(p, cudaMalloc(&p->stack, p->plane_bytes * (size_t)p->slots));
     // the resident stack starts all-zero and no row is dirty: from here on only rows that were written
     // are ever cleared again (rick_zero_dirty)
     RICK_CUDA(p, cudaMemsetAsync(p->stack, 0, p->plane_bytes * (size_t)p->slots, p->stream));
