@@ -19,23 +19,29 @@
  * pixel p <-> l = (p - N/2) dl.
  *
  * Conventions
- *   Pointers: "device" = CUDA device memory of the current device, 16-byte aligned;
- *     "host" = ordinary host memory.  Said per argument.
+ *   Pointers: "device" = CUDA device memory of the current device, 16-byte aligned (checked:
+ *     RICK_ERR_INVALID otherwise -- the kernels use vector loads); "host" = ordinary host memory
+ *     (pinned memory makes the copies asynchronous).  Said per argument.
  *   Ownership: the caller owns every input and output buffer; the library borrows
  *     them until the work it enqueued on the plan's stream has completed and never
  *     frees them.  The plan owns sort items, plane stack, image, tables and
  *     frees them in rick_plan_destroy.
  *   Stream: every call enqueues on the plan's stream and returns without
  *     synchronising, except rick_get_stats, rick_image_host and rick_plan_destroy.
- *   Errors: int return, 0 = RICK_OK, negative = error.  Nothing throws or aborts
- *     across the ABI.  Argument errors are detected before any work is enqueued.
- *     CUDA errors are sticky on the plan; rick_last_error gives the text.
+ *   Errors: int return, 0 = RICK_OK, negative = error.  Nothing throws, traps or aborts
+ *     across the ABI.  Argument errors (RICK_ERR_INVALID, RICK_ERR_STATE) are detected before
+ *     any work is enqueued and leave the plan usable; so does RICK_ERR_OOM (the scratch that
+ *     could not grow is re-grown by the next call).  A CUDA failure (RICK_ERR_CUDA: a failed
+ *     launch or copy, or the device-side failure flag of the radix sort, which the
+ *     synchronising calls read) is STICKY: every later call on that plan returns
+ *     RICK_ERR_CUDA until rick_plan_destroy; rick_last_error gives the text of the first failure.
  *   State machine: rick_grid -> rick_fft_wplanes -> rick_wcorrect_accumulate ->
  *     rick_gridcorrect; out of order returns RICK_ERR_STATE.  With
  *     plane_batch < n_wplanes or cube = 1 only rick_image / rick_image_host are
  *     valid (the staged calls need the whole stack of one image resident).
  *   Off-grid visibilities (footprint leaves the grid) are not an error: they are
- *     skipped and counted in n_dropped.
+ *     skipped and counted in n_dropped.  So are visibilities with a non-finite u, v or w
+ *     (reading R23); a non-finite w takes no part in the w range.
  *   Threading: a plan is not thread-safe; distinct plans are independent.
  *   There is no CPU fallback: without a CUDA device rick_plan returns RICK_ERR_CUDA.
  */
@@ -55,11 +61,18 @@ enum { RICK_GRID_F64 = 0, RICK_GRID_F32 = 1 };
 enum { RICK_VIS_C64 = 0, RICK_VIS_C128 = 1 };
 
 typedef struct {
-    int32_t n;           /* grid edge N: power of two, 64 <= N <= 16384 (8192 for F64)                        */
+    int32_t n;           /* grid edge N: power of two, 64 <= N <= 16384; <= 8192 for F64: one row or
+                          * column of the plane (N * 16 B) must fit one SM's shared memory, which is how
+                          * every 1-D pass reads and writes the stack exactly once                     */
     int32_t n_wplanes;   /* N_w >= 1                                                            */
-    int32_t support;     /* S, odd, 3..15 (Eq. 5: full kernel width in cells)                   */
+    int32_t support;     /* S, odd, 3..15 for F64, 3..9 for F32 (Eq. 5: full kernel width in cells; the
+                          * unclamped taper, reading R12, amplifies fp32 rounding beyond the 1e-4 bar
+                          * of the fp32 path from S = 11 on)                                    */
     double  pixel_rad;   /* dl, radians per pixel, > 0                                          */
-    double  kb_beta;     /* Kaiser-Bessel beta; <= 0 -> 2.34*S (reading R5)                     */
+    double  kb_beta;     /* Kaiser-Bessel beta; <= 0 -> 2.34*S (reading R5).  Accepted range: the taper
+                          * c(nu) must stay above 1e-12 c(0) on the N pixels (beta >~ pi S / 2 - 1; a
+                          * smaller beta puts a zero of c inside the image) and the per-tap polynomial
+                          * fit of the kernel must hold to 1e-14 (beta <~ 4 S, and <= 60)        */
     int32_t grid_prec;   /* RICK_GRID_F64 (complex double mesh) | RICK_GRID_F32   */
     int32_t tile;        /* uv-tile edge B in cells (power of two, 8..32); 0 -> 16              */
     int32_t plane_batch; /* w-planes resident at once; 0 -> all N_w                             */
@@ -71,10 +84,15 @@ typedef struct {
 typedef struct {
     int64_t n_vis;       /* M of the last rick_grid / rick_image                                */
     int64_t n_gridded;   /* on-grid visibilities                                                */
-    int64_t n_dropped;   /* off-grid visibilities (key = 0xFFFFFFFF)                            */
+    int64_t n_dropped;   /* off-grid visibilities, incl. non-finite u, v or w (key = all ones of key_bits) */
     double  sum_w;       /* sum of weights over gridded visibilities                            */
     double  w_min, w_max; /* of image 0 (wavelengths)                                           */
     int64_t n_launches;  /* kernels launched by this plan since creation                        */
+    int64_t occ_rows;    /* (plane, row) pairs some footprint reaches, of the last sort: the rows the
+                          * row pass transforms and writes, out of n_planes * N                  */
+    int64_t occ_tiles;   /* (plane, B x B tile) pairs some footprint reaches: what the zero-fill clears
+                          * and the row pass reads, out of n_planes * (N/B)^2                    */
+    int64_t n_planes;    /* planes of the last call: N_w, or C * N_w for a cube                 */
 } rick_stats;
 
 /* Create a plan: validates `d`, allocates the plane stack
@@ -84,7 +102,8 @@ typedef struct {
  * or the caller's cube slice by slice), tables (FFT twiddles, taper, kernel coefficients)
  * -- the tables are computed by kernels on `cuda_stream` (a cudaStream_t, may be 0).
  * Returns RICK_ERR_INVALID (bad descriptor), RICK_ERR_CUDA (no device / CUDA
- * failure), RICK_ERR_OOM.  *out is NULL on failure. */
+ * failure), RICK_ERR_OOM.  *out is NULL on failure.  A cube plan that cannot get the memory for a
+ * group of images falls back to one resident image (same results, more launches). */
 int rick_plan(rick_plan_t** out, const rick_plan_desc* d, void* cuda_stream);
 
 /* Synchronises the plan's stream and frees everything the plan owns. NULL is OK. */

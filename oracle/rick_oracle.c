@@ -149,10 +149,11 @@ int rko_index(int64_t n_rows, int32_t n_chan, const double *uvw_m, const double 
             for (int32_t c = 0; c < n_chan; ++c) {
                 if (cube && c != g) continue;
                 double wl = uvw_m[3 * r + 2] * s[c];
+                if (!isfinite(wl)) continue;   /* R23: a non-finite w takes no part in the range */
                 if (wl < lo) lo = wl;
                 if (wl > hi) hi = wl;
             }
-        if (n_rows == 0) { lo = 0.0; hi = 0.0; }
+        if (!(lo <= hi)) { lo = 0.0; hi = 0.0; }   /* no (finite) row at all */
         w_min[g] = lo;
         w_max[g] = hi;
     }
@@ -167,15 +168,21 @@ int rko_index(int64_t n_rows, int32_t n_chan, const double *uvw_m, const double 
             x_u = t * inv_du;
             t = uvw_m[3 * r + 1] * s[c];
             x_v = t * inv_du;
-            int32_t i_u = (int32_t)floor(x_u + shift);
-            int32_t i_v = (int32_t)floor(x_v + shift);
             const double dw = (w_max[img] - w_min[img]) / (double)Nw;
             const double inv_dw = dw > 0.0 ? 1.0 / dw : 0.0;
             double wl = uvw_m[3 * r + 2] * s[c];
-            int32_t i_p = (int32_t)floor((wl - w_min[img]) * inv_dw);
-            if (i_p > Nw - 1) i_p = Nw - 1;
-            if (i_p < 0) i_p = 0; /* only reachable with a caller-given w_min */
-            int on = (i_u - h >= 0) && (i_u + h <= N - 1) && (i_v - h >= 0) && (i_v + h <= N - 1);
+            /* R23: a visibility with a non-finite u, v or w cannot lie on the grid -> dropped
+             * (R10); coordinates beyond the int range likewise (the casts below stay defined). */
+            const double f_u = floor(x_u + shift), f_v = floor(x_v + shift);
+            const int fin = isfinite(x_u) && isfinite(x_v) && isfinite(wl) &&
+                            fabs(f_u) < 2147483000.0 && fabs(f_v) < 2147483000.0;
+            int32_t i_u = fin ? (int32_t)f_u : 0;
+            int32_t i_v = fin ? (int32_t)f_v : 0;
+            double f_p = fin ? floor((wl - w_min[img]) * inv_dw) : 0.0;
+            if (f_p > (double)(Nw - 1)) f_p = (double)(Nw - 1);
+            if (!(f_p >= 0.0)) f_p = 0.0; /* only reachable with a caller-given w_min */
+            int32_t i_p = (int32_t)f_p;
+            int on = fin && (i_u - h >= 0) && (i_u + h <= N - 1) && (i_v - h >= 0) && (i_v + h <= N - 1);
             iu[k] = i_u; iv[k] = i_v; ip[k] = i_p;
             if (xu) xu[k] = x_u;
             if (xv) xv[k] = x_v;

@@ -124,3 +124,73 @@ def aggregate_replicas(units_per_rank: float, ms_local: float, device="cpu") -> 
     total_units = dist_sum(units_per_rank, device)
     ms = dist_max(ms_local, device)
     return {"units": total_units, "ms": ms, "per_s": total_units / (ms * 1e-3)}
+
+
+def csrc_sha256(root: str) -> str:
+    """Hash of the kernel sources: ncu traffic figures in profiles/traffic.json are valid only for the
+    sources they were captured at."""
+    import hashlib
+    d = os.path.join(root, "paper_2601_19714_b200", "csrc")
+    h = hashlib.sha256()
+    for name in sorted(os.listdir(d)):
+        if name.endswith((".cu", ".cuh")):
+            with open(os.path.join(d, name), "rb") as f:
+                h.update(name.encode() + b"\0" + f.read())
+    return h.hexdigest()
+
+
+# ----------------------------------------------------------------------------------------------
+# cuFFT, timed as the GPU-side baseline of a4 (bench.py only; the library never links it)
+# ----------------------------------------------------------------------------------------------
+_CUFFT_Z2Z, _CUFFT_C2C, _CUFFT_INVERSE = 0x69, 0x29, 1
+
+
+def _load_cufft():
+    import ctypes
+    import glob
+    import torch
+    cands = glob.glob(os.path.join(os.path.dirname(torch.__file__), "..", "nvidia", "cufft", "lib", "libcufft.so*"))
+    cands += ["libcufft.so.11", "/usr/local/cuda/lib64/libcufft.so.11", "libcufft.so"]
+    err = None
+    for c in cands:
+        try:
+            return ctypes.CDLL(c)
+        except OSError as e:
+            err = e
+    raise RuntimeError(f"libcufft not found: {err}")
+
+
+def time_cufft_2d(n: int, batch: int, double: bool = True, reps: int = 3) -> float:
+    """Milliseconds of one in-place batched 2-D complex transform (cufftPlanMany, Z2Z or C2C, + sign) of
+    `batch` dense n x n planes, CUDA events on the current stream, best of `reps` after one warm-up."""
+    import ctypes as C
+    import torch
+    lib = _load_cufft()
+    plan = C.c_int(0)
+    dims = (C.c_int * 2)(n, n)
+    kind = _CUFFT_Z2Z if double else _CUFFT_C2C
+    rc = lib.cufftPlanMany(C.byref(plan), 2, dims, None, 1, 0, None, 1, 0, kind, batch)
+    if rc != 0:
+        raise RuntimeError(f"cufftPlanMany failed: {rc}")
+    try:
+        stream = torch.cuda.current_stream()
+        lib.cufftSetStream(plan, C.c_void_p(stream.cuda_stream))
+        buf = torch.zeros((batch, n, n), dtype=torch.complex128 if double else torch.complex64, device="cuda")
+        buf[:, n // 2 - 8:n // 2 + 8, n // 2 - 8:n // 2 + 8] = 1.0
+        fn = lib.cufftExecZ2Z if double else lib.cufftExecC2C
+        ptr = C.c_void_p(buf.data_ptr())
+        best = float("inf")
+        for i in range(reps + 1):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            rc = fn(plan, ptr, ptr, _CUFFT_INVERSE)
+            e1.record()
+            torch.cuda.synchronize()
+            if rc != 0:
+                raise RuntimeError(f"cufftExec failed: {rc}")
+            if i > 0:
+                best = min(best, e0.elapsed_time(e1))
+        del buf
+        return best
+    finally:
+        lib.cufftDestroy(plan)

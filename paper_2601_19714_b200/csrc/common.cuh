@@ -25,7 +25,7 @@ struct DevCounters {
     unsigned long long n_dropped;
     double sum_w;                   // sum of weights over gridded visibilities
     unsigned int grid_chunk;        // dynamic work counter of the gridder
-    unsigned int pad;
+    unsigned int error;             // sticky device-side failure flag (a radix tile lost its predecessor)
 };
 
 struct rick_plan_s {
@@ -37,9 +37,10 @@ struct rick_plan_s {
     cudaStream_t stream;
     cudaStream_t stream2;    // low-priority side stream: the zero-fill runs beside index + sort
     cudaStream_t stream3;    // copy stream of rick_image_host (visibilities in, image parts out)
-    cudaEvent_t ev_fork, ev_join, ev_vis, ev_part;
+    cudaEvent_t ev_fork, ev_join, ev_vis, ev_part, ev_wgt;
     int n_sm;
     int state;               // 0 idle, 1 gridded, 2 transformed, 3 corrected, 4 tapered
+    int failed;              // sticky: the first CUDA failure (RICK_ERR_CUDA); every later call returns it
     std::string err;
     int64_t n_launches;
 
@@ -117,7 +118,9 @@ struct rick_plan_s {
         cudaError_t e__ = (call);                                                      \
         if (e__ != cudaSuccess) {                                                      \
             (p)->err = std::string(#call) + ": " + cudaGetErrorString(e__);            \
-            return e__ == cudaErrorMemoryAllocation ? RICK_ERR_OOM : RICK_ERR_CUDA;    \
+            if (e__ == cudaErrorMemoryAllocation) { cudaGetLastError(); return RICK_ERR_OOM; } \
+            (p)->failed = RICK_ERR_CUDA;                                               \
+            return RICK_ERR_CUDA;                                                      \
         }                                                                              \
     } while (0)
 
@@ -145,6 +148,7 @@ void rick_prof_end(rick_plan_t* p, cudaStream_t st);
         cudaError_t e__ = cudaGetLastError();                                          \
         if (e__ != cudaSuccess) {                                                      \
             (p)->err = std::string("kernel launch: ") + cudaGetErrorString(e__);       \
+            (p)->failed = RICK_ERR_CUDA;                                               \
             return RICK_ERR_CUDA;                                                      \
         }                                                                              \
     } while (0)

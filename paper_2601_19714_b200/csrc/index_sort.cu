@@ -26,8 +26,7 @@ __global__ void k_counters_reset(DevCounters* c)
     c->n_gridded = 0ull;
     c->n_dropped = 0ull;
     c->sum_w = 0.0;
-    c->grid_chunk = 0u;
-    c->pad = 0u;
+    c->grid_chunk = 0u;      // (c->error is sticky: cleared at plan creation only)
 }
 
 __global__ void k_wrange_rows(const double* __restrict__ uvw, long long R, DevCounters* c)
@@ -35,7 +34,9 @@ __global__ void k_wrange_rows(const double* __restrict__ uvw, long long R, DevCo
     unsigned long long lo = 0xFFFFFFFFFFFFFFFFull, hi = 0ull;
     for (long long r = blockIdx.x * (long long)blockDim.x + threadIdx.x; r < R;
          r += (long long)gridDim.x * blockDim.x) {
-        unsigned long long e = rick_ord_encode(uvw[3 * r + 2]);
+        const double w = uvw[3 * r + 2];
+        if (!isfinite(w)) continue;                 // R23: a non-finite w takes no part in the range
+        unsigned long long e = rick_ord_encode(w);
         lo = e < lo ? e : lo;
         hi = e > hi ? e : hi;
     }
@@ -59,7 +60,7 @@ __global__ void k_wrange_finish(const DevCounters* c, const double* __restrict__
     const int n_img = cube ? C : 1;
     if (g >= n_img) return;
     double lo, hi;
-    if (R == 0) {
+    if (R == 0 || c->wmin_bits > c->wmax_bits) {     // no row, or none with a finite w
         lo = 0.0;
         hi = 0.0;
     } else {
@@ -126,14 +127,22 @@ k_index_key(const double* __restrict__ uvw, const float* __restrict__ wgt,
         const double um = uvw[3ull * r + 0], vm = uvw[3ull * r + 1], wm = uvw[3ull * r + 2];
         const double xu = __dmul_rn(__dmul_rn(um, s), inv_du);
         const double xv = __dmul_rn(__dmul_rn(vm, s), inv_du);
-        const int iu = (int)floor(__dadd_rn(xu, shift));
-        const int iv = (int)floor(__dadd_rn(xv, shift));
+        // on-grid test on the doubles, before any cast: floor(x) - h >= 0 <=> x >= h and
+        // floor(x) + h <= N-1 <=> x < N-h for integer h, and both are false for NaN / inf (R23: a
+        // visibility with a non-finite u, v or w is dropped; (int)floor() of such a value
+        // saturated and could pass the integer test)
+        const double su = __dadd_rn(xu, shift), sv = __dadd_rn(xv, shift);
+        const double wl = __dmul_rn(wm, s);
+        const double lo_ok = (double)h, hi_ok = (double)(N - h);
+        const bool ok = su >= lo_ok && su < hi_ok && sv >= lo_ok && sv < hi_ok && isfinite(wl);
+        const int iu = ok ? (int)floor(su) : 0;
+        const int iv = ok ? (int)floor(sv) : 0;
         const int img = cube ? (int)c : 0;
         const WRange wr = wrange[img];
-        int ip = (int)floor(__dmul_rn(__dsub_rn(__dmul_rn(wm, s), wr.w_min), wr.inv_dw));
-        ip = ip > Nw - 1 ? Nw - 1 : ip;
-        ip = ip < 0 ? 0 : ip;
-        const bool ok = (iu - h >= 0) && (iu + h <= N - 1) && (iv - h >= 0) && (iv + h <= N - 1);
+        double fp = ok ? floor(__dmul_rn(__dsub_rn(wl, wr.w_min), wr.inv_dw)) : 0.0;
+        fp = fp > (double)(Nw - 1) ? (double)(Nw - 1) : fp;
+        fp = fp >= 0.0 ? fp : 0.0;
+        const int ip = (int)fp;
         unsigned long long key = key_dropped;
         if (ok) {
             unsigned long long kk = (unsigned long long)img * (unsigned)Nw + (unsigned)ip;
@@ -241,7 +250,7 @@ __global__ void __launch_bounds__(256) k_digit_bases(const unsigned int* __restr
 __global__ void __launch_bounds__(RS_THREADS, RS_MINB)
 k_radix_onesweep(const u64* __restrict__ in, u64* __restrict__ out, unsigned int M, int shift, uint32_t mask,
                  int nbins, const unsigned long long* __restrict__ gbase, volatile unsigned long long* status,
-                 unsigned int* __restrict__ ticket)
+                 unsigned int* __restrict__ ticket, volatile unsigned int* dev_error)
 {
     __shared__ uint32_t cnt[RS_THREADS / 32][256];
     __shared__ u64 buf[RS_TILE];
@@ -323,9 +332,17 @@ k_radix_onesweep(const u64* __restrict__ in, u64* __restrict__ out, unsigned int
                         unsigned int spins = 0;
                         while ((v[j] >> 62) == 0ull) {
                             __nanosleep(40);
-                            if (++spins > (1u << 24)) __trap();      // a lost predecessor: fail loudly, never hang
+                            // a lost predecessor: never hang and never trap (a trap would poison the caller's
+                            // context across the ABI) -- raise the plan's device error flag, which the next
+                            // synchronising call turns into RICK_ERR_CUDA, and let every waiting tile drain
+                            if (++spins > (1u << 22) || ((spins & 255u) == 0u && *dev_error != 0u)) {
+                                *dev_error = 1u;
+                                done = true;
+                                break;
+                            }
                             v[j] = q[-256 * (long long)j];
                         }
+                        if (done) break;
                         excl += v[j] & OS_VAL;
                         if ((v[j] >> 62) == 2ull) done = true;
                     }
@@ -513,7 +530,7 @@ int rick_index_sort(rick_plan_t* p, const double* uvw_m, const float* weights, i
             u64* o = bufs[pass & 1];
             RICK_KERNEL(p, RK_RADIX_SCATTER, k_radix_onesweep<<<nblocks, RS_THREADS, 0, st>>>(
                 in, o, M, p->idx_bits + rp.shift[pass], rp.mask[pass], 1 << nb_bits[pass], p->os_gbase + pass * 256,
-                p->os_status + (size_t)pass * nblocks * 256, p->os_small + RS_MAXPASS * 256 + pass));
+                p->os_status + (size_t)pass * nblocks * 256, p->os_small + RS_MAXPASS * 256 + pass, &p->counters->error));
             in = o;
         }
         p->sorted_items = (unsigned long long*)in;

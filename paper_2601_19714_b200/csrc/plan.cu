@@ -9,6 +9,28 @@
 
 static bool is_pow2(int x) { return x > 0 && (x & (x - 1)) == 0; }
 
+// every entry point: a plan that has seen a CUDA failure stays failed (rick.h "Errors"); the text of the
+// first failure stays readable through rick_last_error
+#define RICK_ENTER(p)                                   \
+    do {                                                \
+        if (!(p)) return RICK_ERR_INVALID;              \
+        if ((p)->failed) return (p)->failed;            \
+        (p)->err.clear();                               \
+    } while (0)
+
+static bool aligned16(const void* q) { return (reinterpret_cast<uintptr_t>(q) & 15u) == 0; }
+
+// closed form of the taper (tables.cu k_taper) on the host, for the plan-time check of kb_beta
+static double taper_host(double nu, int S, double beta, double i0_beta)
+{
+    const double x = 3.14159265358979323846 * (double)S * nu, a = beta * beta - x * x;
+    double f;
+    if (fabs(a) < 1e-6) f = 1.0 + a / 6.0;
+    else if (a > 0.0) { const double r = sqrt(a); f = sinh(r) / r; }
+    else { const double r = sqrt(-a); f = sin(r) / r; }
+    return (double)S / i0_beta * f;
+}
+
 static void free_dev(void* q)
 {
     if (q) cudaFree(q);
@@ -102,6 +124,7 @@ extern "C" int rick_plan_destroy(rick_plan_t* p)
     if (p->stream3) { cudaStreamSynchronize(p->stream3); cudaStreamDestroy(p->stream3); }
     if (p->ev_vis) cudaEventDestroy(p->ev_vis);
     if (p->ev_part) cudaEventDestroy(p->ev_part);
+    if (p->ev_wgt) cudaEventDestroy(p->ev_wgt);
     for (int i = 0; i < 2; ++i) {
         if (p->ev_chunk_in[i]) cudaEventDestroy(p->ev_chunk_in[i]);
         if (p->ev_chunk_free[i]) cudaEventDestroy(p->ev_chunk_free[i]);
@@ -142,6 +165,7 @@ static int plan_init(rick_plan_t* p)
         RICK_CUDA(p, cudaStreamCreateWithFlags(&p->stream3, cudaStreamNonBlocking));
         RICK_CUDA(p, cudaEventCreateWithFlags(&p->ev_vis, cudaEventDisableTiming));
         RICK_CUDA(p, cudaEventCreateWithFlags(&p->ev_part, cudaEventDisableTiming));
+        RICK_CUDA(p, cudaEventCreateWithFlags(&p->ev_wgt, cudaEventDisableTiming));
         for (int i = 0; i < 2; ++i) {
             RICK_CUDA(p, cudaEventCreateWithFlags(&p->ev_chunk_in[i], cudaEventDisableTiming));
             RICK_CUDA(p, cudaEventCreateWithFlags(&p->ev_chunk_free[i], cudaEventDisableTiming));
@@ -173,6 +197,23 @@ extern "C" int rick_plan(rick_plan_t** out, const rick_plan_desc* d, void* cuda_
     if (isinf(d->w_min) || isinf(d->w_max)) return RICK_ERR_INVALID;
     if (d->w_min == d->w_min && d->w_max == d->w_max && d->w_max < d->w_min) return RICK_ERR_INVALID;
     if (d->kb_beta == d->kb_beta && d->kb_beta > 60.0) return RICK_ERR_INVALID;
+    // fp32 grid: the taper is not clamped (reading R12) and its corner value falls with S (S = 7: 3.8e-4 of
+    // the centre, S = 11: ~1e-8), so beyond S = 9 the fp32 rounding of the planes, amplified at the corners,
+    // exceeds the 1e-4 bar of the fp32 path (measured 3e-4 at S = 11): such plans are refused
+    if (d->grid_prec == RICK_GRID_F32 && d->support > 9) return RICK_ERR_INVALID;
+    {
+        // kb_beta too SMALL: for beta < pi S / 2 the taper c(nu) enters its sin(r)/r branch inside
+        // |nu| <= 1/2 and can cross zero, and a6 would divide by ~0.  Refuse a plan whose taper falls below
+        // 1e-12 of its centre value anywhere on the N pixels.
+        const double beta = d->kb_beta > 0.0 ? d->kb_beta : 2.34 * (double)d->support;
+        const double c0 = taper_host(0.0, d->support, beta, 1.0);
+        double cmin = c0;
+        for (int p = 0; p < d->n; ++p) {
+            const double c = taper_host((double)(p - d->n / 2) / (double)d->n, d->support, beta, 1.0);
+            if (!(c >= cmin)) cmin = c;
+        }
+        if (!(cmin > 1e-12 * c0)) return RICK_ERR_INVALID;
+    }
 
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return RICK_ERR_CUDA;   // no CPU fallback
@@ -228,8 +269,11 @@ static void item_bits(const rick_plan_t* p, int32_t n_chan, unsigned long long M
     *idx_bits = ib;
 }
 
+// dev_ptrs: the buffers are device memory the kernels read directly (alignment matters); dev_w / dev_out: the
+// optional weights and image_out of that call (may be null)
 static int check_inputs(rick_plan_t* p, const void* vis, int32_t vis_dtype, const double* uvw_m,
-                        const double* chan_freq_hz, int32_t n_chan, int64_t n_rows)
+                        const double* chan_freq_hz, int32_t n_chan, int64_t n_rows, bool dev_ptrs = false,
+                        const void* dev_w = nullptr, const void* dev_out = nullptr)
 {
     if (vis_dtype != RICK_VIS_C64 && vis_dtype != RICK_VIS_C128) { p->err = "bad vis_dtype"; return RICK_ERR_INVALID; }
     if (n_chan < 1 || n_chan > RICK_MAX_CHAN || !chan_freq_hz) { p->err = "bad channels"; return RICK_ERR_INVALID; }
@@ -237,6 +281,11 @@ static int check_inputs(rick_plan_t* p, const void* vis, int32_t vis_dtype, cons
     if (n_rows > 0 && (!vis || !uvw_m)) { p->err = "null input"; return RICK_ERR_INVALID; }
     for (int c = 0; c < n_chan; ++c)
         if (!(chan_freq_hz[c] > 0.0) || !isfinite(chan_freq_hz[c])) { p->err = "bad frequency"; return RICK_ERR_INVALID; }
+    // the kernels read vis with 8- / 16-byte vector loads: a misaligned pointer would fault the context
+    if (dev_ptrs && (!aligned16(vis) || !aligned16(uvw_m) || !aligned16(dev_w) || !aligned16(dev_out))) {
+        p->err = "device pointer not 16-byte aligned (vis / uvw_m / weights / image_out)";
+        return RICK_ERR_INVALID;
+    }
     const unsigned long long M = (unsigned long long)n_rows * (unsigned long long)n_chan;
     if (M >= 0xFFFFFFFFull) { p->err = "too many visibilities for 32-bit indices"; return RICK_ERR_INVALID; }
     int kb, ib;
@@ -328,10 +377,9 @@ static int sort_and_zero(rick_plan_t* p, const double* uvw_m, const float* weigh
 extern "C" int rick_grid(rick_plan_t* p, const void* vis, int32_t vis_dtype, const double* uvw_m,
                          const float* weights, const double* chan_freq_hz, int32_t n_chan, int64_t n_rows)
 {
-    if (!p) return RICK_ERR_INVALID;
-    p->err.clear();
+    RICK_ENTER(p);
     if (p->batch != p->Nw || p->d.cube) { p->err = "staged calls need the whole stack resident and cube = 0"; return RICK_ERR_STATE; }
-    int rc = check_inputs(p, vis, vis_dtype, uvw_m, chan_freq_hz, n_chan, n_rows);
+    int rc = check_inputs(p, vis, vis_dtype, uvw_m, chan_freq_hz, n_chan, n_rows, true, weights);
     if (rc) return rc;
     p->state = 0;
     if ((rc = prepare(p, chan_freq_hz, n_chan, n_rows))) return rc;
@@ -344,8 +392,7 @@ extern "C" int rick_grid(rick_plan_t* p, const void* vis, int32_t vis_dtype, con
 
 extern "C" int rick_fft_wplanes(rick_plan_t* p)
 {
-    if (!p) return RICK_ERR_INVALID;
-    p->err.clear();
+    RICK_ENTER(p);
     if (p->state != 1) { p->err = "rick_fft_wplanes needs a gridded stack"; return RICK_ERR_STATE; }
     const int rc = rick_fft_planes(p, 0, p->Nw);
     if (rc) return rc;
@@ -355,8 +402,7 @@ extern "C" int rick_fft_wplanes(rick_plan_t* p)
 
 extern "C" int rick_wcorrect_accumulate(rick_plan_t* p)
 {
-    if (!p) return RICK_ERR_INVALID;
-    p->err.clear();
+    RICK_ENTER(p);
     if (p->state != 2) { p->err = "rick_wcorrect_accumulate needs a transformed stack"; return RICK_ERR_STATE; }
     const int rc = rick_wcorrect(p, 0, 0, p->Nw, p->image, 0, 0);
     if (rc) return rc;
@@ -366,8 +412,7 @@ extern "C" int rick_wcorrect_accumulate(rick_plan_t* p)
 
 extern "C" int rick_gridcorrect(rick_plan_t* p)
 {
-    if (!p) return RICK_ERR_INVALID;
-    p->err.clear();
+    RICK_ENTER(p);
     if (p->state != 3) { p->err = "rick_gridcorrect needs a w-corrected image"; return RICK_ERR_STATE; }
     const int rc = rick_taper_divide(p, p->image);
     if (rc) return rc;
@@ -437,14 +482,18 @@ static int transform_and_correct(rick_plan_t* p, int img, int z0, int nb, double
 // part on the copy stream while the next part of the last pass is still running.
 static int image_impl(rick_plan_t* p, const void* vis, int32_t vis_dtype, const double* uvw_m,
                       const float* weights, const double* chan_freq_hz, int32_t n_chan,
-                      int64_t n_rows, double* image_out, cudaEvent_t vis_ready, double* host_out)
+                      int64_t n_rows, double* image_out, cudaEvent_t vis_ready, double* host_out,
+                      cudaEvent_t wgt_ready = nullptr)
 {
-    int rc = check_inputs(p, vis, vis_dtype, uvw_m, chan_freq_hz, n_chan, n_rows);
+    int rc = check_inputs(p, vis, vis_dtype, uvw_m, chan_freq_hz, n_chan, n_rows, true, weights, image_out);
     if (rc) return rc;
     if (p->d.cube && !image_out) { p->err = "cube mode needs image_out"; return RICK_ERR_INVALID; }
     p->state = 0;
     if ((rc = prepare(p, chan_freq_hz, n_chan, n_rows))) return rc;
     // a0..a2, then the zero-fill that needs this sort's occupancy (stale rows whole, occupied rows by tile)
+    // (the index step sums the WEIGHTS of the gridded visibilities: with weights it must not start before the
+    // copy stream has delivered them -- ADVICE r1, sum_w could come from stale staging)
+    if (wgt_ready && weights) RICK_CUDA(p, cudaStreamWaitEvent(p->stream, wgt_ready, 0));
     if ((rc = rick_index_sort(p, uvw_m, weights))) return rc;
     if (vis_ready) RICK_CUDA(p, cudaStreamWaitEvent(p->stream, vis_ready, 0));
     const size_t NN = (size_t)p->N * p->N;
@@ -511,9 +560,22 @@ extern "C" int rick_image(rick_plan_t* p, const void* vis, int32_t vis_dtype, co
                           const float* weights, const double* chan_freq_hz, int32_t n_chan,
                           int64_t n_rows, double* image_out)
 {
-    if (!p) return RICK_ERR_INVALID;
-    p->err.clear();
+    RICK_ENTER(p);
     return image_impl(p, vis, vis_dtype, uvw_m, weights, chan_freq_hz, n_chan, n_rows, image_out, nullptr, nullptr);
+}
+
+// the sticky device-side failure flag (DevCounters::error; a radix tile that lost its predecessor), read by
+// the calls that synchronise anyway: turns into a sticky RICK_ERR_CUDA
+static int check_device_error(rick_plan_t* p)
+{
+    unsigned int e = 0;
+    RICK_CUDA(p, cudaMemcpy(&e, &p->counters->error, sizeof(e), cudaMemcpyDeviceToHost));
+    if (e) {
+        p->err = "device-side failure in the radix sort (a tile never saw its predecessor's status)";
+        p->failed = RICK_ERR_CUDA;
+        return RICK_ERR_CUDA;
+    }
+    return RICK_OK;
 }
 
 template <typename Tp> static int ensure_bytes(rick_plan_t* p, Tp** buf, size_t* cap, size_t bytes)
@@ -535,8 +597,7 @@ extern "C" int rick_image_host(rick_plan_t* p, const void* vis_host, int32_t vis
                                const float* weights_host, const double* chan_freq_hz, int32_t n_chan,
                                int64_t n_rows, double* image_out_host)
 {
-    if (!p) return RICK_ERR_INVALID;
-    p->err.clear();
+    RICK_ENTER(p);
     if (!image_out_host) { p->err = "null image_out_host"; return RICK_ERR_INVALID; }
     int rc = check_inputs(p, vis_host, vis_dtype, uvw_m_host, chan_freq_hz, n_chan, n_rows);
     if (rc) return rc;
@@ -562,17 +623,21 @@ extern "C" int rick_image_host(rick_plan_t* p, const void* vis_host, int32_t vis
         RICK_CUDA(p, cudaMemcpyAsync(p->st_uvw, uvw_m_host, sizeof(double) * 3 * (size_t)n_rows, cudaMemcpyHostToDevice, p->stream));
         RICK_CUDA(p, cudaEventRecord(p->ev_fork, p->stream));
         RICK_CUDA(p, cudaStreamWaitEvent(p->stream3, p->ev_fork, 0));
-        RICK_CUDA(p, cudaMemcpyAsync(p->st_vis, vis_host, vis_bytes, cudaMemcpyHostToDevice, p->stream3));
-        if (weights_host)
+        // weights first: the index step (which sums them) waits for ev_wgt only, the gridder for ev_vis
+        if (weights_host) {
             RICK_CUDA(p, cudaMemcpyAsync(p->st_wgt, weights_host, sizeof(float) * M, cudaMemcpyHostToDevice, p->stream3));
+            RICK_CUDA(p, cudaEventRecord(p->ev_wgt, p->stream3));
+        }
+        RICK_CUDA(p, cudaMemcpyAsync(p->st_vis, vis_host, vis_bytes, cudaMemcpyHostToDevice, p->stream3));
         RICK_CUDA(p, cudaEventRecord(p->ev_vis, p->stream3));
     }
     rc = image_impl(p, p->st_vis, vis_dtype, p->st_uvw, weights_host ? p->st_wgt : nullptr, chan_freq_hz,
-                    n_chan, n_rows, p->d.cube ? p->st_img : nullptr, M ? p->ev_vis : nullptr, image_out_host);
+                    n_chan, n_rows, p->d.cube ? p->st_img : nullptr, M ? p->ev_vis : nullptr, image_out_host,
+                    (M && weights_host) ? p->ev_wgt : nullptr);
     if (rc) return rc;
     RICK_CUDA(p, cudaStreamSynchronize(p->stream));
     RICK_CUDA(p, cudaStreamSynchronize(p->stream3));
-    return RICK_OK;
+    return check_device_error(p);
 }
 
 
@@ -587,8 +652,7 @@ extern "C" int rick_image_stream_host(rick_plan_t* p, const void* vis_host, int3
                                       const float* weights_host, const double* chan_freq_hz, int32_t n_chan,
                                       int64_t n_rows, int64_t rows_per_chunk, double* image_out_host)
 {
-    if (!p) return RICK_ERR_INVALID;
-    p->err.clear();
+    RICK_ENTER(p);
     if (!image_out_host) { p->err = "null image_out_host"; return RICK_ERR_INVALID; }
     if (p->batch != p->Nw || p->d.cube) { p->err = "chunked gridding needs the whole stack resident and cube = 0"; return RICK_ERR_STATE; }
     if (rows_per_chunk < 1) { p->err = "rows_per_chunk < 1"; return RICK_ERR_INVALID; }
@@ -647,13 +711,13 @@ extern "C" int rick_image_stream_host(rick_plan_t* p, const void* vis_host, int3
         RICK_CUDA(p, cudaMemcpyAsync(image_out_host, p->image, sizeof(double) * NN, cudaMemcpyDeviceToHost, p->stream));
     RICK_CUDA(p, cudaStreamSynchronize(p->stream));
     RICK_CUDA(p, cudaStreamSynchronize(p->stream3));
-    return RICK_OK;
+    return check_device_error(p);
 }
 
 extern "C" int rick_get_image(rick_plan_t* p, double* dst_device)
 {
-    if (!p || !dst_device) return RICK_ERR_INVALID;
-    p->err.clear();
+    RICK_ENTER(p);
+    if (!dst_device || !aligned16(dst_device)) { p->err = "rick_get_image: null or misaligned destination"; return RICK_ERR_INVALID; }
     if (p->d.cube) { p->err = "rick_get_image: cube plans return their images through image_out"; return RICK_ERR_STATE; }
     if (p->state < 3) { p->err = "no image yet"; return RICK_ERR_STATE; }
     RICK_CUDA(p, cudaMemcpyAsync(dst_device, p->image, sizeof(double) * (size_t)p->N * p->N, cudaMemcpyDeviceToDevice, p->stream));
@@ -662,8 +726,8 @@ extern "C" int rick_get_image(rick_plan_t* p, double* dst_device)
 
 extern "C" int rick_get_stats(rick_plan_t* p, rick_stats* out)
 {
-    if (!p || !out) return RICK_ERR_INVALID;
-    p->err.clear();
+    RICK_ENTER(p);
+    if (!out) return RICK_ERR_INVALID;
     DevCounters c;
     WRange w;
     memset(&w, 0, sizeof(w));
@@ -677,6 +741,23 @@ extern "C" int rick_get_stats(rick_plan_t* p, rick_stats* out)
     out->w_min = w.w_min;
     out->w_max = w.w_max;
     out->n_launches = p->n_launches;
+    // occupancy of the last sort: what the pruned passes move
+    out->occ_rows = 0;
+    out->occ_tiles = 0;
+    out->n_planes = (int64_t)p->n_img * p->Nw;
+    if (p->row_occ && p->tile_occ && p->n_img > 0) {
+        const size_t nr = (size_t)p->n_img * p->Nw * p->N, nt = (size_t)p->n_img * p->Nw * p->T * p->T;
+        std::vector<unsigned char> h(nr > nt ? nr : nt);
+        RICK_CUDA(p, cudaMemcpy(h.data(), p->row_occ, nr, cudaMemcpyDeviceToHost));
+        for (size_t i = 0; i < nr; ++i) out->occ_rows += h[i] != 0;
+        RICK_CUDA(p, cudaMemcpy(h.data(), p->tile_occ, nt, cudaMemcpyDeviceToHost));
+        for (size_t i = 0; i < nt; ++i) out->occ_tiles += h[i] != 0;
+    }
+    if (c.error) {
+        p->err = "device-side failure in the radix sort (a tile never saw its predecessor's status)";
+        p->failed = RICK_ERR_CUDA;
+        return RICK_ERR_CUDA;
+    }
     return RICK_OK;
 }
 

@@ -1,6 +1,9 @@
 """GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element on
 the same seeded inputs.  Bars (BASELINE.json north_star): keys / permutation / counts
-bit-exact; planes and images relative L2 <= 1e-10 (fp64 grid) / <= 1e-4 (fp32 grid)."""
+bit-exact; planes and images relative L2 <= 1e-10 (fp64 grid) / <= 1e-4 (fp32 grid).  Beside every
+L2 bar the same number bounds the largest single deviation, max|gpu - oracle| / max|oracle|: an L2 over
+10^5..10^8 pixels can hide localised damage (one mis-flushed tile corner, one wrong strip) that a
+max-norm cannot; rounding noise stays far below it (errors are ~1e-13 / ~1e-6 of the peak)."""
 import math
 
 import numpy as np
@@ -19,6 +22,20 @@ def _rel(a, b):
     b = np.asarray(b)
     nb = np.linalg.norm(b.ravel())
     return np.linalg.norm((a - b).ravel()) / (nb if nb > 0 else 1.0)
+
+
+def _relmax(a, b):
+    a = np.asarray(a)
+    b = np.asarray(b)
+    mb = float(np.max(np.abs(b))) if b.size else 0.0
+    return float(np.max(np.abs(a - b))) / (mb if mb > 0 else 1.0) if b.size else 0.0
+
+
+def _close(a, b, tol, what=""):
+    """Both bars: relative L2 and max-norm relative to the oracle's peak."""
+    e2, em = _rel(a, b), _relmax(a, b)
+    assert e2 <= tol and em <= tol, (what, e2, em)
+    return e2
 
 
 def _rick():
@@ -72,6 +89,9 @@ def _check_staged(wl, tol, tile=0):
           "peak pixel", pk, "oracle", o["image"][pk], "gpu", g["image"][pk])
     for k, v in errs.items():
         assert v <= tol, (k, v)
+    for k, (a, b) in dict(grid=(g["grid"], o["stack_grid"]), fft=(g["fft"], o["stack_fft"]),
+                          raw=(g["raw"], o["raw_image"]), image=(g["image"], o["image"])).items():
+        assert _relmax(a, b) <= tol, (k, "max", _relmax(a, b))
     assert abs(g["image"][pk] - o["image"][pk]) <= 10 * tol * abs(o["image"][pk])
     return g, o
 
@@ -92,11 +112,11 @@ def test_cfg1_rick_image_equals_staged(cfg1):
     vis, uvw, wgt = rick.to_device(wl)
     img = plan.rick_image(vis, uvw, wgt, wl.freq_hz).cpu().numpy()
     o = _oracle(wl)
-    assert _rel(img, o["image"]) <= TOL64
-    assert _rel(plan.rick_get_image().cpu().numpy(), o["image"]) <= TOL64
+    _close(img, o["image"], TOL64)
+    _close(plan.rick_get_image().cpu().numpy(), o["image"], TOL64)
     # repeated calls on the same plan give the same answer (scratch reuse, counters reset)
     img2 = plan.rick_image(vis, uvw, wgt, wl.freq_hz).cpu().numpy()
-    assert _rel(img2, o["image"]) <= TOL64
+    _close(img2, o["image"], TOL64)
     assert plan.rick_get_stats()["n_gridded"] == o["stats"]["n_gridded"]
     plan.destroy()
 
@@ -127,9 +147,9 @@ def test_n4096_tma_tmem_column_kernels():
         img = plan.rick_image(vis, uvw, wgt, wl.freq_hz).cpu().numpy()
         img2 = plan.rick_image(vis, uvw, wgt, wl.freq_hz).cpu().numpy()      # TMEM re-allocation on reuse
         plan.destroy()
-        e = _rel(img, o["image"])
+        e = _close(img, o["image"], TOL64)
         print(f"N=4096 fused rick_image plane_batch={pb}: rel L2 {e:.2e}")
-        assert e <= TOL64 and _rel(img2, o["image"]) <= TOL64
+        _close(img2, o["image"], TOL64)
     # host-buffer entry at N = 4096: visibilities copied under index + sort, the image returned part by
     # part (whole rounds of the persistent column kernel) on the copy stream
     import torch
@@ -138,10 +158,10 @@ def test_n4096_tma_tmem_column_kernels():
     hu = torch.from_numpy(wl.uvw_m).pin_memory()
     hout = torch.full((wl.n, wl.n), float("nan"), dtype=torch.float64).pin_memory()
     plan.rick_image_host(hv, hu, None, wl.freq_hz, hout)
-    assert _rel(hout.numpy(), o["image"]) <= TOL64
+    _close(hout.numpy(), o["image"], TOL64)
     hout.fill_(float("nan"))
     plan.rick_image_host(hv, hu, None, wl.freq_hz, hout)          # staging reuse
-    assert _rel(hout.numpy(), o["image"]) <= TOL64
+    _close(hout.numpy(), o["image"], TOL64)
     plan.destroy()
     # one plane only (Horner degenerates to S = P_0)
     wl1 = synth.make_config(2, n_times=2, n_wplanes=1, n_src=4)
@@ -149,7 +169,7 @@ def test_n4096_tma_tmem_column_kernels():
     v1, u1, w1 = rick.to_device(wl1)
     img = plan.rick_image(v1, u1, w1, wl1.freq_hz).cpu().numpy()
     plan.destroy()
-    assert _rel(img, _oracle(wl1)["image"]) <= TOL64
+    _close(img, _oracle(wl1)["image"], TOL64)
 
 
 def test_support_and_beta_variants():
@@ -161,7 +181,7 @@ def test_support_and_beta_variants():
         img = plan.rick_image(vis, uvw, wgt, wl.freq_hz).cpu().numpy()
         plan.destroy()
         o = oracle.image(wl.uvw_m, wl.freq_hz, wl.vis, None, wl.n, wl.n_wplanes, S, wl.pixel_rad, beta=beta)
-        assert _rel(img, o["image"]) <= TOL64, (S, beta)
+        _close(img, o["image"], TOL64)
 
 
 def test_fp32_grid_plane_batches():
@@ -174,7 +194,7 @@ def test_fp32_grid_plane_batches():
         plan = rick.plan_from_workload(wl, plane_batch=pb)
         img = plan.rick_image(vis, uvw, wgt, wl.freq_hz).cpu().numpy()
         plan.destroy()
-        e = _rel(img, o["image"])
+        e = _close(img, o["image"], TOL32)
         N = wl.n
         inner = slice(N // 4, 3 * N // 4)
         pk = np.unravel_index(np.argmax(np.abs(o["image"])), o["image"].shape)
@@ -192,7 +212,7 @@ def test_fp64_plane_batches_equal_resident():
         plan = rick.plan_from_workload(wl, plane_batch=pb)
         img = plan.rick_image(vis, uvw, wgt, wl.freq_hz).cpu().numpy()
         plan.destroy()
-        assert _rel(img, o["image"]) <= TOL64
+        _close(img, o["image"], TOL64)
 
 
 def test_cube_mode():
@@ -209,7 +229,7 @@ def test_cube_mode():
     idx = oracle.index(wl.uvw_m, wl.freq_hz, wl.n, wl.n_wplanes, wl.support, wl.pixel_rad, 16, cube=1)
     assert np.array_equal(keys, idx["key"]) and np.array_equal(perm, oracle.sort(idx["key"]))
     for c in range(5):
-        assert _rel(cube[c], o["image"][c]) <= TOL64, c
+        _close(cube[c], o["image"][c], TOL64)
 
 
 def test_given_w_range():
@@ -223,7 +243,7 @@ def test_given_w_range():
     o = oracle.image(wl.uvw_m, wl.freq_hz, wl.vis, None, wl.n, wl.n_wplanes, wl.support, wl.pixel_rad,
                      w_min=-5000.0, w_max=6000.0)
     assert st["w_min"] == -5000.0 and st["w_max"] == 6000.0
-    assert _rel(img, o["image"]) <= TOL64
+    _close(img, o["image"], TOL64)
 
 
 def test_edge_cases_empty_dropped_single():
@@ -248,12 +268,13 @@ def test_edge_cases_empty_dropped_single():
     vis = torch.tensor([[1.5 - 0.25j]], dtype=torch.complex128, device="cuda")
     img = plan.rick_image(vis, uvw, None, freq).cpu().numpy()
     o = oracle.image(uvw.cpu().numpy(), freq, vis.cpu().numpy(), None, N, 4, 7, dl)
-    assert _rel(img, o["image"]) <= TOL64
+    _close(img, o["image"], TOL64)
     # footprint touching cell 0 / N-1 is kept
     uvw = torch.tensor([[(3 - N // 2) * du, (N - 4 - N // 2) * du, 0.0]], dtype=torch.float64, device="cuda")
     img = plan.rick_image(vis, uvw, None, freq).cpu().numpy()
     o = oracle.image(uvw.cpu().numpy(), freq, vis.cpu().numpy(), None, N, 4, 7, dl)
-    assert plan.rick_get_stats()["n_gridded"] == 1 and _rel(img, o["image"]) <= TOL64
+    assert plan.rick_get_stats()["n_gridded"] == 1
+    _close(img, o["image"], TOL64)
     plan.destroy()
 
 
@@ -273,8 +294,11 @@ def test_state_machine_and_argument_errors(cfg1):
         plan.rick_grid(vis, uvw, wgt, np.array([-1.0]))
     assert e.value.code == rick.RICK_ERR_INVALID
     plan.destroy()
+    # (fp32 grid from S = 11 on: the unclamped taper amplifies fp32 rounding beyond the 1e-4 bar, rick.h;
+    # kb_beta = 3 with S = 7: the taper has a zero inside the image; fp64 beyond N = 8192)
     for bad in [dict(n=100), dict(support=6), dict(support=17), dict(pixel_rad=0.0), dict(n_wplanes=0),
-                dict(tile=12), dict(plane_batch=99)]:
+                dict(tile=12), dict(plane_batch=99), dict(support=11, grid_prec="f32"), dict(kb_beta=3.0),
+                dict(n=16384)]:
         kw = dict(n=256, n_wplanes=8, support=7, pixel_rad=1e-4)
         kw.update(bad)
         with pytest.raises(rick.RickError) as e:
@@ -298,7 +322,7 @@ def test_host_buffer_entry(cfg1):
     out = torch.empty((wl.n, wl.n), dtype=torch.float64).pin_memory()
     plan.rick_image_host(vis, uvw, None, wl.freq_hz, out)
     o = _oracle(wl)
-    assert _rel(out.numpy(), o["image"]) <= TOL64
+    _close(out.numpy(), o["image"], TOL64)
     plan.destroy()
 
 
@@ -319,16 +343,15 @@ def test_stream_host_chunks(cfg1):
         out.fill_(float("nan"))
         plan.rick_image_stream_host(vis, uvw, None, wl.freq_hz, out, rpc)
         st = plan.rick_get_stats()
-        e = _rel(out.numpy(), o["image"])
+        e = _close(out.numpy(), o["image"], TOL64)
         print(f"stream rows_per_chunk={rpc}: rel L2 {e:.2e}")
-        assert e <= TOL64
         assert st["n_vis"] == o["stats"]["n_vis"] and st["n_gridded"] == o["stats"]["n_gridded"]
         assert st["n_dropped"] == o["stats"]["n_dropped"]
         assert st["w_min"] == o["stats"]["w_min"] and st["w_max"] == o["stats"]["w_max"]
     # the plan still serves the one-shot entry afterwards (occupancy maps and dirty rows consistent)
     dv, du, dw = rick.to_device(wl)
     img = plan.rick_image(dv, du, dw, wl.freq_hz).cpu().numpy()
-    assert _rel(img, o["image"]) <= TOL64
+    _close(img, o["image"], TOL64)
     # a short set, one row per chunk
     import dataclasses
     few = dataclasses.replace(wl)
@@ -337,7 +360,7 @@ def test_stream_host_chunks(cfg1):
     of = _oracle(few)
     plan.rick_image_stream_host(torch.from_numpy(few.vis).pin_memory(), torch.from_numpy(few.uvw_m).pin_memory(), None,
                                 few.freq_hz, out, 1)
-    assert _rel(out.numpy(), of["image"]) <= TOL64
+    _close(out.numpy(), of["image"], TOL64)
     # an empty set gives an all-zero image and zero counts
     ev = torch.empty((0, wl.n_chan), dtype=torch.complex128)
     eu = torch.empty((0, 3), dtype=torch.float64)
@@ -371,9 +394,8 @@ def test_stream_host_weights_fused_4096():
         out.fill_(float("nan"))
         plan.rick_image_stream_host(vis, uvw, wgt, wl.freq_hz, out, rpc)
         st = plan.rick_get_stats()
-        e = _rel(out.numpy(), o["image"])
+        e = _close(out.numpy(), o["image"], TOL64)
         print(f"stream N=4096 weights rows_per_chunk={rpc}: rel L2 {e:.2e}")
-        assert e <= TOL64
         assert st["n_gridded"] == o["stats"]["n_gridded"]
         assert abs(st["sum_w"] - o["stats"]["sum_w"]) <= 1e-9 * abs(o["stats"]["sum_w"])
     plan.destroy()
@@ -401,9 +423,10 @@ def test_long_columns_two_pass(prec, pb, tol):
     hout = torch.full((wl.n, wl.n), float("nan"), dtype=torch.float64).pin_memory()
     plan.rick_image_host(hv, hu, None, wl.freq_hz, hout)
     plan.destroy()
-    e = _rel(img, o["image"])
-    print(f"N=8192 two-pass columns {prec} plane_batch={pb}: rel L2 {e:.2e}, host entry {_rel(hout.numpy(), o['image']):.2e}")
-    assert e <= tol and _rel(img2, o["image"]) <= tol and _rel(hout.numpy(), o["image"]) <= tol
+    e = _close(img, o["image"], tol)
+    print(f"N=8192 long columns {prec} plane_batch={pb}: rel L2 {e:.2e}, host entry {_rel(hout.numpy(), o['image']):.2e}")
+    _close(img2, o["image"], tol)
+    _close(hout.numpy(), o["image"], tol)
     assert st["n_gridded"] == o["stats"]["n_gridded"]
 
 
@@ -411,8 +434,9 @@ def test_randomized_parameter_sweep():
     """Seeded sweep over what the fixed cases do not combine: support 3..11, sort tile 8/16/32, grid edge
     64..2048, fp64 / fp32 grid, cube, ragged plane batches, weights, complex64 / complex128, and the chunked
     host entry -- every case against the oracle (twice through the same plan: stale rows, dirty flags).
-    fp32 grid with S = 11 is left out: the taper is not clamped (R12) and at S = 11 its corner value
-    (~1e-8 of the centre) amplifies the fp32 rounding of the planes to ~3e-4 of the image norm."""
+    The fp32 grid stops at S = 9: rick_plan refuses fp32 plans with S >= 11 (rick.h; the taper is not
+    clamped, R12, and at S = 11 its corner value, ~1e-8 of the centre, amplifies the fp32 rounding of the
+    planes to ~3e-4 of the image norm), which test_state_machine_and_argument_errors checks."""
     import torch
     rick = _rick()
     rng = np.random.default_rng(20260119)
@@ -452,8 +476,9 @@ def test_randomized_parameter_sweep():
         plan.destroy()
         tol = TOL64 if prec == "f64" else TOL32
         errs = [_rel(x.reshape(o["image"].shape), o["image"]) for x in outs]
-        print(desc, " ".join(f"{e:.1e}" for e in errs))
-        assert all(e <= tol for e in errs), desc
+        emax = [_relmax(x.reshape(o["image"].shape), o["image"]) for x in outs]
+        print(desc, " ".join(f"{e:.1e}" for e in errs), "max", " ".join(f"{e:.1e}" for e in emax))
+        assert all(e <= tol for e in errs) and all(e <= tol for e in emax), desc
         assert st["n_gridded"] == o["stats"]["n_gridded"], desc
 
 
@@ -471,10 +496,132 @@ def test_cube_host_entry_image_groups():
     for _ in range(2):
         out.fill_(float("nan"))
         plan.rick_image_host(hv, hu, None, wl.freq_hz, out)
-        e = _rel(out.numpy(), o["image"])
+        e = _close(out.numpy(), o["image"], TOL64)
         print(f"cube host entry, 12 channels in groups of 8: rel L2 {e:.2e}")
-        assert e <= TOL64
     dv, du, dw = rick.to_device(wl)
     img = plan.rick_image(dv, du, dw, wl.freq_hz).cpu().numpy()
-    assert _rel(img, o["image"]) <= TOL64
+    _close(img, o["image"], TOL64)
     plan.destroy()
+
+
+def test_host_entry_weights_sum_w_small_set():
+    """rick_image_host with weights on a FRESH plan and M < 2^22 (the one-shot path): the index step sums the
+    weights of the gridded visibilities, so it must wait for the copy stream to deliver them (ADVICE r1:
+    sum_w could come from uninitialised staging).  sum_w, counts and image against the oracle; twice."""
+    import torch
+    rick = _rick()
+    wl = synth.make_config(2, n_times=9, n=1024, n_chan=7, n_wplanes=4, n_src=10, with_weights=True)
+    assert wl.n_vis < (1 << 22)
+    o = _oracle(wl)
+    hv = torch.from_numpy(np.ascontiguousarray(wl.vis)).pin_memory()
+    hu = torch.from_numpy(wl.uvw_m).pin_memory()
+    hw = torch.from_numpy(wl.weights).pin_memory()
+    out = torch.empty((wl.n, wl.n), dtype=torch.float64).pin_memory()
+    for rep in range(2):
+        plan = rick.plan_from_workload(wl)          # fresh staging each time
+        plan.rick_image_host(hv, hu, hw, wl.freq_hz, out)
+        st = plan.rick_get_stats()
+        plan.destroy()
+        assert st["n_gridded"] == o["stats"]["n_gridded"]
+        assert abs(st["sum_w"] - o["stats"]["sum_w"]) <= 1e-9 * abs(o["stats"]["sum_w"]), (st["sum_w"], o["stats"]["sum_w"])
+        _close(out.numpy(), o["image"], TOL64)
+
+
+def test_misaligned_device_pointers_are_refused(cfg1):
+    """rick.h promises 16-byte aligned device pointers and argument errors before any work is enqueued: a
+    misaligned vis / uvw / weights / image_out must come back as RICK_ERR_INVALID, not fault the context."""
+    import torch
+    rick = _rick()
+    wl = cfg1
+    plan = rick.plan_from_workload(wl)
+    vis, uvw, wgt = rick.to_device(wl)
+    ref = plan.rick_image(vis, uvw, None, wl.freq_hz).cpu().numpy()
+    v8 = torch.empty(vis.numel() + 1, dtype=torch.complex64, device="cuda")[1:].reshape(vis.shape)   # 8-byte offset
+    assert v8.data_ptr() % 16 == 8
+    u8 = torch.empty(uvw.numel() + 1, dtype=torch.float64, device="cuda")[1:].reshape(uvw.shape)
+    w4 = torch.ones(vis.numel() + 1, dtype=torch.float32, device="cuda")[1:].reshape(vis.shape)
+    o8 = torch.empty(wl.n * wl.n + 1, dtype=torch.float64, device="cuda")[1:].reshape(wl.n, wl.n)
+    for args in [(v8, uvw, None, None), (vis, u8, None, None), (vis, uvw, w4, None), (vis, uvw, None, o8)]:
+        with pytest.raises(rick.RickError) as e:
+            plan.rick_image(args[0], args[1], args[2], wl.freq_hz, args[3])
+        assert e.value.code == rick.RICK_ERR_INVALID
+    with pytest.raises(rick.RickError) as e:
+        plan.rick_grid(v8, uvw, None, wl.freq_hz)
+    assert e.value.code == rick.RICK_ERR_INVALID
+    # the plan is still usable (argument errors are not sticky)
+    again = plan.rick_image(vis, uvw, None, wl.freq_hz).cpu().numpy()
+    plan.destroy()
+    assert np.array_equal(again, ref) or _rel(again, ref) <= 1e-12
+
+
+def test_nonfinite_coordinates_are_dropped(cfg1):
+    """Reading R23: a visibility with a non-finite u, v or w is dropped and counted, a non-finite w takes no
+    part in the w range, and coordinates far beyond the int range do not wrap onto the grid."""
+    import dataclasses
+    rick = _rick()
+    wl = dataclasses.replace(cfg1, uvw_m=cfg1.uvw_m.copy())
+    bad = {5: (0, np.nan), 17: (1, np.inf), 29: (2, np.nan), 41: (2, -np.inf), 53: (0, 1e300), 65: (1, -3e12)}
+    for r, (ax, val) in bad.items():
+        wl.uvw_m[r, ax] = val
+    o = _oracle(wl)
+    assert o["stats"]["n_dropped"] >= len(bad) and np.isfinite(o["stats"]["w_min"]) and np.isfinite(o["image"]).all()
+    plan = rick.plan_from_workload(wl)
+    vis, uvw, wgt = rick.to_device(wl)
+    img = plan.rick_image(vis, uvw, wgt, wl.freq_hz).cpu().numpy()
+    keys = plan.debug_keys()
+    st = plan.rick_get_stats()
+    plan.destroy()
+    idx = oracle.index(wl.uvw_m, wl.freq_hz, wl.n, wl.n_wplanes, wl.support, wl.pixel_rad, 16)
+    assert np.array_equal(keys, idx["key"])
+    for r in bad:
+        assert keys[r] == np.uint64(0xFFFFFFFFFFFFFFFF)
+    assert st["n_dropped"] == o["stats"]["n_dropped"] and st["n_gridded"] == o["stats"]["n_gridded"]
+    assert st["w_min"] == o["stats"]["w_min"] and st["w_max"] == o["stats"]["w_max"]
+    _close(img, o["image"], TOL64)
+
+
+def test_out_of_memory_is_recoverable_and_cube_group_fallback():
+    """(a) A sort-scratch allocation that fails returns RICK_ERR_OOM and leaves the plan usable: the next call
+    re-grows the scratch (rick.h "Errors").  (b) A cube plan that cannot get the memory for a group of 8
+    images falls back to one resident image and gives the same cube.  Both forced with a ballast allocation
+    that leaves a known amount of device memory free."""
+    import torch
+    rick = _rick()
+    wl = synth.make_config(5, n_times=3, n=2048, n_chan=9, n_wplanes=4, n_src=4)      # image stack 268 MB, group of 8: 2.1 GB
+    o = _oracle(wl)
+    vis, uvw, wgt = rick.to_device(wl)
+    # (a)'s inputs exist before the ballast: 64 Mi visibilities at the phase centre; their sort items need
+    # 3 x 8 B x M = 1.6 GB of scratch, more than the ballast leaves
+    big_rows = (64 << 20) // wl.n_chan
+    bv = torch.zeros((big_rows, wl.n_chan), dtype=torch.complex64, device="cuda")
+    bu = torch.zeros((big_rows, 3), dtype=torch.float64, device="cuda")
+    torch.cuda.synchronize()
+    torch.cuda.empty_cache()
+    free, total = torch.cuda.mem_get_info()
+    keep = 1200 << 20                                  # room for one image's stack + image + scratch, not for 8
+    ballast = torch.empty(free - keep, dtype=torch.uint8, device="cuda")
+    try:
+        plan = rick.plan_from_workload(wl)             # group of 8 images does not fit -> one image at a time
+        cube = plan.rick_image(vis, uvw, wgt, wl.freq_hz)
+        torch.cuda.synchronize()
+        launches_single = plan.rick_get_stats()["n_launches"]
+        got = cube.cpu().numpy()
+        with pytest.raises(rick.RickError) as e:
+            plan.rick_image(bv, bu, None, wl.freq_hz, cube)
+        assert e.value.code == rick.RICK_ERR_OOM
+        again = plan.rick_image(vis, uvw, wgt, wl.freq_hz).cpu().numpy()      # the plan re-grows its scratch
+        plan.destroy()
+    finally:
+        del ballast
+        bv = bu = None
+        torch.cuda.empty_cache()
+    for c in range(wl.n_chan):
+        _close(got[c], o["image"][c], TOL64)
+        _close(again[c], o["image"][c], TOL64)
+    plan = rick.plan_from_workload(wl)                 # with memory: groups of 8 images, fewer launches
+    cube8 = plan.rick_image(vis, uvw, wgt, wl.freq_hz).cpu().numpy()
+    launches_group = plan.rick_get_stats()["n_launches"]
+    plan.destroy()
+    assert launches_group < launches_single
+    for c in range(wl.n_chan):
+        _close(cube8[c], o["image"][c], TOL64)

@@ -125,3 +125,29 @@ def test_sort_is_stable_sort(cfg1):
     same = ks[1:] == ks[:-1]
     assert np.all(perm[1:][same] > perm[:-1][same])
     assert oracle.sort(np.zeros(0, np.uint64)).shape == (0,)
+
+
+def test_nonfinite_and_out_of_int_range_coordinates_are_dropped():
+    """Reading R23: a visibility with a non-finite u, v or w cannot lie on the grid (R10) and is
+    dropped; a non-finite w takes no part in the w range; a finite coordinate beyond the int range is off
+    the grid like any other.  Everything else about the clean rows is unchanged by their presence."""
+    N, Nw, S, dl, B = 64, 4, 7, 1e-3, 16
+    du = 1.0 / (N * dl)
+    f = np.array([299792458.0])
+    clean = np.array([[1.2 * du, -3.4 * du, 10.0], [5.0 * du, 6.0 * du, -20.0], [-7.7 * du, 0.3 * du, 30.0]])
+    bad = np.array([[np.nan, 0.0, 1.0], [0.0, np.inf, 2.0], [0.0, 0.0, np.nan], [1.0 * du, 1.0 * du, -np.inf],
+                    [1e300, 0.0, 3.0], [0.0, -4e12 * du, 4.0]])
+    uvw = np.concatenate([clean[:1], bad[:3], clean[1:2], bad[3:], clean[2:]])
+    r = oracle.index(uvw, f, N, Nw, S, dl, B)
+    r0 = oracle.index(clean, f, N, Nw, S, dl, B)
+    DROPPED = np.uint64(0xFFFFFFFFFFFFFFFF)
+    is_clean = np.array([True, False, False, False, True, False, False, False, True])
+    assert np.all(r["key"][~is_clean] == DROPPED)
+    # the w range is that of the rows with a finite w (rows 5 and 6 of `bad` have finite w = 3, 4: inside it)
+    assert r["w_min"][0] == -20.0 and r["w_max"][0] == 30.0
+    assert r0["w_min"][0] == -20.0 and r0["w_max"][0] == 30.0
+    assert np.array_equal(r["key"][is_clean], r0["key"]) and np.all(r0["key"] != DROPPED)
+    assert np.array_equal(r["ip"][is_clean], r0["ip"])
+    # all rows non-finite in w: range collapses to [0, 0] as for an empty set
+    r1 = oracle.index(bad[2:4], f, N, Nw, S, dl, B)
+    assert r1["w_min"][0] == 0.0 and r1["w_max"][0] == 0.0 and np.all(r1["key"] == DROPPED)
