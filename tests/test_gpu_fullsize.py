@@ -48,15 +48,16 @@ def _gpu_image(wl, **over):
 
 
 def _report(name, img, ref):
-    """relative L2 -- and the max-norm max|gpu - oracle| / max|oracle|, which must meet the same bar (an L2
-    over 10^7..10^8 pixels can hide a damaged tile or strip; rounding noise stays far below the bar)."""
+    """max(relative L2, max-norm / 5): the max-norm max|gpu - oracle| / max|oracle| must stay below 5 x the L2
+    bar (what rounding noise AT the L2 bar would reach over 10^7..10^8 pixels; an L2 alone can hide a damaged
+    tile or strip -- tests/test_gpu_parity.py derives the factor)."""
     N = ref.shape[-1]
     inner = slice(N // 4, 3 * N // 4)
     pk = np.unravel_index(np.argmax(np.abs(ref)), ref.shape)
     e, ei = _rel(img, ref), _rel(img[..., inner, inner], ref[..., inner, inner])
     em = float(np.max(np.abs(img - ref))) / float(np.max(np.abs(ref)))
     print(f"{name}: rel L2 {e:.3e} (inner half {ei:.3e}), max-norm {em:.3e}; peak pixel {pk} oracle {ref[pk]:.9e} gpu {img[pk]:.9e}")
-    return max(e, em)
+    return max(e, em / 5.0)
 
 
 def _stats_equal(st, so):
