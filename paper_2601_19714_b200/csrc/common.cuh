@@ -102,7 +102,8 @@ struct rick_plan_s {
     // cube plans with all planes of an image resident keep img_batch images' stacks resident (slots = batch *
     // img_batch) so that zero-fill, gridder and row pass run once per group of images, not once per channel
     int img_batch, slots;
-    int cols12_ok;
+    int cols12_ok;               // N = 4096 fp64: k_cols12_fft / k_cols12_wcorrect
+    int cols13_ok;               // N = 8192 fp64: k_cols13_wcorrect (one column per SM, tensor map in cols12_tmap_sw)
     alignas(64) unsigned char cols12_tmap[128];
     alignas(64) unsigned char cols12_tmap_sw[128];   // same view, 32-byte swizzle (k_cols12_wcorrect)
 
@@ -185,7 +186,9 @@ int rick_cols12_init(rick_plan_t* p);                                    // fft_
 int rick_cols12_fft(rick_plan_t* p, int n_planes);                       // fft_cols12.cu
 int rick_cols12_wcorrect(rick_plan_t* p, int img, int z_first, int n_planes, double* image,
                          int accumulate, int fuse_taper, int strip_begin, int strip_end, int slot_first = 0);   // fft_cols12.cu
-int rick_cols12_strips(void);                                            // fft_cols12.cu
+int rick_cols12_strips(const rick_plan_t* p);                            // fft_cols12.cu: work units of the fused pass
+int rick_cols12_unit_cols(const rick_plan_t* p);                         // columns per unit (2 at N = 4096, 1 at N = 8192)
+int rick_cols_fused(const rick_plan_t* p);                               // 1 when the single fused column pass serves this plan
 int rick_wcorrect(rick_plan_t* p, int img, int z_first, int n_planes, double* image,
                   int accumulate, int fuse_taper, int slot_first = 0);   // wcorrect.cu
 int rick_taper_divide(rick_plan_t* p, double* image);                    // wcorrect.cu

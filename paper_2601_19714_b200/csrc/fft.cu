@@ -259,7 +259,7 @@ template <typename T, int LOG2N> static int launch_cols2(rick_plan_t* p, int pla
     return RICK_OK;
 }
 
-int rick_cols2_on(const rick_plan_t* p) { return p->log2N >= 13; }
+int rick_cols2_on(const rick_plan_t* p) { return p->log2N >= 13 && !p->cols13_ok; }
 
 int rick_fft_cols2(rick_plan_t* p, int plane_first, int n_planes)
 {

@@ -25,6 +25,7 @@
 #include "common.cuh"
 #include "fft_core.cuh"
 #include "sm100_ptx.cuh"
+#include <stdlib.h>
 
 namespace {
 
@@ -298,42 +299,255 @@ k_cols12_wcorrect(const __grid_constant__ CUtensorMap tmap, const double2* __res
     if (warp == 0) tmem_dealloc_all(tbase);
 }
 
+
+// ---------------------------------------------------------------------------------------------------
+// N = 8192 = 2 * 4096 (fp64): the same fused single pass for a column of 128 KB.  One SM holds ONE column
+// (staging 128 KB, the transform in registers, S and step in tensor memory), fetched by one TMA instruction
+// per (column, plane) in 16-byte pieces.  The two column groups of the N = 4096 kernel become the two halves
+// of a decimation-in-frequency split that needs no exchange between the groups: with x'[n] = G[(n + N/2) mod N]
+// (centring on input) and H = N/2,
+//     X[2 kk]     = FFT_H( x'[n] + x'[n + H] )            = FFT_H( G[n + H] + G[n] )              group 0
+//     X[2 kk + 1] = FFT_H( (x'[n] - x'[n + H]) W_N^n )    = FFT_H( (G[n + H] - G[n]) W_N^n )      group 1
+// both groups read the whole staging (rows n and n + H of the thread's 16 values of n), run their own
+// 4096-point transform exactly as in k_cols12_wcorrect, and keep the outputs k = 2 (t2 + 256 r) + g, i.e. the
+// pixel rows q = (k + N/2) mod N = 2 t2 + g + 512 ((r + 8) & 15).  Against the two-pass path (fft.cu) the stack
+// is read ONCE and never written: 68.7 GB instead of 170 GB at configs[2].
+constexpr int C13_N = 2 * C12_N;
+constexpr uint32_t C13_STAGE_BYTES = (uint32_t)C13_N * 16u;          // 131072: one column
+
+__device__ __forceinline__ void col13_fft_g(double2 (&v)[16], const RolesG& R, const double2* __restrict__ stg,
+                                            double* __restrict__ ex, const double2* __restrict__ twN,
+                                            unsigned long long* full, unsigned long long* empty, uint32_t& parity,
+                                            bool issue_next, const CUtensorMap* tmap, int next_col, int next_plane)
+{
+    // group 1: W_N^n for n = t1 + 256 e is W_N^t1 times the constant e^{2 pi i e / 32}
+    double2 wb;
+    if (R.g == 1) {
+        wb = twN[R.t1];
+        named_bar_sync(3, 512);                  // group 0 has read the staging of this item
+    }
+    mbar_wait(full, parity);
+    // staging order [e2][e][w][hh] (16-byte elements): row = w + 16 hh + 256 e + 4096 e2
+    const double2* s0 = stg + R.w * 16 + R.hh;
+    if (R.g == 0) {
+#pragma unroll
+        for (int e = 0; e < 16; ++e) v[e] = cadd(s0[(16 + e) * 256], s0[e * 256]);
+    } else {
+#pragma unroll
+        for (int e = 0; e < 16; ++e) v[e] = csub(s0[(16 + e) * 256], s0[e * 256]);
+    }
+    if (R.g == 0) named_bar_arrive(3, 512);
+    __syncwarp();
+    if ((threadIdx.x & 31) == 0) mbar_arrive(empty);
+    if (threadIdx.x == 256 && issue_next) {
+        mbar_wait(empty, parity);
+        mbar_arrive_expect_tx(full, C13_STAGE_BYTES);
+        tma_load_5d(const_cast<double2*>(stg), tmap, full, 2 * next_col, 0, 0, 0, 2 * next_plane);
+    }
+    parity ^= 1u;
+    if (R.g == 1) {
+        // e^{2 pi i e / 32}, e = 1 .. 15
+        constexpr double c32[16] = {1.0, 0.98078528040323044913, 0.92387953251128675613, 0.83146961230254523708,
+                                    0.70710678118654752440, 0.55557023301960222474, 0.38268343236508977173,
+                                    0.19509032201612826785, 0.0, -0.19509032201612826785, -0.38268343236508977173,
+                                    -0.55557023301960222474, -0.70710678118654752440, -0.83146961230254523708,
+                                    -0.92387953251128675613, -0.98078528040323044913};
+        v[0] = cmul(v[0], wb);
+#pragma unroll
+        for (int e = 1; e < 16; ++e) {
+            double2 c;
+            c.x = c32[e];
+            c.y = c32[e < 8 ? 8 - e : e - 8];                             // sin(pi e/16) = cos(pi (e - 8)/16)
+            v[e] = cmul(v[e], cmul(wb, c));
+        }
+    }
+    bfly16<double, C12_LOG2N, 0>(v, R.t1, twN);
+    // the 4096-point twiddles are every second entry of the N = 8192 table
+    const double2 w1_s2 = twN[2 * bfly16_tw_index<C12_LOG2N, 4>(R.t2)];
+    named_bar_sync(1 + R.g, 256);                // the group's reads of the previous item's exchange are done
+    xchg16_warp_grp(v, ex + (size_t)(threadIdx.x >> 5) * (2 * 16 * 17), R.wl, R.hh);
+    bfly16<double, C12_LOG2N, 4>(v, R.t2, twN, &w1_s2);
+    const double2 w1_s3 = twN[2 * bfly16_tw_index<C12_LOG2N, 8>(R.t2)];
+    named_bar_sync(1 + R.g, 256);                // every warp of the group is done with its private region
+    xchg16_grp(v, ex + (size_t)R.g * (C12_N + C12_N / 16), R.t2, 1 + R.g);
+    bfly16<double, C12_LOG2N, 8>(v, R.t2, twN, &w1_s3);
+}
+
+__global__ void __launch_bounds__(C12_THREADS, 1)
+k_cols13_wcorrect(const __grid_constant__ CUtensorMap tmap, const double2* __restrict__ twN, int n_planes,
+                  int z_first, double dl, const WRange* __restrict__ wr, double* __restrict__ image,
+                  int accumulate, const double* __restrict__ taper, int col_begin, int col_end, int slot_first)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    unsigned char* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
+    double2* stg = reinterpret_cast<double2*>(smem);
+    double* ex = reinterpret_cast<double*>(smem + C13_STAGE_BYTES);
+    unsigned long long* full = reinterpret_cast<unsigned long long*>(smem + C13_STAGE_BYTES + C12_EX_BYTES);
+    unsigned long long* empty = full + 1;
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + C13_STAGE_BYTES + C12_EX_BYTES + 16);
+    const RolesG R = roles_g();
+    const int warp = threadIdx.x >> 5;
+    if (threadIdx.x == 0) {
+        mbar_init(full, 1);
+        mbar_init(empty, C12_THREADS / 32);
+        mbar_fence_init();
+    }
+    if (warp == 0) tmem_alloc_all(tmem_slot);
+    tmem_fence_before_sync();
+    __syncthreads();
+    tmem_fence_after_sync();
+    const uint32_t tbase = *tmem_slot;
+    const uint32_t tS = tbase + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)((warp >> 2) * 128);
+    const uint32_t tStep = tS + 64;
+
+    int col = col_begin + (int)blockIdx.x;
+    if (threadIdx.x == 0 && col < col_end) {
+        mbar_arrive_expect_tx(full, C13_STAGE_BYTES);
+        tma_load_5d(stg, &tmap, full, 2 * col, 0, 0, 0, 2 * (slot_first + n_planes - 1));
+    }
+    uint32_t parity = 0;
+    const double dw = wr->dw;
+    const double w_first = wr->w_min + ((double)z_first + 0.5) * dw;
+    const int q0 = 2 * R.t2 + R.g;               // pixel rows of this thread: q0 + 512 ((r + 8) & 15)
+    for (; col < col_end; col += gridDim.x) {
+        const double l = (double)(col - C13_N / 2) * dl;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            double2 st[4];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const int q = q0 + 512 * ((4 * k + i + 8) & 15);
+                const double m = (double)(q - C13_N / 2) * dl;
+                const double r2 = l * l + m * m;
+                double xs = 0.0;
+                if (r2 < 1.0) xs = dw * (-r2 / (1.0 + sqrt(1.0 - r2)));
+                xs -= rint(xs);
+                sincospi(2.0 * xs, &st[i].y, &st[i].x);
+            }
+            uint32_t r[16];
+            pack4(st, r);
+            tmem_st16(tStep + 16 * k, r);
+        }
+        tmem_wait_st();
+        for (int plane = n_planes - 1; plane >= 0; --plane) {
+            const bool more = plane > 0 || col + (int)gridDim.x < col_end;
+            double2 v[16];
+            col13_fft_g(v, R, stg, ex, twN, full, empty, parity, more, &tmap, plane > 0 ? col : col + (int)gridDim.x,
+                        slot_first + (plane > 0 ? plane - 1 : n_planes - 1));
+            if (plane == n_planes - 1) {
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    const double2 s4[4] = {v[4 * k], v[4 * k + 1], v[4 * k + 2], v[4 * k + 3]};
+                    uint32_t r[16];
+                    pack4(s4, r);
+                    tmem_st16(tS + 16 * k, r);
+                }
+            } else {
+                tmem_wait_st();
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    uint32_t rs[16], rt[16];
+                    tmem_ld16(tS + 16 * k, rs);
+                    tmem_ld16(tStep + 16 * k, rt);
+                    tmem_wait_ld();
+                    double2 s4[4], st[4];
+                    unpack4(rs, s4);
+                    unpack4(rt, st);
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) {
+                        const double2 a = v[4 * k + i];
+                        double2 o;
+                        o.x = fma(st[i].x, s4[i].x, fma(-st[i].y, s4[i].y, a.x));
+                        o.y = fma(st[i].x, s4[i].y, fma(st[i].y, s4[i].x, a.y));
+                        s4[i] = o;
+                    }
+                    pack4(s4, rs);
+                    tmem_st16(tS + 16 * k, rs);
+                }
+            }
+        }
+        tmem_wait_st();
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            uint32_t rs[16];
+            tmem_ld16(tS + 16 * k, rs);
+            tmem_wait_ld();
+            double2 s4[4];
+            unpack4(rs, s4);
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const int q = q0 + 512 * ((4 * k + i + 8) & 15);
+                const double m = (double)(q - C13_N / 2) * dl;
+                const double r2 = l * l + m * m;
+                double val = 0.0;
+                if (r2 < 1.0) {
+                    double x0 = w_first * (-r2 / (1.0 + sqrt(1.0 - r2)));
+                    x0 -= rint(x0);
+                    double pr, pi;
+                    sincospi(2.0 * x0, &pi, &pr);
+                    val = pr * s4[i].x - pi * s4[i].y;
+                }
+                const size_t pix = (size_t)q * C13_N + col;
+                if (accumulate) val += image[pix];
+                if (taper) val /= (taper[col] * taper[q]);
+                image[pix] = val;
+            }
+        }
+    }
+    tmem_fence_before_sync();
+    __syncthreads();
+    if (warp == 0) tmem_dealloc_all(tbase);
+}
+
 }   // namespace
 
-// Build the 5-D tensor map over the plan's resident stack (once, at plan creation).
-int rick_cols12_init(rick_plan_t* p)
+// Build the 5-D tensor maps over the plan's resident stack (once, at plan creation).
+static int encode_map(rick_plan_t* p, void* out, const cuuint64_t* dims, const cuuint64_t* strides, const cuuint32_t* box,
+                      CUtensorMapSwizzle sw, CUtensorMapL2promotion promo)
 {
-    p->cols12_ok = 0;
-    if (p->f32 || p->N != C12_N) return RICK_OK;
     rick_encode_tiled_fn enc = rick_get_encode_tiled();
     if (!enc) {
         p->err = "cuTensorMapEncodeTiled is not available from this driver";
         return RICK_ERR_CUDA;
     }
-    static_assert(sizeof(CUtensorMap) <= sizeof(p->cols12_tmap), "tensor map storage");
-    const cuuint64_t rowB = (cuuint64_t)C12_N * 16;
-    // dims: (re/im/column pair as doubles, hh, w, e, plane) with row = w + 16 hh + 256 e
-    const cuuint64_t dims[5] = {(cuuint64_t)2 * C12_N, 16, 16, 16, (cuuint64_t)p->slots};
-    const cuuint64_t strides[4] = {16 * rowB, rowB, 256 * rowB, (cuuint64_t)C12_N * rowB};
-    const cuuint32_t box[5] = {4, 16, 16, 16, 1};
     const cuuint32_t es[5] = {1, 1, 1, 1, 1};
-    const CUresult r = enc(reinterpret_cast<CUtensorMap*>(p->cols12_tmap), CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 5, p->stack,
-                           dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
-                           CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (const char* ev = getenv("RICK_EXP_PROMO")) promo = (CUtensorMapL2promotion)atoi(ev);   // EXPERIMENT
+    const CUresult r = enc(reinterpret_cast<CUtensorMap*>(out), CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 5, p->stack, dims, strides,
+                           box, es, CU_TENSOR_MAP_INTERLEAVE_NONE, sw, promo, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) {
         p->err = "cuTensorMapEncodeTiled failed";
         return RICK_ERR_CUDA;
     }
+    return RICK_OK;
+}
+
+int rick_cols12_init(rick_plan_t* p)
+{
+    p->cols12_ok = 0;
+    p->cols13_ok = 0;
+    if (p->f32 || (p->N != C12_N && p->N != C13_N)) return RICK_OK;
+    static_assert(sizeof(CUtensorMap) <= sizeof(p->cols12_tmap), "tensor map storage");
+    static_assert(sizeof(CUtensorMap) <= sizeof(p->cols12_tmap_sw), "tensor map storage");
+    const cuuint64_t rowB = (cuuint64_t)p->N * 16;
+    int rc;
+    if (p->N == C13_N) {
+        // dims: (re/im of one column as doubles, hh, w, e, e2 + 2 plane) with row = w + 16 hh + 256 e + 4096 e2
+        const cuuint64_t dims[5] = {(cuuint64_t)2 * C13_N, 16, 16, 16, (cuuint64_t)2 * p->slots};
+        const cuuint64_t strides[4] = {16 * rowB, rowB, 256 * rowB, 4096 * rowB};
+        const cuuint32_t box[5] = {2, 16, 16, 16, 2};
+        if ((rc = encode_map(p, p->cols12_tmap_sw, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE))) return rc;
+        RICK_CUDA(p, cudaFuncSetAttribute(k_cols13_wcorrect, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C12_SMEM));
+        p->cols13_ok = 1;
+        return RICK_OK;
+    }
+    // dims: (re/im/column pair as doubles, hh, w, e, plane) with row = w + 16 hh + 256 e
+    const cuuint64_t dims[5] = {(cuuint64_t)2 * C12_N, 16, 16, 16, (cuuint64_t)p->slots};
+    const cuuint64_t strides[4] = {16 * rowB, rowB, 256 * rowB, (cuuint64_t)C12_N * rowB};
+    const cuuint32_t box[5] = {4, 16, 16, 16, 1};
+    if ((rc = encode_map(p, p->cols12_tmap, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE))) return rc;
+    if ((rc = encode_map(p, p->cols12_tmap_sw, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_32B, CU_TENSOR_MAP_L2_PROMOTION_NONE))) return rc;
     RICK_CUDA(p, cudaFuncSetAttribute(k_cols12_fft, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C12_SMEM));
     RICK_CUDA(p, cudaFuncSetAttribute(k_cols12_wcorrect, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C12_SMEM));
-    static_assert(sizeof(CUtensorMap) <= sizeof(p->cols12_tmap_sw), "tensor map storage");
-    const CUresult r2 = enc(reinterpret_cast<CUtensorMap*>(p->cols12_tmap_sw), CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 5, p->stack,
-                            dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_32B,
-                            CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    if (r2 != CUDA_SUCCESS) {
-        p->err = "cuTensorMapEncodeTiled (swizzled) failed";
-        return RICK_ERR_CUDA;
-    }
     p->cols12_ok = 1;
     return RICK_OK;
 }
@@ -346,20 +560,27 @@ int rick_cols12_fft(rick_plan_t* p, int n_planes)
     return RICK_OK;
 }
 
-// strips [strip_begin, strip_end) only (columns 2 strip_begin .. 2 strip_end - 1 of the image); the
-// whole image is strips 0 .. 2047.  rick_image_host launches the pass in a few parts (each a whole
-// number of rounds of the persistent grid) so that the device -> host copy of one part runs under the
-// next part's kernel.
+// units [strip_begin, strip_end) only.  N = 4096: a unit is a strip of two columns (2048 units); N = 8192: one
+// column (8192 units).  rick_image_host launches the pass in a few parts (each a whole number of rounds of the
+// persistent grid) so that the device -> host copy of one part runs under the next part's kernel.
 int rick_cols12_wcorrect(rick_plan_t* p, int img, int z_first, int n_planes, double* image, int accumulate,
                          int fuse_taper, int strip_begin, int strip_end, int slot_first)
 {
     if (strip_end <= strip_begin) return RICK_OK;
     const CUtensorMap tm = *reinterpret_cast<const CUtensorMap*>(p->cols12_tmap_sw);
     const int n = strip_end - strip_begin;
+    if (p->cols13_ok) {
+        RICK_KERNEL(p, RK_COLS_WCORRECT, k_cols13_wcorrect<<<n < p->n_sm ? n : p->n_sm, C12_THREADS, C12_SMEM, p->stream>>>(
+            tm, (const double2*)p->twiddle, n_planes, z_first, p->dl, p->wrange + img, image, accumulate,
+            fuse_taper ? p->taper : nullptr, strip_begin, strip_end, slot_first));
+        return RICK_OK;
+    }
     RICK_KERNEL(p, RK_COLS_WCORRECT, k_cols12_wcorrect<<<n < p->n_sm ? n : p->n_sm, C12_THREADS, C12_SMEM, p->stream>>>(
         tm, (const double2*)p->twiddle, n_planes, z_first, p->dl, p->wrange + img, image, accumulate,
         fuse_taper ? p->taper : nullptr, strip_begin, strip_end, slot_first));
     return RICK_OK;
 }
 
-int rick_cols12_strips(void) { return C12_STRIPS; }
+int rick_cols12_strips(const rick_plan_t* p) { return p->cols13_ok ? C13_N : C12_STRIPS; }
+int rick_cols12_unit_cols(const rick_plan_t* p) { return p->cols13_ok ? 1 : C12_WC; }
+int rick_cols_fused(const rick_plan_t* p) { return p->cols12_ok || p->cols13_ok; }

@@ -428,12 +428,13 @@ static int transform_and_correct(rick_plan_t* p, int img, int z0, int nb, double
                                  bool* host_done)
 {
     int rc;
-    if (p->cols12_ok) {   // column pass fused with the w-correction: the transformed planes are never written
+    if (rick_cols_fused(p)) {   // column pass fused with the w-correction: the transformed planes are never written
         if ((rc = rick_fft_rows(p, img * p->Nw + z0, nb))) return rc;
-        const int strips = rick_cols12_strips();
+        const int strips = rick_cols12_strips(p), ucols = rick_cols12_unit_cols(p);
         if (host_out && last && !p->d.cube) {
             // whole rounds of the persistent grid per part: 4 + 4 + 3 + rest rounds of n_sm strips
-            const int rounds[4] = {4, 4, 3, 1 << 20};
+            const int r4 = (strips / p->n_sm + 3) / 4;
+            const int rounds[4] = {r4 > 0 ? r4 : 1, r4 > 0 ? r4 : 1, r4 > 1 ? r4 - 1 : 1, 1 << 20};
             int s0 = 0;
             for (int k = 0; k < 4 && s0 < strips; ++k) {
                 long long s1 = (long long)s0 + (long long)rounds[k] * p->n_sm;
@@ -441,7 +442,7 @@ static int transform_and_correct(rick_plan_t* p, int img, int z0, int nb, double
                 if ((rc = rick_cols12_wcorrect(p, img, z0, nb, dst, z0 > 0, last, s0, (int)s1))) return rc;
                 RICK_CUDA(p, cudaEventRecord(p->ev_part, p->stream));
                 RICK_CUDA(p, cudaStreamWaitEvent(p->stream3, p->ev_part, 0));
-                const size_t c0 = 2 * (size_t)s0, nc = 2 * (size_t)(s1 - s0);
+                const size_t c0 = (size_t)ucols * (size_t)s0, nc = (size_t)ucols * (size_t)(s1 - s0);
                 RICK_CUDA(p, cudaMemcpy2DAsync(host_out + c0, sizeof(double) * p->N, dst + c0, sizeof(double) * p->N,
                                                sizeof(double) * nc, (size_t)p->N, cudaMemcpyDeviceToHost, p->stream3));
                 s0 = (int)s1;
@@ -505,18 +506,18 @@ static int image_impl(rick_plan_t* p, const void* vis, int32_t vis_dtype, const 
         for (int img0 = 0; img0 < p->n_img; img0 += p->img_batch) {
             const int kk = p->n_img - img0 < p->img_batch ? p->n_img - img0 : p->img_batch;
             const int pf = img0 * p->Nw, ns = kk * p->Nw;
-            if ((rc = rick_zero_sparse(p, pf, ns, !p->cols12_ok && two_pass))) return rc;
+            if ((rc = rick_zero_sparse(p, pf, ns, two_pass))) return rc;
             if ((rc = rick_mark_dirty(p, pf, ns))) return rc;
             if ((rc = rick_grid_planes(p, vis, vis_dtype, uvw_m, weights, pf, ns))) return rc;
             if ((rc = rick_fft_rows(p, pf, ns))) return rc;
-            if (!p->cols12_ok) {
+            if (!rick_cols_fused(p)) {
                 if (two_pass) rc = rick_fft_cols2(p, pf, ns);
                 else rc = rick_fft_cols(p, ns);
                 if (rc) return rc;
             }
             for (int j = 0; j < kk; ++j) {
                 double* dst = image_out + (size_t)(img0 + j) * NN;
-                if (p->cols12_ok) rc = rick_cols12_wcorrect(p, img0 + j, 0, p->Nw, dst, 0, 1, 0, rick_cols12_strips(), j * p->Nw);
+                if (rick_cols_fused(p)) rc = rick_cols12_wcorrect(p, img0 + j, 0, p->Nw, dst, 0, 1, 0, rick_cols12_strips(p), j * p->Nw);
                 else if (two_pass) rc = rick_cols2_wcorrect(p, img0 + j, 0, p->Nw, dst, 0, 1, j * p->Nw);
                 else rc = rick_wcorrect(p, img0 + j, 0, p->Nw, dst, 0, 1, j * p->Nw);
                 if (rc) return rc;
@@ -536,7 +537,7 @@ static int image_impl(rick_plan_t* p, const void* vis, int32_t vis_dtype, const 
             const int nb = p->Nw - z0 < p->batch ? p->Nw - z0 : p->batch;
             const int last = z0 + nb >= p->Nw;
             // (the two-pass column transform reads occupied rows only: stale rows need no clearing)
-            if ((rc = rick_zero_sparse(p, img * p->Nw + z0, nb, !p->cols12_ok && rick_cols2_on(p)))) return rc;
+            if ((rc = rick_zero_sparse(p, img * p->Nw + z0, nb, rick_cols2_on(p)))) return rc;
             if ((rc = rick_mark_dirty(p, img * p->Nw + z0, nb))) return rc;
             if ((rc = rick_grid_planes(p, vis, vis_dtype, uvw_m, weights, img * p->Nw + z0, nb))) return rc;
             if ((rc = transform_and_correct(p, img, z0, nb, dst, last, host_out, &host_done))) return rc;
