@@ -101,6 +101,18 @@ def index(uvw_m, freq_hz, N, Nw, S, dl, B, cube=0, w_min=float("nan"), w_max=flo
     return out
 
 
+def fold_w(uvw_m, vis):
+    """Reading R24: rows with w < 0 -> (-u, -v, -w) and conjugated visibilities.  Returns fresh arrays
+    (uvw [R][3] float64, vis [R][C] complex128) and the number of rows folded."""
+    uvw = np.array(uvw_m, dtype=np.float64, order="C", copy=True)
+    v = np.array(np.asarray(vis).astype(np.complex128), order="C", copy=True).reshape(uvw.shape[0], -1)
+    L = lib()
+    L.rko_fold_w.restype = C.c_int64
+    n = L.rko_fold_w(C.c_int64(uvw.shape[0]), C.c_int32(v.shape[1]), _ptr(uvw, C.c_double),
+                     _ptr(v.view(np.float64), C.c_double))
+    return uvw, v, int(n)
+
+
 def sort(key) -> np.ndarray:
     key = np.ascontiguousarray(key, dtype=np.uint64)
     perm = np.empty(key.shape[0], np.uint32)
@@ -145,9 +157,12 @@ def gridcorrect(image, S, beta) -> np.ndarray:
 
 
 def image(uvw_m, freq_hz, vis, wgt, N, Nw, S, dl, beta=0.0, B=16, cube=0,
-          w_min=float("nan"), w_max=float("nan"), stages=15, want_stacks=False, want_raw=False):
+          w_min=float("nan"), w_max=float("nan"), stages=15, want_stacks=False, want_raw=False, fold=False):
     """Whole path a0..a6 (plane-streamed).  Returns dict(image [n_img][N][N] (squeezed when
-    n_img == 1), stats, timings, and optionally stack_grid / stack_fft / raw_image)."""
+    n_img == 1), stats, timings, and optionally stack_grid / stack_fft / raw_image).
+    fold: reading R24, the rows with w < 0 are folded onto w > 0 first (fold_w)."""
+    if fold:
+        uvw_m, vis, _ = fold_w(uvw_m, vis)
     uvw = np.ascontiguousarray(uvw_m, dtype=np.float64)
     fr = np.ascontiguousarray(freq_hz, dtype=np.float64)
     R, Cn = uvw.shape[0], fr.shape[0]

@@ -200,6 +200,32 @@ int rko_index(int64_t n_rows, int32_t n_chan, const double *uvw_m, const double 
     return 0;
 }
 
+/* Reading R24 (not in the paper): conjugate-symmetry FOLDING of the
+ * rows with w < 0.  A real sky gives V(-u,-v,-w) = conj V(u,v,w) (Eq. 1), and the dirty
+ * image keeps only the real part (R13), so replacing a row (u,v,w) with w < 0 by (-u,-v,-w) and the
+ * visibilities of that row by their conjugates changes no term of the direct sum
+ *   Re[ V e^{+2 pi i (u l + v m + w (n-1))} ] = Re[ conj(V) e^{-2 pi i (...)} ],
+ * while every w becomes >= 0: the w range the N_w planes have to cover halves.  Applied to the inputs
+ * IN PLACE, before step 1; everything after it is the unchanged path.  uvw_m [R][3] metres, vis [R][C]
+ * complex128 interleaved.  A row with w == 0 (either sign) or a non-finite w is left alone.
+ * Returns the number of rows folded. */
+int64_t rko_fold_w(int64_t n_rows, int32_t n_chan, double *uvw_m, double *vis)
+{
+    int64_t n = 0;
+    for (int64_t r = 0; r < n_rows; ++r) {
+        if (!(uvw_m[3 * r + 2] < 0.0)) continue;
+        uvw_m[3 * r + 0] = -uvw_m[3 * r + 0];
+        uvw_m[3 * r + 1] = -uvw_m[3 * r + 1];
+        uvw_m[3 * r + 2] = -uvw_m[3 * r + 2];
+        for (int32_t c = 0; c < n_chan; ++c) {
+            double *v = vis + 2 * (r * (int64_t)n_chan + c);
+            v[1] = -v[1];
+        }
+        ++n;
+    }
+    return n;
+}
+
 /* Stable sort by key == sort by (key, original index): perm[q] = index of the
  * visibility at sorted position q. */
 typedef struct { uint64_t key; uint64_t idx; } rko_pair;
