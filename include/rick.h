@@ -77,9 +77,26 @@ typedef struct {
     int32_t tile;        /* uv-tile edge B in cells (power of two, 8..32); 0 -> 16              */
     int32_t plane_batch; /* w-planes resident at once; 0 -> all N_w                             */
     int32_t cube;        /* 0: all channels into one image; 1: one image per channel (R16)      */
-    int32_t reserved;    /* must be 0                                                           */
+    int32_t flags;       /* RICK_FLAG_* bits, others must be 0                                  */
     double  w_min, w_max; /* wavelengths; NaN -> derived from the data in rick_grid (R4)        */
+    int32_t z_begin;     /* w-plane SHARD: this plan owns  */
+    int32_t z_count;     /* the planes z_begin .. z_begin + z_count - 1 of the n_wplanes; z_count = 0 ->
+                          * all of them (z_begin must be 0).  The w range and the plane of every visibility
+                          * are those of the whole problem; visibilities of other planes are skipped (not
+                          * counted), off-grid ones are counted by the shard with z_begin = 0 only, so the
+                          * statistics of the shards add up.  The image of a shard is its planes' share of
+                          * the sum (a5), taper applied (a6 is linear): the shards' images ADD UP to the
+                          * image of the whole problem (one reduction over the ranks).  The resident stack
+                          * holds min(plane_batch, z_count) planes.  cube = 1 shards by channels instead
+                          * (disjoint channel lists, nothing to reduce): z_count must be 0.        */
 } rick_plan_desc;
+
+/* flags */
+enum { RICK_FLAG_FOLD_W = 1 };  /* reading R24: rows with w < 0 are imaged as (-u,-v,-w)
+                                 * with conjugated visibilities (V(-u,-v,-w) = conj V, Eq. 1; the
+                                 * image keeps the real part only, R13): every w >= 0, the planes cover half the
+                                 * range.  Same direct sum; the w-stacked image differs from the unfolded one
+                                 * within the w-quantisation error (it is the more accurate one).        */
 
 typedef struct {
     int64_t n_vis;       /* M of the last rick_grid / rick_image                                */
@@ -163,6 +180,20 @@ int rick_image_host(rick_plan_t* p, const void* vis_host, int32_t vis_dtype, con
 int rick_image_stream_host(rick_plan_t* p, const void* vis_host, int32_t vis_dtype, const double* uvw_m_host,
                            const float* weights_host, const double* chan_freq_hz, int32_t n_chan,
                            int64_t n_rows, int64_t rows_per_chunk, double* image_out_host);
+
+/* Histogram of the w-planes ("histogram-based balancing"): runs a0 and the
+ * index step over all visibilities and counts the on-grid ones per plane of the WHOLE problem (the plan's
+ * shard is ignored, RICK_FLAG_FOLD_W is honoured).  uvw_m device [R][3]; chan_freq_hz HOST [C];
+ * hist_host HOST [n_wplanes] int64.  cube = 0 only (RICK_ERR_STATE).  SYNCHRONISES the stream. */
+int rick_plane_histogram(rick_plan_t* p, const double* uvw_m, const double* chan_freq_hz, int32_t n_chan,
+                         int64_t n_rows, int64_t* hist_host);
+
+/* Host-only arithmetic (no device, no plan): cut n_wplanes planes into n_parts CONTIGUOUS ranges whose largest
+ * cost is minimal, cost(range) = sum over its planes of (hist[z] + plane_cost) -- hist[z] visibilities to sort
+ * and grid, plane_cost = what one plane's FFT + correction costs, in visibilities (>= 0).  bounds: [n_parts + 1],
+ * range r = planes bounds[r] .. bounds[r+1] - 1; every range holds at least one plane when
+ * n_parts <= n_wplanes, else the trailing ranges are empty.  Returns RICK_ERR_INVALID on bad arguments. */
+int rick_partition_planes(const int64_t* hist, int32_t n_wplanes, int32_t n_parts, double plane_cost, int32_t* bounds);
 
 /* Copy of the plan's image ([N][N] double) into dst_device (cube = 0 only). */
 int rick_get_image(rick_plan_t* p, double* dst_device);

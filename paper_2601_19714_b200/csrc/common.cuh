@@ -31,6 +31,8 @@ struct DevCounters {
 struct rick_plan_s {
     rick_plan_desc d;
     int N, Nw, S, h, B, T, log2N, log2B;
+    int Nw_total, z0;        // the whole problem's planes and this plan's first one (Nw = planes of this shard)
+    int fold;                // RICK_FLAG_FOLD_W
     int f32;                 // grid precision
     int batch;               // resident planes
     double beta, dl, inv_du;
@@ -163,6 +165,7 @@ int rick_tables_build(rick_plan_t* p);                                   // tabl
 #define RICK_SORT_OCC_ACCUM 2
 int rick_index_sort(rick_plan_t* p, const double* uvw_m, const float* weights, int flags = 0);   // index_sort.cu
 int rick_wrange_all(rick_plan_t* p, const double* uvw_m, int64_t n_rows);                         // index_sort.cu
+int rick_plane_hist(rick_plan_t* p, const double* uvw_m, unsigned long long* hist_dev);          // index_sort.cu
 int rick_zero_dirty(rick_plan_t* p, int n_slots, cudaStream_t st);        // grid.cu: zero the dirty rows of slots 0..n_slots-1
 // grid.cu: occupied rows by tile; stale rows whole unless keep_stale (the two-pass column transform never reads
 // a row that is not occupied, so rick_image leaves such rows dirty instead of clearing them)

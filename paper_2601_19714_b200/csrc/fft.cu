@@ -393,7 +393,7 @@ static int launch_cols_b_wcorrect(rick_plan_t* p, int img, int z_first, int n_pl
     if (n_col16 <= 0) return RICK_OK;
     const size_t n_threads = (size_t)n_col16 * 16 * (N / 16) * 2;     // a multiple of 256
     RICK_KERNEL(p, RK_WCORRECT, k_cols_b_wcorrect<T, LOG2N><<<(unsigned int)(n_threads / 256), 256, 0, p->stream>>>(
-        (const C*)p->stack + (size_t)slot_first * N * N, n_planes, z_first, p->dl, p->wrange + img, image, accumulate,
+        (const C*)p->stack + (size_t)slot_first * N * N, n_planes, p->z0 + z_first, p->dl, p->wrange + img, image, accumulate,
         fuse_taper ? p->taper : nullptr, col_begin, n_col16));
     return RICK_OK;
 }

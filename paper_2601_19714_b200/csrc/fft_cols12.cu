@@ -571,12 +571,12 @@ int rick_cols12_wcorrect(rick_plan_t* p, int img, int z_first, int n_planes, dou
     const int n = strip_end - strip_begin;
     if (p->cols13_ok) {
         RICK_KERNEL(p, RK_COLS_WCORRECT, k_cols13_wcorrect<<<n < p->n_sm ? n : p->n_sm, C12_THREADS, C12_SMEM, p->stream>>>(
-            tm, (const double2*)p->twiddle, n_planes, z_first, p->dl, p->wrange + img, image, accumulate,
+            tm, (const double2*)p->twiddle, n_planes, p->z0 + z_first, p->dl, p->wrange + img, image, accumulate,
             fuse_taper ? p->taper : nullptr, strip_begin, strip_end, slot_first));
         return RICK_OK;
     }
     RICK_KERNEL(p, RK_COLS_WCORRECT, k_cols12_wcorrect<<<n < p->n_sm ? n : p->n_sm, C12_THREADS, C12_SMEM, p->stream>>>(
-        tm, (const double2*)p->twiddle, n_planes, z_first, p->dl, p->wrange + img, image, accumulate,
+        tm, (const double2*)p->twiddle, n_planes, p->z0 + z_first, p->dl, p->wrange + img, image, accumulate,
         fuse_taper ? p->taper : nullptr, strip_begin, strip_end, slot_first));
     return RICK_OK;
 }

@@ -45,6 +45,7 @@ struct GridParams {
     void* stack;
     int N, h, B, log2B, T, TWp, TH, C;
     int vis_c128;
+    int fold;                            // RICK_FLAG_FOLD_W: rows with w < 0 are gridded at (-u, -v) with conj V (R24)
     double inv_du;
     unsigned int* chunk_counter;
 };
@@ -261,7 +262,7 @@ __global__ void __launch_bounds__(GRID_WARPS * 32, 2) k_grid(const __grid_consta
     // inputs of one visibility, loaded one batch ahead of their use
     struct VisIn {
         u64 key;
-        double um, vm, s, vr, vi;      // vr, vi: raw value as loaded (complex128), else see raw
+        double um, vm, wm, s, vr, vi;  // vr, vi: raw value as loaded (complex128), else see raw
         float2 raw;                    // complex64 as loaded
         float om;                      // weight as loaded
     };
@@ -277,6 +278,7 @@ __global__ void __launch_bounds__(GRID_WARPS * 32, 2) k_grid(const __grid_consta
         in.s = P.chan_scale[c];
         in.um = P.uvw[3ull * r + 0];
         in.vm = P.uvw[3ull * r + 1];
+        in.wm = P.fold ? P.uvw[3ull * r + 2] : 0.0;
         if (P.vis_c128) {
             const double2 v = reinterpret_cast<const double2*>(P.vis)[idx];
             in.vr = v.x;
@@ -291,6 +293,11 @@ __global__ void __launch_bounds__(GRID_WARPS * 32, 2) k_grid(const __grid_consta
         if (!P.vis_c128) {
             in.vr = (double)in.raw.x;
             in.vi = (double)in.raw.y;
+        }
+        if (in.wm < 0.0) {              // folded row (R24): (u, v) -> (-u, -v), V -> conj V
+            in.um = -in.um;
+            in.vm = -in.vm;
+            in.vi = -in.vi;
         }
         if (P.wgt) {
             const double om = (double)in.om;
@@ -602,6 +609,7 @@ int rick_grid_planes(rick_plan_t* p, const void* vis, int vis_dtype, const doubl
     P.TWp = grid_pitch(p->B, p->S);
     P.C = p->C;
     P.vis_c128 = vis_dtype == RICK_VIS_C128;
+    P.fold = p->fold;
     P.inv_du = p->inv_du;
     P.chunk_counter = &p->counters->grid_chunk;
     if (p->M == 0) return RICK_OK;

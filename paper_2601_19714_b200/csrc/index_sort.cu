@@ -29,13 +29,14 @@ __global__ void k_counters_reset(DevCounters* c)
     c->grid_chunk = 0u;      // (c->error is sticky: cleared at plan creation only)
 }
 
-__global__ void k_wrange_rows(const double* __restrict__ uvw, long long R, DevCounters* c)
+__global__ void k_wrange_rows(const double* __restrict__ uvw, long long R, DevCounters* c, int fold)
 {
     unsigned long long lo = 0xFFFFFFFFFFFFFFFFull, hi = 0ull;
     for (long long r = blockIdx.x * (long long)blockDim.x + threadIdx.x; r < R;
          r += (long long)gridDim.x * blockDim.x) {
-        const double w = uvw[3 * r + 2];
+        double w = uvw[3 * r + 2];
         if (!isfinite(w)) continue;                 // R23: a non-finite w takes no part in the range
+        if (fold) w = fabs(w);                      // R24: rows with w < 0 are imaged at -w
         unsigned long long e = rick_ord_encode(w);
         lo = e < lo ? e : lo;
         hi = e > hi ? e : hi;
@@ -97,6 +98,67 @@ struct RadixPlan {
     unsigned int mask[RS_MAXPASS];
 };
 
+// Index arithmetic of one visibility (DESIGN.md section 3 steps 2, 3; R24 fold first): centre cell, plane of the WHOLE
+// problem, on-grid flag.  Each operation individually rounded, in the normative order.
+__device__ __forceinline__ bool vis_index(double um, double vm, double wm, const double s, const WRange& wr, const int N,
+                                          const int Nw_total, const int h, const double inv_du, const int fold, int& iu,
+                                          int& iv, int& ip)
+{
+    if (fold && wm < 0.0) {
+        um = -um;
+        vm = -vm;
+        wm = -wm;
+    }
+    const double shift = (double)(N / 2) + 0.5;
+    const double xu = __dmul_rn(__dmul_rn(um, s), inv_du);
+    const double xv = __dmul_rn(__dmul_rn(vm, s), inv_du);
+    // on-grid test on the doubles, before any cast: floor(x) - h >= 0 <=> x >= h and
+    // floor(x) + h <= N-1 <=> x < N-h for integer h, and both are false for NaN / inf (R23: a
+    // visibility with a non-finite u, v or w is dropped; (int)floor() of such a value
+    // saturated and could pass the integer test)
+    const double su = __dadd_rn(xu, shift), sv = __dadd_rn(xv, shift);
+    const double wl = __dmul_rn(wm, s);
+    const double lo_ok = (double)h, hi_ok = (double)(N - h);
+    const bool ok = su >= lo_ok && su < hi_ok && sv >= lo_ok && sv < hi_ok && isfinite(wl);
+    iu = ok ? (int)floor(su) : 0;
+    iv = ok ? (int)floor(sv) : 0;
+    double fp = ok ? floor(__dmul_rn(__dsub_rn(wl, wr.w_min), wr.inv_dw)) : 0.0;
+    fp = fp > (double)(Nw_total - 1) ? (double)(Nw_total - 1) : fp;
+    fp = fp >= 0.0 ? fp : 0.0;
+    ip = (int)fp;
+    return ok;
+}
+
+// Per-plane counts of the on-grid visibilities of the whole problem (rick_plane_histogram; cube = 0).
+__global__ void __launch_bounds__(256)
+k_plane_hist(const double* __restrict__ uvw, const double* __restrict__ chan_scale, const WRange* __restrict__ wrange,
+             unsigned int M, unsigned int C, int N, int Nw_total, int h, double inv_du, int fold,
+             unsigned long long* __restrict__ hist)
+{
+    extern __shared__ unsigned int s_cnt[];          // [Nw_total] when it fits (<= 8192 planes), else global atomics
+    const bool use_s = Nw_total <= 8192;
+    if (use_s) {
+        for (int i = threadIdx.x; i < Nw_total; i += blockDim.x) s_cnt[i] = 0u;
+        __syncthreads();
+    }
+    const WRange wr = wrange[0];
+    for (unsigned long long kk0 = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; kk0 < M;
+         kk0 += (unsigned long long)gridDim.x * blockDim.x) {
+        const unsigned int k = (unsigned int)kk0;
+        const unsigned int r = k / C, c = k - r * C;
+        int iu, iv, ip;
+        if (!vis_index(uvw[3ull * r + 0], uvw[3ull * r + 1], uvw[3ull * r + 2], chan_scale[c], wr, N, Nw_total, h, inv_du,
+                       fold, iu, iv, ip))
+            continue;
+        if (use_s) atomicAdd(&s_cnt[ip], 1u); else atomicAdd(&hist[ip], 1ull);
+    }
+    if (use_s) {
+        __syncthreads();
+        for (int i = threadIdx.x; i < Nw_total; i += blockDim.x)
+            if (s_cnt[i]) atomicAdd(&hist[i], (unsigned long long)s_cnt[i]);
+    }
+}
+
 // ------------------------------------------------------------------------------------------
 // a1: one thread per visibility k = r*C + c.  Writes the sort item (key << idx_bits) | k.
 // ------------------------------------------------------------------------------------------
@@ -106,7 +168,7 @@ k_index_key(const double* __restrict__ uvw, const float* __restrict__ wgt,
             unsigned int M, unsigned int C, int N, int Nw, int h, int log2B, int T, int cube,
             double inv_du, int idx_bits, unsigned long long key_dropped,
             unsigned long long* __restrict__ items, DevCounters* cnt, RadixPlan rp,
-            unsigned int* __restrict__ ghist)
+            unsigned int* __restrict__ ghist, int fold, int z0, int Nw_total)
 {
     // digit histograms of ALL radix passes (they do not depend on the order of the items), so that
     // every pass is one read + one write of the items (k_radix_onesweep)
@@ -117,42 +179,28 @@ k_index_key(const double* __restrict__ uvw, const float* __restrict__ wgt,
     // atomics per warp made this kernel atomic-bound)
     unsigned int on = 0, off = 0;
     double sw = 0.0;
-    const double shift = (double)(N / 2) + 0.5;
     const int Bm = (1 << log2B) - 1;
     for (unsigned long long kk0 = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; kk0 < M;
          kk0 += (unsigned long long)gridDim.x * blockDim.x) {
         const unsigned int k = (unsigned int)kk0;
         const unsigned int r = k / C, c = k - r * C;
-        const double s = chan_scale[c];
-        const double um = uvw[3ull * r + 0], vm = uvw[3ull * r + 1], wm = uvw[3ull * r + 2];
-        const double xu = __dmul_rn(__dmul_rn(um, s), inv_du);
-        const double xv = __dmul_rn(__dmul_rn(vm, s), inv_du);
-        // on-grid test on the doubles, before any cast: floor(x) - h >= 0 <=> x >= h and
-        // floor(x) + h <= N-1 <=> x < N-h for integer h, and both are false for NaN / inf (R23: a
-        // visibility with a non-finite u, v or w is dropped; (int)floor() of such a value
-        // saturated and could pass the integer test)
-        const double su = __dadd_rn(xu, shift), sv = __dadd_rn(xv, shift);
-        const double wl = __dmul_rn(wm, s);
-        const double lo_ok = (double)h, hi_ok = (double)(N - h);
-        const bool ok = su >= lo_ok && su < hi_ok && sv >= lo_ok && sv < hi_ok && isfinite(wl);
-        const int iu = ok ? (int)floor(su) : 0;
-        const int iv = ok ? (int)floor(sv) : 0;
         const int img = cube ? (int)c : 0;
-        const WRange wr = wrange[img];
-        double fp = ok ? floor(__dmul_rn(__dsub_rn(wl, wr.w_min), wr.inv_dw)) : 0.0;
-        fp = fp > (double)(Nw - 1) ? (double)(Nw - 1) : fp;
-        fp = fp >= 0.0 ? fp : 0.0;
-        const int ip = (int)fp;
+        int iu, iv, ipg;
+        const bool ok = vis_index(uvw[3ull * r + 0], uvw[3ull * r + 1], uvw[3ull * r + 2], chan_scale[c], wrange[img], N,
+                                  Nw_total, h, inv_du, fold, iu, iv, ipg);
+        // this plan's shard of the planes: z0 .. z0 + Nw - 1 (the whole range unless the plan is a shard)
+        const int ip = ipg - z0;
+        const bool mine = ip >= 0 && ip < Nw;
         unsigned long long key = key_dropped;
-        if (ok) {
+        if (ok && mine) {
             unsigned long long kk = (unsigned long long)img * (unsigned)Nw + (unsigned)ip;
             kk = (kk * (unsigned)T + (unsigned)(iv >> log2B)) * (unsigned)T + (unsigned)(iu >> log2B);
             kk = (((kk << log2B) + (unsigned)(iv & Bm)) << log2B) + (unsigned)(iu & Bm);
             key = kk;
             on++;
             sw += wgt ? (double)wgt[k] : 1.0;
-        } else {
-            off++;
+        } else if (!ok && z0 == 0) {
+            off++;                  // off-grid visibilities are counted once, by the shard that owns plane 0
         }
         items[k] = (key << idx_bits) | (unsigned long long)k;
 #pragma unroll
@@ -464,11 +512,29 @@ int rick_wrange_all(rick_plan_t* p, const double* uvw_m, int64_t n_rows)
     if (n_rows > 0) {
         int nb = (int)((n_rows + 255) / 256);
         if (nb > p->n_sm * 8) nb = p->n_sm * 8;
-        RICK_KERNEL(p, RK_WRANGE, k_wrange_rows<<<nb, 256, 0, st>>>(uvw_m, (long long)n_rows, p->counters));
+        RICK_KERNEL(p, RK_WRANGE, k_wrange_rows<<<nb, 256, 0, st>>>(uvw_m, (long long)n_rows, p->counters, p->fold));
     }
     RICK_KERNEL(p, RK_WRANGE, k_wrange_finish<<<(p->n_img + 127) / 128, 128, 0, st>>>(p->counters, p->chan_scale, p->C, p->d.cube,
-                                                          p->Nw, p->d.w_min, p->d.w_max,
+                                                          p->Nw_total, p->d.w_min, p->d.w_max,
                                                           (long long)n_rows, p->wrange));
+    return RICK_OK;
+}
+
+// a0 + per-plane counts of the whole problem into hist_dev[Nw_total] (cleared here)
+int rick_plane_hist(rick_plan_t* p, const double* uvw_m, unsigned long long* hist_dev)
+{
+    cudaStream_t st = p->stream;
+    const int rc = rick_wrange_all(p, uvw_m, p->R);
+    if (rc) return rc;
+    RICK_CUDA(p, cudaMemsetAsync(hist_dev, 0, sizeof(unsigned long long) * (size_t)p->Nw_total, st));
+    const unsigned int M = (unsigned int)p->M;
+    if (M > 0) {
+        unsigned int nb = (M + 255) / 256;
+        if (nb > (unsigned)p->n_sm * 8u) nb = (unsigned)p->n_sm * 8u;
+        const size_t sm = p->Nw_total <= 8192 ? sizeof(unsigned int) * (size_t)p->Nw_total : 0;
+        RICK_KERNEL(p, RK_INDEX_KEY, k_plane_hist<<<nb, 256, sm, st>>>(uvw_m, p->chan_scale, p->wrange, M, (unsigned)p->C, p->N,
+                                                                      p->Nw_total, p->h, p->inv_du, p->fold, hist_dev));
+    }
     return RICK_OK;
 }
 
@@ -521,7 +587,7 @@ int rick_index_sort(rick_plan_t* p, const double* uvw_m, const float* weights, i
             RICK_KERNEL(p, RK_INDEX_KEY, k_index_key<<<nb, 256, 0, st>>>(uvw_m, weights, p->chan_scale, p->wrange, M,
                                                     (unsigned)p->C, p->N, p->Nw, p->h, p->log2B, p->T,
                                                     p->d.cube, p->inv_du, p->idx_bits, key_dropped, p->items,
-                                                    p->counters, rp, p->os_small));
+                                                    p->counters, rp, p->os_small, p->fold, p->z0, p->Nw_total));
         }
         RICK_KERNEL(p, RK_SCAN, k_digit_bases<<<1, 256, 0, st>>>(p->os_small, rp.npass, p->os_gbase));
         const u64* in = (const u64*)p->items;

@@ -191,9 +191,11 @@ extern "C" int rick_plan(rick_plan_t** out, const rick_plan_desc* d, void* cuda_
     if (d->grid_prec == RICK_GRID_F64 && d->n > 8192) return RICK_ERR_INVALID;
     const int B = d->tile ? d->tile : 16;
     if (!is_pow2(B) || B < 8 || B > 32 || B > d->n) return RICK_ERR_INVALID;
-    if (d->plane_batch < 0 || d->plane_batch > d->n_wplanes) return RICK_ERR_INVALID;
+    if (d->plane_batch < 0 || d->plane_batch > (d->z_count > 0 ? d->z_count : d->n_wplanes)) return RICK_ERR_INVALID;
     if (d->cube != 0 && d->cube != 1) return RICK_ERR_INVALID;
-    if (d->reserved != 0) return RICK_ERR_INVALID;
+    if (d->flags & ~RICK_FLAG_FOLD_W) return RICK_ERR_INVALID;
+    if (d->z_count < 0 || d->z_begin < 0 || (d->z_count == 0 && d->z_begin != 0)) return RICK_ERR_INVALID;
+    if (d->z_count > 0 && ((int64_t)d->z_begin + d->z_count > d->n_wplanes || d->cube)) return RICK_ERR_INVALID;
     if (isinf(d->w_min) || isinf(d->w_max)) return RICK_ERR_INVALID;
     if (d->w_min == d->w_min && d->w_max == d->w_max && d->w_max < d->w_min) return RICK_ERR_INVALID;
     if (d->kb_beta == d->kb_beta && d->kb_beta > 60.0) return RICK_ERR_INVALID;
@@ -222,7 +224,10 @@ extern "C" int rick_plan(rick_plan_t** out, const rick_plan_desc* d, void* cuda_
     if (!p) return RICK_ERR_OOM;
     p->d = *d;
     p->N = d->n;
-    p->Nw = d->n_wplanes;
+    p->Nw_total = d->n_wplanes;
+    p->z0 = d->z_begin;
+    p->Nw = d->z_count > 0 ? d->z_count : d->n_wplanes;
+    p->fold = (d->flags & RICK_FLAG_FOLD_W) ? 1 : 0;
     p->S = d->support;
     p->h = (d->support - 1) / 2;
     p->B = B;
@@ -232,7 +237,7 @@ extern "C" int rick_plan(rick_plan_t** out, const rick_plan_desc* d, void* cuda_
     p->log2B = 0;
     while ((1 << p->log2B) < B) p->log2B++;
     p->f32 = d->grid_prec == RICK_GRID_F32;
-    p->batch = d->plane_batch ? d->plane_batch : d->n_wplanes;
+    p->batch = d->plane_batch ? d->plane_batch : p->Nw;
     // cube with every plane of an image resident: keep up to 8 images' stacks (at most 48 GB) resident
     p->img_batch = 1;
     if (d->cube && p->batch == p->Nw) {
@@ -302,6 +307,8 @@ template <typename Tp> static int grow(rick_plan_t* p, Tp** buf, size_t n)
     return RICK_OK;
 }
 
+static int prepare_scales(rick_plan_t* p, const double* chan_freq_hz, int32_t n_chan);
+
 static int prepare(rick_plan_t* p, const double* chan_freq_hz, int32_t n_chan, int64_t n_rows)
 {
     p->C = n_chan;
@@ -339,6 +346,13 @@ static int prepare(rick_plan_t* p, const double* chan_freq_hz, int32_t n_chan, i
         if ((rc = grow(p, &p->tile_occ, tocc_bytes))) return rc;
         p->tile_occ_cap = tocc_bytes;
     }
+    return prepare_scales(p, chan_freq_hz, n_chan);
+}
+
+// per-channel scales s_c = f_c / c0 on the device (+ room for the w range of every image)
+static int prepare_scales(rick_plan_t* p, const double* chan_freq_hz, int32_t n_chan)
+{
+    int rc;
     if (n_chan > p->chan_cap) {
         if ((rc = grow(p, &p->chan_scale, (size_t)n_chan))) return rc;
         if ((rc = grow(p, &p->wrange, (size_t)n_chan))) return rc;
@@ -713,6 +727,80 @@ extern "C" int rick_image_stream_host(rick_plan_t* p, const void* vis_host, int3
     RICK_CUDA(p, cudaStreamSynchronize(p->stream));
     RICK_CUDA(p, cudaStreamSynchronize(p->stream3));
     return check_device_error(p);
+}
+
+extern "C" int rick_plane_histogram(rick_plan_t* p, const double* uvw_m, const double* chan_freq_hz, int32_t n_chan,
+                                    int64_t n_rows, int64_t* hist_host)
+{
+    RICK_ENTER(p);
+    if (!hist_host) { p->err = "null hist_host"; return RICK_ERR_INVALID; }
+    if (p->d.cube) { p->err = "rick_plane_histogram: cube plans shard by channels"; return RICK_ERR_STATE; }
+    static const float2 dummy_vis = {0.f, 0.f};
+    int rc = check_inputs(p, n_rows > 0 ? (const void*)&dummy_vis : nullptr, RICK_VIS_C64, uvw_m, chan_freq_hz, n_chan, n_rows);
+    if (rc) return rc;
+    if (n_rows > 0 && !aligned16(uvw_m)) { p->err = "device pointer not 16-byte aligned (uvw_m)"; return RICK_ERR_INVALID; }
+    p->state = 0;
+    p->C = n_chan;                  // (no sort scratch: the histogram needs the scales and the w range only)
+    p->R = n_rows;
+    p->M = n_rows * (int64_t)n_chan;
+    p->n_img = 1;
+    if ((rc = prepare_scales(p, chan_freq_hz, n_chan))) return rc;
+    unsigned long long* hd = nullptr;
+    RICK_CUDA(p, cudaMalloc(&hd, sizeof(unsigned long long) * (size_t)p->Nw_total));
+    rc = rick_plane_hist(p, uvw_m, hd);
+    if (rc == RICK_OK) {
+        cudaError_t e = cudaMemcpyAsync(hist_host, hd, sizeof(unsigned long long) * (size_t)p->Nw_total, cudaMemcpyDeviceToHost, p->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(p->stream);
+        if (e != cudaSuccess) { p->err = std::string("rick_plane_histogram: ") + cudaGetErrorString(e); p->failed = RICK_ERR_CUDA; rc = RICK_ERR_CUDA; }
+    }
+    cudaFree(hd);
+    return rc;
+}
+
+// Linear partition: smallest bottleneck by bisection on the bound, greedy feasibility (a range is closed when
+// the next plane would exceed the bound); then the ranges are laid out greedily under the optimal bound, leaving
+// at least one plane for every later part.
+extern "C" int rick_partition_planes(const int64_t* hist, int32_t n_wplanes, int32_t n_parts, double plane_cost, int32_t* bounds)
+{
+    if (!hist || !bounds || n_wplanes < 1 || n_parts < 1 || !(plane_cost >= 0.0)) return RICK_ERR_INVALID;
+    for (int z = 0; z < n_wplanes; ++z)
+        if (hist[z] < 0) return RICK_ERR_INVALID;
+    auto cost = [&](int z) { return (double)hist[z] + plane_cost; };
+    auto parts_needed = [&](double bound) {
+        int parts = 1;
+        double acc = 0.0;
+        for (int z = 0; z < n_wplanes; ++z) {
+            const double c = cost(z);
+            if (acc > 0.0 && acc + c > bound) { ++parts; acc = 0.0; }
+            acc += c;
+        }
+        return parts;
+    };
+    double lo = 0.0, hi = 0.0;
+    for (int z = 0; z < n_wplanes; ++z) { hi += cost(z); if (cost(z) > lo) lo = cost(z); }
+    for (int it = 0; it < 100 && hi - lo > 1e-9 * (hi > 1.0 ? hi : 1.0); ++it) {
+        const double mid = 0.5 * (lo + hi);
+        if (parts_needed(mid) <= n_parts) hi = mid; else lo = mid;
+    }
+    const double bound = hi;
+    int z = 0;
+    bounds[0] = 0;
+    for (int r = 0; r < n_parts; ++r) {
+        double acc = 0.0;
+        int must_leave = n_wplanes - z - 1;                 // one plane for every later part, as far as the planes go
+        if (must_leave < 0) must_leave = 0;
+        if (must_leave > n_parts - 1 - r) must_leave = n_parts - 1 - r;
+        int taken = 0;
+        while (z < n_wplanes - must_leave || (r == n_parts - 1 && z < n_wplanes)) {
+            const double c = cost(z);
+            if (taken > 0 && acc + c > bound && r < n_parts - 1) break;
+            acc += c;
+            ++z;
+            ++taken;
+        }
+        bounds[r + 1] = z;
+    }
+    return RICK_OK;
 }
 
 extern "C" int rick_get_image(rick_plan_t* p, double* dst_device)

@@ -78,10 +78,10 @@ int rick_wcorrect(rick_plan_t* p, int img, int z_first, int n_planes, double* im
     const double* tp = fuse_taper ? p->taper : nullptr;
     if (p->f32) {
         RICK_KERNEL(p, RK_WCORRECT, k_wcorrect<float2><<<blocks, 256, 0, p->stream>>>(
-            (const float2*)p->stack + (size_t)slot_first * p->N * p->N, n_planes, z_first, p->N, p->dl, p->wrange + img, image, accumulate, tp));
+            (const float2*)p->stack + (size_t)slot_first * p->N * p->N, n_planes, p->z0 + z_first, p->N, p->dl, p->wrange + img, image, accumulate, tp));
     } else {
         RICK_KERNEL(p, RK_WCORRECT, k_wcorrect<double2><<<blocks, 256, 0, p->stream>>>(
-            (const double2*)p->stack + (size_t)slot_first * p->N * p->N, n_planes, z_first, p->N, p->dl, p->wrange + img, image, accumulate, tp));
+            (const double2*)p->stack + (size_t)slot_first * p->N * p->N, n_planes, p->z0 + z_first, p->N, p->dl, p->wrange + img, image, accumulate, tp));
     }
     return RICK_OK;
 }

@@ -20,10 +20,11 @@ LIB_PATH = os.path.join(_HERE, "librick_b200.so")
 RICK_OK, RICK_ERR_INVALID, RICK_ERR_STATE, RICK_ERR_CUDA, RICK_ERR_OOM = 0, -1, -2, -3, -4
 RICK_GRID_F64, RICK_GRID_F32 = 0, 1
 RICK_VIS_C64, RICK_VIS_C128 = 0, 1
+RICK_FLAG_FOLD_W = 1
 
 EXPORTS = ["rick_plan", "rick_plan_destroy", "rick_grid", "rick_fft_wplanes",
            "rick_wcorrect_accumulate", "rick_gridcorrect", "rick_image", "rick_image_host",
-           "rick_image_stream_host",
+           "rick_image_stream_host", "rick_plane_histogram", "rick_partition_planes",
            "rick_get_image", "rick_get_stats", "rick_last_error", "rick_debug_items",
            "rick_debug_planes", "rick_version", "rick_profile",
            "rick_profile_read", "rick_kernel_name"]
@@ -33,7 +34,8 @@ class PlanDesc(C.Structure):
     _fields_ = [("n", C.c_int32), ("n_wplanes", C.c_int32), ("support", C.c_int32),
                 ("pixel_rad", C.c_double), ("kb_beta", C.c_double), ("grid_prec", C.c_int32),
                 ("tile", C.c_int32), ("plane_batch", C.c_int32), ("cube", C.c_int32),
-                ("reserved", C.c_int32), ("w_min", C.c_double), ("w_max", C.c_double)]
+                ("flags", C.c_int32), ("w_min", C.c_double), ("w_max", C.c_double),
+                ("z_begin", C.c_int32), ("z_count", C.c_int32)]
 
 
 class Stats(C.Structure):
@@ -71,6 +73,8 @@ def load_library():
     L.rick_image.argtypes = [vp, vp, i32, vp, vp, C.POINTER(C.c_double), i32, i64, vp]
     L.rick_image_host.argtypes = [vp, vp, i32, vp, vp, C.POINTER(C.c_double), i32, i64, vp]
     L.rick_image_stream_host.argtypes = [vp, vp, i32, vp, vp, C.POINTER(C.c_double), i32, i64, i64, vp]
+    L.rick_plane_histogram.argtypes = [vp, vp, C.POINTER(C.c_double), i32, i64, C.POINTER(C.c_int64)]
+    L.rick_partition_planes.argtypes = [C.POINTER(C.c_int64), i32, i32, C.c_double, C.POINTER(i32)]
     L.rick_get_image.argtypes = [vp, vp]
     L.rick_get_stats.argtypes = [vp, C.POINTER(Stats)]
     L.rick_last_error.argtypes = [vp]
@@ -101,14 +105,17 @@ class Plan:
     """rick_plan + the staged calls.  Tensors are torch CUDA tensors unless noted."""
 
     def __init__(self, n, n_wplanes, support, pixel_rad, kb_beta=0.0, grid_prec="f64", tile=0,
-                 plane_batch=0, cube=0, w_min=float("nan"), w_max=float("nan"), stream=None):
+                 plane_batch=0, cube=0, w_min=float("nan"), w_max=float("nan"), stream=None, flags=0,
+                 z_begin=0, z_count=0):
         self._lib = load_library()
         if not torch.cuda.is_available():
             raise RuntimeError("librick_b200 needs a CUDA device (no CPU fallback)")
         self.desc = PlanDesc(int(n), int(n_wplanes), int(support), float(pixel_rad), float(kb_beta),
                              RICK_GRID_F32 if grid_prec in ("f32", RICK_GRID_F32) else RICK_GRID_F64,
-                             int(tile), int(plane_batch), int(cube), 0, float(w_min), float(w_max))
+                             int(tile), int(plane_batch), int(cube), int(flags), float(w_min), float(w_max),
+                             int(z_begin), int(z_count))
         self.n, self.n_wplanes, self.cube = int(n), int(n_wplanes), int(cube)
+        self.n_planes_resident = int(z_count) if z_count else int(n_wplanes)
         self.f32 = self.desc.grid_prec == RICK_GRID_F32
         self.stream = stream if stream is not None else torch.cuda.current_stream()
         self._h = C.c_void_p()
@@ -202,6 +209,16 @@ class Plan:
             C.c_void_p(image_out.data_ptr())))
         return image_out
 
+    def rick_plane_histogram(self, uvw_m, chan_freq_hz) -> np.ndarray:
+        """[n_wplanes] int64: on-grid visibilities per w-plane of the whole problem (synchronises)."""
+        freq = np.ascontiguousarray(chan_freq_hz, dtype=np.float64)
+        hist = np.zeros(self.n_wplanes, np.int64)
+        self._keep = (uvw_m, freq)
+        self._check(self._lib.rick_plane_histogram(self._h, _dev_ptr(uvw_m), freq.ctypes.data_as(C.POINTER(C.c_double)),
+                                                   int(freq.shape[0]), int(uvw_m.shape[0]),
+                                                   hist.ctypes.data_as(C.POINTER(C.c_int64))))
+        return hist
+
     def rick_get_image(self) -> torch.Tensor:
         out = torch.empty((self.n, self.n), dtype=torch.float64, device="cuda")
         self._check(self._lib.rick_get_image(self._h, _dev_ptr(out)))
@@ -266,8 +283,9 @@ class Plan:
 
     def debug_planes(self) -> Optional[torch.Tensor]:
         dt = torch.complex64 if self.f32 else torch.complex128
-        nb = (8 if self.f32 else 16) * self.n_wplanes * self.n * self.n
-        return self._copy_from(self._lib.rick_debug_planes(self._h), nb, dt, (self.n_wplanes, self.n, self.n))
+        nz = self.n_planes_resident
+        nb = (8 if self.f32 else 16) * nz * self.n * self.n
+        return self._copy_from(self._lib.rick_debug_planes(self._h), nb, dt, (nz, self.n, self.n))
 
     def destroy(self):
         if getattr(self, "_h", None) and self._h.value:
@@ -279,6 +297,18 @@ class Plan:
             self.destroy()
         except Exception:
             pass
+
+
+def rick_partition_planes(hist, n_parts: int, plane_cost: float) -> np.ndarray:
+    """[n_parts + 1] int32 bounds of contiguous plane ranges with the smallest largest cost (host arithmetic of
+    the library; needs no device)."""
+    h = np.ascontiguousarray(hist, dtype=np.int64)
+    bounds = np.zeros(int(n_parts) + 1, np.int32)
+    rc = load_library().rick_partition_planes(h.ctypes.data_as(C.POINTER(C.c_int64)), int(h.shape[0]), int(n_parts),
+                                              float(plane_cost), bounds.ctypes.data_as(C.POINTER(C.c_int32)))
+    if rc != RICK_OK:
+        raise RickError(rc, "rick_partition_planes: bad arguments")
+    return bounds
 
 
 def version() -> str:
