@@ -156,14 +156,38 @@ def measure(cfg, args, rank, world, headline):
     from paper_2601_19714_b200 import rick
 
     wl = make_workload(cfg, args, "cuda")
+    shard = None
+    if world > 1:
+        # strong scaling: this rank's share of the ONE problem.  Set-up (untimed, once per visibility set):
+        # the per-plane histogram, the plane bounds, this rank's plan.
+        import dataclasses
+        from paper_2601_19714_b200 import sharded
+        if wl.cube:
+            cb = sharded.channel_bounds(wl.n_chan, world)
+            c0, c1 = int(cb[rank]), max(int(cb[rank + 1]), int(cb[rank]) + 1)
+            wl = dataclasses.replace(wl, freq_hz=wl.freq_hz[c0:c1].copy(), vis=np.ascontiguousarray(wl.vis[:, c0:c1]),
+                                     weights=None if wl.weights is None else np.ascontiguousarray(wl.weights[:, c0:c1]))
+            shard = {"kind": "channels", "bounds": cb.tolist()}
     vis, uvw, wgt = rick.to_device(wl)
-    plan = rick.plan_from_workload(wl)
+    if world > 1 and not wl.cube:
+        sh = sharded.ShardedImager(dict(n=wl.n, n_wplanes=wl.n_wplanes, support=wl.support, pixel_rad=wl.pixel_rad,
+                                        grid_prec=wl.grid_prec, plane_batch=wl.plane_batch), rank, world)
+        bounds = sh.prepare(uvw, wl.freq_hz)
+        shard = {"kind": "w-planes", "bounds": bounds.tolist(), "plane_cost_vis": sh.cost,
+                 "hist_max": int(sh.hist.max()), "hist_min": int(sh.hist.min())}
+        plan = sh.plan
+        if plan is None:
+            raise SystemExit(f"rank {rank}: more ranks than w-planes")
+    else:
+        plan = rick.plan_from_workload(wl)
     image = torch.empty((wl.n_chan, wl.n, wl.n) if wl.cube else (wl.n, wl.n), dtype=torch.float64, device="cuda")
     steps = args.steps if headline else max(1, min(args.steps, args.secondary_steps))
     warmup = max(args.warmup, 3) if headline else 2
 
     def step():
         plan.rick_image(vis, uvw, wgt, wl.freq_hz, image)
+        if world > 1 and not wl.cube:
+            sharded.reduce_image(image, dst=0)          # the one collective of the path: the N x N real image
 
     for _ in range(warmup):
         step()
@@ -185,9 +209,10 @@ def measure(cfg, args, rank, world, headline):
     bu.dist_barrier()
     ms_total = ev0.elapsed_time(ev1)
     launches = plan.rick_get_stats()["n_launches"] - l0
-    agg = bu.aggregate_replicas(wl.n_vis * steps, ms_total, device="cuda")
-    ms_per_step = agg["ms"] / steps
-    value = agg["per_s"] / 1e6
+    n_vis_total = bu.dist_sum(wl.n_vis, "cuda") if (world > 1 and wl.cube) else wl.n_vis     # the whole problem
+    ms_max = bu.dist_max(ms_total, "cuda")              # max over ranks
+    ms_per_step = ms_max / steps
+    value = n_vis_total * steps / (ms_max * 1e-3) / 1e6
 
     # ---- second loop: the library brackets every launch with CUDA events on the stream it launches on
     psteps = max(1, min(steps, 5))
@@ -276,10 +301,24 @@ def measure(cfg, args, rank, world, headline):
         plan.rick_image_host(hv, hu, hw, wl.freq_hz, hout)
     torch.cuda.synchronize()
     e2e_ms = (time.perf_counter() - t0) * 1e3
-    e2e = bu.aggregate_replicas(wl.n_vis * k_e2e, e2e_ms, device="cuda")
+    if world > 1 and not wl.cube:
+        # end to end over the shards: every rank copies the inputs from pinned host memory, images its planes,
+        # the images are reduced, rank 0 reads the result back
+        t0 = time.perf_counter()
+        for _ in range(k_e2e):
+            dv, du = hv.to("cuda", non_blocking=True), hu.to("cuda", non_blocking=True)
+            dw = None if hw is None else hw.to("cuda", non_blocking=True)
+            plan.rick_image(dv, du, dw, wl.freq_hz, image)
+            sharded.reduce_image(image, dst=0)
+            if rank == 0:
+                hout[0].copy_(image, non_blocking=True)
+            torch.cuda.synchronize()
+        e2e_ms = (time.perf_counter() - t0) * 1e3
+    e2e_max = bu.dist_max(e2e_ms, "cuda")
+    e2e = {"ms": e2e_max, "per_s": n_vis_total * k_e2e / (e2e_max * 1e-3)}
     h2d = hv.numel() * hv.element_size() + hu.numel() * 8 + (0 if hw is None else hw.numel() * 4)
     # out-of-core visibilities (rick_image_stream_host): the same host buffers in 8 chunks of rows
-    if headline and not wl.cube and not wl.plane_batch:
+    if headline and world == 1 and not wl.cube and not wl.plane_batch:
         rpc = (wl.n_rows + 7) // 8
         plan.rick_image_stream_host(hv, hu, hw, wl.freq_hz, hout[0], rpc)      # warm (grows the staging)
         torch.cuda.synchronize()
@@ -322,7 +361,8 @@ def measure(cfg, args, rank, world, headline):
            "clocks": clocks,
            "e2e": {"value": e2e["per_s"] / 1e6, "unit": "Mvis/s", "h2d_bytes_per_step": h2d,
                    "d2h_bytes_per_step": nimg * wl.n * wl.n * 8, "ms_per_step": e2e["ms"] / k_e2e, "steps": k_e2e},
-           "gpu_launches": int(launches), "roofline": dom, "rooflines": rooflines, "stages": stages}
+           "gpu_launches": int(launches), "roofline": dom, "rooflines": rooflines, "stages": stages, "shard": shard,
+           "n_vis_total": int(n_vis_total)}
     return rec, wl
 
 
@@ -416,10 +456,12 @@ def main():
     if rank == 0:
         line = {"metric": METRIC, "value": rec["value"], "unit": "Mvis/s", "n_gpus": world, "steps": rec["steps"],
                 "warmup": rec["warmup"], "ms_per_step": rec["ms_per_step"], "higher_is_better": True,
-                "scaling": "weak", "vs_baseline": None, "dtype": rec["dtype"], "data": "synthetic",
-                "config": {"workload": rec["workload"], "n_vis": rec["n_vis"], "grid": rec["grid"],
+                "scaling": "strong" if world > 1 else "weak", "vs_baseline": None, "dtype": rec["dtype"], "data": "synthetic",
+                "config": {"workload": rec["workload"], "n_vis": rec["n_vis_total"], "grid": rec["grid"],
                            "w_planes": rec["w_planes"], "support": rec["support"],
-                           "parallelism": f"replicas x{world}" if world > 1 else "single GPU", "l2": rec["l2"]},
+                           "parallelism": (f"{rec['shard']['kind']} sharded over {world} GPUs, one reduction of the image"
+                                           if world > 1 else "single GPU"),
+                           "shard": rec["shard"], "l2": rec["l2"]},
                 "clocks": rec["clocks"], "e2e": rec["e2e"], "gpu_launches": rec["gpu_launches"],
                 "roofline": rec["roofline"], "rooflines": rec["rooflines"], "cpu_baseline": cpu_baseline,
                 "stages": rec["stages"], "configs": others}
