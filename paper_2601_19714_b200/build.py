@@ -10,7 +10,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "librick_b200.so")
-SOURCES = ["plan.cu", "tables.cu", "index_sort.cu", "grid.cu", "fft.cu", "fft_cols12.cu", "wcorrect.cu"]
+SOURCES = ["plan.cu", "tables.cu", "index_sort.cu", "grid.cu", "fft.cu", "fft_cols12.cu", "fft_cols_sparse.cu", "wcorrect.cu"]
 HEADERS = ["common.cuh", "fft_core.cuh", "sm100_ptx.cuh", os.path.join("..", "..", "include", "rick.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-O2"]

@@ -109,6 +109,14 @@ struct rick_plan_s {
     alignas(64) unsigned char cols12_tmap[128];
     alignas(64) unsigned char cols12_tmap_sw[128];   // same view, 32-byte swizzle (k_cols12_wcorrect)
 
+    // fp32 grid with long columns (fft_cols_sparse.cu): per-plane row lists / bitmaps / prefix sums of the occupied
+    // rows, the largest count (sp_count[Nw]) and the transposed accumulation image
+    int sp_ok;
+    unsigned int *sp_bits, *sp_prefix;
+    unsigned short* sp_list;
+    int* sp_count;
+    double* sp_imageT;
+
     // host-buffer staging for rick_image_host
     void* st_vis; size_t st_vis_cap;
     double* st_uvw; size_t st_uvw_cap;
@@ -185,6 +193,16 @@ int rick_fft_cols2(rick_plan_t* p, int plane_first, int n_planes);
 int rick_cols2_on(const rick_plan_t* p);     // 1 when the two-pass transform applies to this plan (N >= 8192)
 int rick_cols2_wcorrect(rick_plan_t* p, int img, int z_first, int n_planes, double* image, int accumulate,
                         int fuse_taper, int slot_first = 0, int col_begin = 0, int col_end = -1);   // columns [col_begin, col_end), multiples of 16; -1 = N
+// fft_cols_sparse.cu: single fused column pass of the fp32 grid with long columns over the occupied rows only;
+// every launch returns at once on the device when some plane has more than N/2 occupied rows (the two-pass
+// kernels then run: they return at once in the other case -- rick_sparse_maxcount / rick_sparse_cap)
+int rick_sparse_init(rick_plan_t* p);
+void rick_sparse_free(rick_plan_t* p);
+int rick_sparse_prepare(rick_plan_t* p);
+int rick_sparse_wcorrect(rick_plan_t* p, int z_first, int n_planes, int accumulate);
+int rick_sparse_finish(rick_plan_t* p, double* image, int fuse_taper);
+const int* rick_sparse_maxcount(const rick_plan_t* p);
+int rick_sparse_cap(const rick_plan_t* p);
 int rick_cols12_init(rick_plan_t* p);                                    // fft_cols12.cu
 int rick_cols12_fft(rick_plan_t* p, int n_planes);                       // fft_cols12.cu
 int rick_cols12_wcorrect(rick_plan_t* p, int img, int z_first, int n_planes, double* image,

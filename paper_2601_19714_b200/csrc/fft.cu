@@ -205,10 +205,12 @@ template <typename T, int LOG2N> struct Col2Cfg {
 template <typename T, int LOG2N>
 __global__ void __launch_bounds__(Col2Cfg<T, LOG2N>::THREADS, C2_MINB / Col2Cfg<T, LOG2N>::THREADS)
 k_fft_cols_a(typename cplx_of<T>::type* __restrict__ stack, const typename cplx_of<T>::type* __restrict__ tw2,
-             const typename cplx_of<T>::type* __restrict__ twN, const unsigned char* __restrict__ occ)
+             const typename cplx_of<T>::type* __restrict__ twN, const unsigned char* __restrict__ occ,
+             const int* __restrict__ sparse_max, int sparse_cap)
 {
     typedef typename cplx_of<T>::type C;
     typedef Col2Cfg<T, LOG2N> K;
+    if (sparse_max && *sparse_max <= sparse_cap) return;      // the sparse fused pass (fft_cols_sparse.cu) serves this image
     extern __shared__ __align__(16) unsigned char smem_raw[];
     C* sm = reinterpret_cast<C*>(smem_raw);
     constexpr int STRIPS = K::N / K::W;
@@ -255,7 +257,8 @@ template <typename T, int LOG2N> static int launch_cols2(rick_plan_t* p, int pla
     RICK_CUDA(p, cudaFuncSetAttribute(k_fft_cols_a<T, LOG2N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)K::SMEM));
     const unsigned int blocks_a = (unsigned int)((size_t)n_planes * (K::N / K::W) * 16);
     RICK_KERNEL(p, RK_FFT_COLS, k_fft_cols_a<T, LOG2N><<<blocks_a, K::THREADS, K::SMEM, p->stream>>>(
-        (C*)p->stack, (const C*)p->twiddle2, (const C*)p->twiddle, p->row_occ + (size_t)plane_first * p->N));
+        (C*)p->stack, (const C*)p->twiddle2, (const C*)p->twiddle, p->row_occ + (size_t)plane_first * p->N,
+        rick_sparse_maxcount(p), rick_sparse_cap(p)));
     return RICK_OK;
 }
 
@@ -321,10 +324,11 @@ template <typename T, int LOG2N>
 __global__ void __launch_bounds__(256, 2)
 k_cols_b_wcorrect(const typename cplx_of<T>::type* __restrict__ stack, int n_planes, int z_first, double dl,
                   const WRange* __restrict__ wr, double* __restrict__ image, int accumulate,
-                  const double* __restrict__ taper, int col_begin, int n_col16)
+                  const double* __restrict__ taper, int col_begin, int n_col16, const int* __restrict__ sparse_max, int sparse_cap)
 {
     typedef typename cplx_of<T>::type C;
     constexpr int N = 1 << LOG2N, N2 = N / 16;
+    if (sparse_max && *sparse_max <= sparse_cap) return;      // the sparse fused pass serves this image
     // columns col_begin .. col_begin + 16 n_col16 - 1 only (the host-buffer entry launches the pass in parts)
     const size_t gid = (size_t)blockIdx.x * 256 + threadIdx.x;       // < 16 n_col16 * N2 * 2 by construction of the grid
     const int pl = (int)(gid & 15), h = (int)((gid >> 4) & 1);
@@ -394,7 +398,7 @@ static int launch_cols_b_wcorrect(rick_plan_t* p, int img, int z_first, int n_pl
     const size_t n_threads = (size_t)n_col16 * 16 * (N / 16) * 2;     // a multiple of 256
     RICK_KERNEL(p, RK_WCORRECT, k_cols_b_wcorrect<T, LOG2N><<<(unsigned int)(n_threads / 256), 256, 0, p->stream>>>(
         (const C*)p->stack + (size_t)slot_first * N * N, n_planes, p->z0 + z_first, p->dl, p->wrange + img, image, accumulate,
-        fuse_taper ? p->taper : nullptr, col_begin, n_col16));
+        fuse_taper ? p->taper : nullptr, col_begin, n_col16, rick_sparse_maxcount(p), rick_sparse_cap(p)));
     return RICK_OK;
 }
 

@@ -114,6 +114,7 @@ extern "C" int rick_plan_destroy(rick_plan_t* p)
     free_dev(p->os_small); free_dev(p->os_gbase); free_dev(p->os_status); free_dev(p->plane_start); free_dev(p->chan_scale);
     free_dev(p->row_occ); free_dev(p->row_dirty); free_dev(p->tile_occ); free_dev(p->row_list);
     free_dev(p->wrange); free_dev(p->counters);
+    rick_sparse_free(p);
     free_dev(p->st_vis); free_dev(p->st_uvw); free_dev(p->st_wgt); free_dev(p->st_img);
     for (cudaEvent_t e : p->prof_ev) cudaEventDestroy(e);
     if (p->h_scale) cudaFreeHost(p->h_scale);
@@ -175,6 +176,8 @@ static int plan_init(rick_plan_t* p)
     RICK_CUDA(p, cudaMemsetAsync(p->counters, 0, sizeof(DevCounters), p->stream));
     const int rc = rick_tables_build(p);
     if (rc) return rc;
+    const int rc2 = rick_sparse_init(p);
+    if (rc2) return rc2;
     return rick_cols12_init(p);
 }
 
@@ -469,8 +472,18 @@ static int transform_and_correct(rick_plan_t* p, int img, int z0, int nb, double
         const int two_pass = rick_cols2_on(p);
         if (two_pass) {       // long columns: pass A at full line width, pass B fused with the correction
             if ((rc = rick_fft_rows(p, img * p->Nw + z0, nb))) return rc;
+            if (p->sp_ok) {
+                // fp32 grid: one fused pass over the occupied rows only, when every plane of the image has few
+                // enough of them (decided on the device: either these launches or the two-pass ones below return
+                // at once).  It accumulates a transposed image, turned (and tapered) after the last batch.
+                if (z0 == 0 && (rc = rick_sparse_prepare(p))) return rc;
+                if ((rc = rick_sparse_wcorrect(p, z0, nb, z0 > 0))) return rc;
+            }
             if ((rc = rick_fft_cols2(p, img * p->Nw + z0, nb))) return rc;
-            if (host_out && last && !p->d.cube) {
+            if (p->sp_ok) {
+                if ((rc = rick_cols2_wcorrect(p, img, z0, nb, dst, z0 > 0, last))) return rc;
+                if (last && (rc = rick_sparse_finish(p, dst, 1))) return rc;
+            } else if (host_out && last && !p->d.cube) {
                 // four column ranges: the image columns of one part cross to the host under the next part
                 const int step = p->N / 4;
                 for (int c0 = 0; c0 < p->N; c0 += step) {

@@ -434,6 +434,49 @@ def test_long_columns_two_pass(prec, pb, tol):
     assert st["n_gridded"] == o["stats"]["n_gridded"]
 
 
+def test_fp32_long_columns_sparse_and_dense_paths():
+    """fp32 grid, N = 8192: rick_image takes the single fused column pass over the occupied rows when every
+    plane has at most N/2 of them, and the two-pass kernels otherwise -- decided on the device.  Both against
+    the oracle: a sparse case (few time steps), a dense one (coverage over more than half of the rows of a
+    plane), and the dense one in plane batches (the decision must hold for every batch of the image)."""
+    rick = _rick()
+    for name, wl, over in (("sparse", synth.make_config(4, n_times=4, n=8192, n_wplanes=3, n_src=6), dict(plane_batch=2)),
+                           ("dense", synth.make_config(3, n_times=96, n_wplanes=2, n_src=6), {}),
+                           ("dense, batches of 1", synth.make_config(3, n_times=96, n_wplanes=2, n_src=6), dict(plane_batch=1))):
+        wl.grid_prec = "f32"
+        o = _oracle(wl)
+        plan = rick.plan_from_workload(wl, **over)
+        vis, uvw, wgt = rick.to_device(wl)
+        img = plan.rick_image(vis, uvw, wgt, wl.freq_hz).cpu().numpy()
+        st = plan.rick_get_stats()
+        plan.rick_profile(True)
+        img2 = plan.rick_image(vis, uvw, wgt, wl.freq_hz).cpu().numpy()
+        prof = plan.rick_profile_read()
+        plan.rick_profile(False)
+        plan.destroy()
+        idx = oracle.index(wl.uvw_m, wl.freq_hz, wl.n, wl.n_wplanes, wl.support, wl.pixel_rad, 16)
+        keep = idx["key"] != np.uint64(0xFFFFFFFFFFFFFFFF)
+        # occupied rows per plane as the plan counts them: tile rows (16) of the centre cells plus the halo
+        occ_max = 0
+        for z in range(wl.n_wplanes):
+            tv = np.unique(idx["iv"][keep & (idx["ip"] == z)] // 16)
+            rows = np.zeros(wl.n, bool)
+            for t in tv:
+                rows[max(0, t * 16 - 3):min(wl.n, t * 16 + 16 + 3)] = True
+            occ_max = max(occ_max, int(rows.sum()))
+        e = _close(img, o["image"], TOL32, name)
+        _close(img2, o["image"], TOL32, name + " (second call)")
+        print(f"fp32 N=8192 {name}: most occupied plane {occ_max} of {wl.n} rows, rel L2 {e:.2e}; "
+              f"kernel ms: sparse fused {prof['fft_cols_wcorrect'][0]:.3f}, two-pass {prof['fft_cols'][0] + prof['wcorrect'][0]:.3f}")
+        assert (occ_max <= wl.n // 2) == name.startswith("sparse")
+        assert st["n_gridded"] == o["stats"]["n_gridded"]
+        # the path that was NOT taken returned at once
+        if name.startswith("sparse"):
+            assert prof["fft_cols_wcorrect"][0] > 5 * (prof["fft_cols"][0] + prof["wcorrect"][0])
+        else:
+            assert prof["fft_cols"][0] + prof["wcorrect"][0] > 5 * prof["fft_cols_wcorrect"][0]
+
+
 def test_randomized_parameter_sweep():
     """Seeded sweep over what the fixed cases do not combine: support 3..11, sort tile 8/16/32, grid edge
     64..2048, fp64 / fp32 grid, cube, ragged plane batches, weights, complex64 / complex128, and the chunked
