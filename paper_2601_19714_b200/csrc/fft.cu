@@ -206,7 +206,7 @@ template <typename T, int LOG2N>
 __global__ void __launch_bounds__(Col2Cfg<T, LOG2N>::THREADS, C2_MINB / Col2Cfg<T, LOG2N>::THREADS)
 k_fft_cols_a(typename cplx_of<T>::type* __restrict__ stack, const typename cplx_of<T>::type* __restrict__ tw2,
              const typename cplx_of<T>::type* __restrict__ twN, const unsigned char* __restrict__ occ,
-             const int* __restrict__ sparse_max, int sparse_cap)
+             const int* __restrict__ sparse_max, int sparse_cap, unsigned int n_units)
 {
     typedef typename cplx_of<T>::type C;
     typedef Col2Cfg<T, LOG2N> K;
@@ -214,37 +214,41 @@ k_fft_cols_a(typename cplx_of<T>::type* __restrict__ stack, const typename cplx_
     extern __shared__ __align__(16) unsigned char smem_raw[];
     C* sm = reinterpret_cast<C*>(smem_raw);
     constexpr int STRIPS = K::N / K::W;
-    const int n1 = blockIdx.x & 15;                    // the 16 CTAs of a strip are launched together
-    const unsigned int rest = blockIdx.x >> 4;
-    const int strip = (int)(rest % STRIPS), plane = (int)(rest / STRIPS);
     const int c = threadIdx.x % K::W, t = threadIdx.x / K::W;
-    C* g = stack + (size_t)plane * K::N * K::N + (size_t)n1 * K::N + (size_t)strip * K::W + c;
-    // rows no footprint reaches were never transformed by the row pass and count as zero: they are not read
-    // (and rick_image does not clear them, rick_zero_sparse keep_stale); the pass writes every row
-    const unsigned char* oc = occ + (size_t)plane * K::N + n1;
-    C v[16];
+    // persistent CTAs over the (plane, strip, n1) units: a launch that returns at once (above) costs nothing
+    for (unsigned int unit = blockIdx.x; unit < n_units; unit += gridDim.x) {
+        const int n1 = unit & 15;                    // the 16 units of a strip are taken by neighbouring CTAs
+        const unsigned int rest = unit >> 4;
+        const int strip = (int)(rest % STRIPS), plane = (int)(rest / STRIPS);
+        C* g = stack + (size_t)plane * K::N * K::N + (size_t)n1 * K::N + (size_t)strip * K::W + c;
+        // rows no footprint reaches were never transformed by the row pass and count as zero: they are not read
+        // (and rick_image does not clear them, rick_zero_sparse keep_stale); the pass writes every row
+        const unsigned char* oc = occ + (size_t)plane * K::N + n1;
+        C v[16];
 #pragma unroll
-    for (int e = 0; e < 16; ++e) {
-        const int n2 = t + K::NT2 * ((e + 8) & 15);
-        C x;
-        x.x = 0;
-        x.y = 0;
-        if (oc[16 * n2]) x = g[(size_t)16 * n2 * K::N];
-        v[e] = x;
-    }
-    fft_thread<T, K::LOG2N2>(v, t, sm, K::W, c, tw2);
-    // four outputs at a time: their twiddle loads are not hoisted above the transform (register budget)
-#pragma unroll
-    for (int e0 = 0; e0 < 16; e0 += 4) {
-        asm volatile("" ::: "memory");
-        C w[4];
-#pragma unroll
-        for (int i = 0; i < 4; ++i) w[i] = twN[n1 * (t + K::NT2 * (e0 + i))];
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            const int m2 = t + K::NT2 * (e0 + i);
-            g[(size_t)16 * m2 * K::N] = cmul(v[e0 + i], w[i]);      // twN[0] = 1 when n1 = 0
+        for (int e = 0; e < 16; ++e) {
+            const int n2 = t + K::NT2 * ((e + 8) & 15);
+            C x;
+            x.x = 0;
+            x.y = 0;
+            if (oc[16 * n2]) x = g[(size_t)16 * n2 * K::N];
+            v[e] = x;
         }
+        fft_thread<T, K::LOG2N2>(v, t, sm, K::W, c, tw2);
+        // four outputs at a time: their twiddle loads are not hoisted above the transform (register budget)
+#pragma unroll
+        for (int e0 = 0; e0 < 16; e0 += 4) {
+            asm volatile("" ::: "memory");
+            C w[4];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) w[i] = twN[n1 * (t + K::NT2 * (e0 + i))];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const int m2 = t + K::NT2 * (e0 + i);
+                g[(size_t)16 * m2 * K::N] = cmul(v[e0 + i], w[i]);      // twN[0] = 1 when n1 = 0
+            }
+        }
+        __syncthreads();                             // the exchange buffer is free for the next unit
     }
 }
 
@@ -255,10 +259,15 @@ template <typename T, int LOG2N> static int launch_cols2(rick_plan_t* p, int pla
     const int rcd = rick_all_dirty(p, n_planes);       // the pass writes every row of the slots
     if (rcd) return rcd;
     RICK_CUDA(p, cudaFuncSetAttribute(k_fft_cols_a<T, LOG2N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)K::SMEM));
-    const unsigned int blocks_a = (unsigned int)((size_t)n_planes * (K::N / K::W) * 16);
+    const unsigned int n_units = (unsigned int)((size_t)n_planes * (K::N / K::W) * 16);
+    int per_sm = 1;
+    RICK_CUDA(p, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_fft_cols_a<T, LOG2N>, K::THREADS, K::SMEM));
+    if (per_sm < 1) per_sm = 1;
+    unsigned int blocks_a = (unsigned int)(p->n_sm * per_sm);
+    if (blocks_a > n_units) blocks_a = n_units;
     RICK_KERNEL(p, RK_FFT_COLS, k_fft_cols_a<T, LOG2N><<<blocks_a, K::THREADS, K::SMEM, p->stream>>>(
         (C*)p->stack, (const C*)p->twiddle2, (const C*)p->twiddle, p->row_occ + (size_t)plane_first * p->N,
-        rick_sparse_maxcount(p), rick_sparse_cap(p)));
+        rick_sparse_maxcount(p), rick_sparse_cap(p), n_units));
     return RICK_OK;
 }
 
