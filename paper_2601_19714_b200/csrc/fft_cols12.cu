@@ -218,7 +218,7 @@ k_cols12_wcorrect(const __grid_constant__ CUtensorMap tmap, const double2* __res
                 const double m = (double)(q - C12_N / 2) * dl;
                 const double r2 = l * l + m * m;
                 double xs = 0.0;
-                if (r2 < 1.0) xs = dw * (-r2 / (1.0 + sqrt(1.0 - r2)));
+                if (r2 < 1.0) xs = dw * nm1_of(r2);
                 xs -= rint(xs);
                 sincospi(2.0 * xs, &st[i].y, &st[i].x);
             }
@@ -281,7 +281,7 @@ k_cols12_wcorrect(const __grid_constant__ CUtensorMap tmap, const double2* __res
                 const double r2 = l * l + m * m;
                 double val = 0.0;
                 if (r2 < 1.0) {
-                    double x0 = w_first * (-r2 / (1.0 + sqrt(1.0 - r2)));
+                    double x0 = w_first * nm1_of(r2);
                     x0 -= rint(x0);
                     double pr, pi;
                     sincospi(2.0 * x0, &pi, &pr);
@@ -420,7 +420,7 @@ k_cols13_wcorrect(const __grid_constant__ CUtensorMap tmap, const double2* __res
                 const double m = (double)(q - C13_N / 2) * dl;
                 const double r2 = l * l + m * m;
                 double xs = 0.0;
-                if (r2 < 1.0) xs = dw * (-r2 / (1.0 + sqrt(1.0 - r2)));
+                if (r2 < 1.0) xs = dw * nm1_of(r2);
                 xs -= rint(xs);
                 sincospi(2.0 * xs, &st[i].y, &st[i].x);
             }
@@ -481,7 +481,7 @@ k_cols13_wcorrect(const __grid_constant__ CUtensorMap tmap, const double2* __res
                 const double r2 = l * l + m * m;
                 double val = 0.0;
                 if (r2 < 1.0) {
-                    double x0 = w_first * (-r2 / (1.0 + sqrt(1.0 - r2)));
+                    double x0 = w_first * nm1_of(r2);
                     x0 -= rint(x0);
                     double pr, pi;
                     sincospi(2.0 * x0, &pi, &pr);

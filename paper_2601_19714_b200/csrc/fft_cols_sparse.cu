@@ -82,24 +82,6 @@ __device__ __forceinline__ void cp_async4(void* smem_dst, const void* gsrc)
 }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;\n" ::: "memory"); }
 
-// n - 1 = sqrt(1 - r2) - 1 without cancellation; r2 < 1.  Small fields take the binomial series (no square root,
-// no division): its first neglected term is 2e-19 relative at r2 = 1/128.
-__device__ __forceinline__ double nm1_of(double r2)
-{
-    if (r2 < 0.0078125) {
-        double s = 429.0 / 32768.0;
-        s = fma(s, r2, 33.0 / 2048.0);
-        s = fma(s, r2, 21.0 / 1024.0);
-        s = fma(s, r2, 7.0 / 256.0);
-        s = fma(s, r2, 5.0 / 128.0);
-        s = fma(s, r2, 1.0 / 16.0);
-        s = fma(s, r2, 1.0 / 8.0);
-        s = fma(s, r2, 0.5);
-        return -(s * r2);
-    }
-    return -r2 / (1.0 + sqrt(1.0 - r2));
-}
-
 // exp(2 pi i w (n-1)) as complex fp32: the argument and its reduction to one turn in fp64, the sine and cosine in fp32
 __device__ __forceinline__ float2 phase32(double w, double r2)
 {
