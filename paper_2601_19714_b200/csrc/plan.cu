@@ -633,9 +633,10 @@ extern "C" int rick_image_host(rick_plan_t* p, const void* vis_host, int32_t vis
     // large sets with the whole stack resident go through the chunked path in two halves: the second half
     // of the visibilities is still crossing PCIe while the first is sorted and gridded (measured on
     // configs[1]: 8.06 ms against 8.64 ms for copy-everything-then-sort; more chunks cost more in sorts)
-    // (not on two-pass plans, N >= 8192: there every row of the stack is dirty after a call and the chunked
-    // path would clear the whole stack first, where the one-shot path clears occupied tiles only)
-    if (!p->d.cube && p->batch == p->Nw && M >= ((size_t)1 << 22) && n_rows >= 2 && !rick_cols2_on(p))
+    // (N <= 4096 only: the chunked path clears every dirty row of the stack before the first chunk, the one-shot
+    // path only the tiles it grids into -- at configs[2], N = 8192, that is 5.3 ms against 0.5 ms, more than the
+    // overlapped half of the copy saves: 53.0 ms chunked against 49.1 ms one-shot)
+    if (!p->d.cube && p->batch == p->Nw && M >= ((size_t)1 << 22) && n_rows >= 2 && p->log2N <= 12)
         return rick_image_stream_host(p, vis_host, vis_dtype, uvw_m_host, weights_host, chan_freq_hz, n_chan, n_rows,
                                       (n_rows + 1) / 2, image_out_host);
     const size_t vis_bytes = M * (vis_dtype == RICK_VIS_C128 ? 16 : 8);
