@@ -38,10 +38,12 @@ def _cases():
             ("cfg2 mid 1024^2 weights", synth.make_config(2, n_times=8, n=1024, n_wplanes=6, n_src=8, with_weights=True), {}),
             ("N=4096 fused columns", synth.make_config(2, n_times=2, n_wplanes=5, n_src=4), {}),
             ("N=8192 fused columns", synth.make_config(3, n_times=2, n_wplanes=3, n_src=4), {}),
-            ("fp32 plane batches", synth.make_config(4, n_times=4, n=1024, n_wplanes=7, n_src=4), dict(plane_batch=2))]
+            ("fp32 plane batches", synth.make_config(4, n_times=4, n=1024, n_wplanes=7, n_src=4), dict(plane_batch=2)),
+            ("fp32 N=8192 fused columns over the occupied rows", synth.make_config(4, n_times=2, n=8192, n_wplanes=4, n_src=4),
+             dict(plane_batch=2))]
 
 
-@pytest.mark.parametrize("case", range(5))
+@pytest.mark.parametrize("case", range(6))
 def test_fold_w_matches_the_folded_oracle(case):
     rick = _rick()
     name, wl, over = _cases()[case]
@@ -81,7 +83,7 @@ def test_plane_histogram_equals_oracle_counts():
             assert np.array_equal(hist, want), (name, fold, hist, want)
 
 
-@pytest.mark.parametrize("case", range(5))
+@pytest.mark.parametrize("case", range(6))
 def test_shards_add_up_to_the_whole_image(case):
     rick = _rick()
     from paper_2601_19714_b200 import sharded
@@ -113,6 +115,35 @@ def test_shards_add_up_to_the_whole_image(case):
         print(f"shards {name} world={world} ranges {seen}: rel L2 of the sum {e:.2e}")
         assert n_gridded == o["stats"]["n_gridded"] and n_dropped == o["stats"]["n_dropped"]
         assert abs(sum_w - o["stats"]["sum_w"]) <= 1e-9 * max(1.0, o["stats"]["sum_w"])
+
+
+def test_fold_w_in_cube_mode_and_through_the_chunked_host_entry():
+    """RICK_FLAG_FOLD_W with cube = 1 (every channel its own folded w range) and through rick_image_stream_host
+    (a0 over all rows folds too), N = 8192 fp64 chunked as well (the fused single-pass column kernel)."""
+    rick = _rick()
+    import torch
+    wl = synth.make_config(5, n_times=8, n=512, n_chan=3, n_wplanes=4, n_src=5)
+    o = oracle.image(wl.uvw_m, wl.freq_hz, wl.vis, None, wl.n, wl.n_wplanes, wl.support, wl.pixel_rad, cube=1, fold=True)
+    plan = rick.plan_from_workload(wl, flags=rick.RICK_FLAG_FOLD_W)
+    vis, uvw, wgt = rick.to_device(wl)
+    cube = plan.rick_image(vis, uvw, wgt, wl.freq_hz).cpu().numpy()
+    plan.destroy()
+    for c in range(wl.n_chan):
+        _close(cube[c], o["image"][c], TOL64, f"cube channel {c} folded")
+    for name, wl, flags in (("cfg1 folded", synth.make_config(1), rick.RICK_FLAG_FOLD_W),
+                            ("N=8192 fp64", synth.make_config(3, n_times=3, n_wplanes=3, n_src=4), 0)):
+        o = oracle.image(wl.uvw_m, wl.freq_hz, wl.vis, None, wl.n, wl.n_wplanes, wl.support, wl.pixel_rad, fold=bool(flags))
+        plan = rick.plan_from_workload(wl, flags=flags)
+        hv = torch.from_numpy(np.ascontiguousarray(wl.vis)).pin_memory()
+        hu = torch.from_numpy(wl.uvw_m).pin_memory()
+        out = torch.full((wl.n, wl.n), float("nan"), dtype=torch.float64).pin_memory()
+        for rpc in (wl.n_rows // 3 + 1, wl.n_rows):
+            plan.rick_image_stream_host(hv, hu, None, wl.freq_hz, out, rpc)
+            e = _close(out.numpy(), o["image"], TOL64, f"{name} stream rows_per_chunk={rpc}")
+            st = plan.rick_get_stats()
+            assert st["n_gridded"] == o["stats"]["n_gridded"] and st["n_dropped"] == o["stats"]["n_dropped"]
+        plan.destroy()
+        print(f"stream host {name}: rel L2 {e:.2e}")
 
 
 def test_shard_and_flag_argument_errors(cfg1):
