@@ -49,7 +49,7 @@ struct rick_plan_s {
     // tables
     void* twiddle;           // [N] complex of grid_prec: e^{+2 pi i k/N}
     void* twiddle2;          // [N/16] e^{+2 pi i k/(N/16)}: the long-column two-pass transform (N >= 8192), else null
-    double* taper;           // [N] c((p-N/2)/N)
+    double* taper;           // [2N]: c((p-N/2)/N), then the reciprocals 1/c
     double kb_poly[15 * (RICK_KB_DEG + 1)];   // host: [S][DEG+1], tap a on d = (a-h) - s/2, s in [-1,1]
 
     // resident buffers

@@ -208,6 +208,7 @@ k_cols12_wcorrect(const __grid_constant__ CUtensorMap tmap, const double2* __res
     for (; strip < strip_end; strip += gridDim.x) {
         const int p = strip * C12_WC + R.g;
         const double l = (double)(p - C12_N / 2) * dl;
+        const double itp = taper ? taper[C12_N + p] : 1.0;       // 1 / c(nu_p): taper[N ..) holds the reciprocals
         // step = exp(2 pi i dw (n-1)) of this thread's 16 pixels (rows t2 + 256 ((e+8)&15)) -> TMEM
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
@@ -289,7 +290,7 @@ k_cols12_wcorrect(const __grid_constant__ CUtensorMap tmap, const double2* __res
                 }
                 const size_t pix = (size_t)q * C12_N + p;
                 if (accumulate) val += image[pix];
-                if (taper) val /= (taper[p] * taper[q]);
+                if (taper) val *= itp * taper[C12_N + q];
                 image[pix] = val;
             }
         }
@@ -411,6 +412,7 @@ k_cols13_wcorrect(const __grid_constant__ CUtensorMap tmap, const double2* __res
     const int q0 = 2 * R.t2 + R.g;               // pixel rows of this thread: q0 + 512 ((r + 8) & 15)
     for (; col < col_end; col += gridDim.x) {
         const double l = (double)(col - C13_N / 2) * dl;
+        const double itp = taper ? taper[C13_N + col] : 1.0;     // 1 / c(nu_p)
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
             double2 st[4];
@@ -489,7 +491,7 @@ k_cols13_wcorrect(const __grid_constant__ CUtensorMap tmap, const double2* __res
                 }
                 const size_t pix = (size_t)q * C13_N + col;
                 if (accumulate) val += image[pix];
-                if (taper) val /= (taper[col] * taper[q]);
+                if (taper) val *= itp * taper[C13_N + q];
                 image[pix] = val;
             }
         }

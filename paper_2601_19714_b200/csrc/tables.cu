@@ -45,6 +45,7 @@ __global__ void k_taper(double* __restrict__ taper, int N, int S, double beta, d
         f = sin(r) / r;
     }
     taper[p] = (double)S / i0_beta * f;
+    taper[N + p] = 1.0 / taper[p];          // [N .. 2N): the reciprocals (the fused column kernels multiply)
 }
 
 static long double i0_series(long double x)
@@ -120,7 +121,7 @@ int rick_tables_build(rick_plan_t* p)
         return RICK_ERR_INVALID;
     }
 
-    RICK_CUDA(p, cudaMalloc(&p->taper, sizeof(double) * N));
+    RICK_CUDA(p, cudaMalloc(&p->taper, sizeof(double) * 2 * N));
     RICK_KERNEL(p, RK_TABLES, k_taper<<<(N + 255) / 256, 256, 0, p->stream>>>(p->taper, N, p->S, p->beta, (double)i0));
 
     RICK_CUDA(p, cudaMalloc(&p->twiddle, (p->f32 ? sizeof(float2) : sizeof(double2)) * (size_t)N));
