@@ -24,7 +24,8 @@
  *     (pinned memory makes the copies asynchronous).  Said per argument.
  *   Ownership: the caller owns every input and output buffer; the library borrows
  *     them until the work it enqueued on the plan's stream has completed and never
- *     frees them.  The plan owns sort items, plane stack, image, tables and
+ *     frees them.  The plan owns sort items, plane stack, image, tables (for the fp32 grid with
+ *     N >= 8192 also a transposed accumulation image of N*N doubles and the per-plane row maps) and
  *     frees them in rick_plan_destroy.
  *   Stream: every call enqueues on the plan's stream and returns without
  *     synchronising, except rick_get_stats, rick_image_host and rick_plan_destroy.
@@ -213,8 +214,9 @@ const char* rick_last_error(const rick_plan_t* p);
 const uint64_t* rick_debug_items(rick_plan_t* p, int32_t sorted, int32_t* idx_bits, int32_t* key_bits);
 void*           rick_debug_planes(rick_plan_t* p); /* [N_w][N][N] complex of grid_prec; meaningful after the
                                                     * STAGED calls only: rick_image leaves the stack
-                                                    * half-transformed (rows only at N = 4096 fp64, rows + the
-                                                    * first column pass at N >= 8192) */
+                                                    * half-transformed (occupied rows transformed along u, the
+                                                    * column pass fused with the correction never writes planes;
+                                                    * on the two-pass fallback also the first column pass) */
 
 /* Per-kernel timing with CUDA events on the plan's stream (for roofline reporting).
  * rick_profile(p, 1) clears the records and brackets every later kernel launch with a
