@@ -174,6 +174,8 @@ def measure(cfg, args, rank, world, headline):
             wl = dataclasses.replace(wl, freq_hz=wl.freq_hz[c0:c1].copy(), vis=np.ascontiguousarray(wl.vis[:, c0:c1]),
                                      weights=None if wl.weights is None else np.ascontiguousarray(wl.weights[:, c0:c1]))
             shard = {"kind": "channels", "bounds": cb.tolist()}
+    if world > 1 and not wl.cube and world > wl.n_wplanes:       # the same on every rank: nobody enters a collective
+        raise SystemExit(f"--gpus {world}: more ranks than w-planes ({wl.n_wplanes})")
     vis, uvw, wgt = rick.to_device(wl)
     if world > 1 and not wl.cube:
         sh = sharded.ShardedImager(dict(n=wl.n, n_wplanes=wl.n_wplanes, support=wl.support, pixel_rad=wl.pixel_rad,
@@ -181,9 +183,7 @@ def measure(cfg, args, rank, world, headline):
         bounds = sh.prepare(uvw, wl.freq_hz)
         shard = {"kind": "w-planes", "bounds": bounds.tolist(), "plane_cost_vis": sh.cost,
                  "hist_max": int(sh.hist.max()), "hist_min": int(sh.hist.min())}
-        plan = sh.plan
-        if plan is None:
-            raise SystemExit(f"rank {rank}: more ranks than w-planes")
+        plan = sh.plan                      # (never None: every rank owns at least one plane when world <= N_w)
     else:
         plan = rick.plan_from_workload(wl)
     image = torch.empty((wl.n_chan, wl.n, wl.n) if wl.cube else (wl.n, wl.n), dtype=torch.float64, device="cuda")
