@@ -25,7 +25,6 @@
 #include "common.cuh"
 #include "fft_core.cuh"
 #include "sm100_ptx.cuh"
-#include <stdlib.h>
 
 namespace {
 
@@ -513,7 +512,6 @@ static int encode_map(rick_plan_t* p, void* out, const cuuint64_t* dims, const c
         return RICK_ERR_CUDA;
     }
     const cuuint32_t es[5] = {1, 1, 1, 1, 1};
-    if (const char* ev = getenv("RICK_EXP_PROMO")) promo = (CUtensorMapL2promotion)atoi(ev);   // EXPERIMENT
     const CUresult r = enc(reinterpret_cast<CUtensorMap*>(out), CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 5, p->stack, dims, strides,
                            box, es, CU_TENSOR_MAP_INTERLEAVE_NONE, sw, promo, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) {
