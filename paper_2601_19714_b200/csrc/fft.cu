@@ -8,6 +8,7 @@
 // Centring = index rotation by N/2 = register renaming e -> (e+8) mod 16 (fft_core.cuh).
 #include "common.cuh"
 #include "fft_core.cuh"
+#include "sm100_ptx.cuh"
 
 template <typename T, int LOG2N> struct RowCfg {
     static constexpr int N = 1 << LOG2N, NT = N / 16;
@@ -88,9 +89,25 @@ k_fft_rows(typename cplx_of<T>::type* __restrict__ stack,
             if ((int)threadIdx.x < n_flags) f0 = *flag_addr(grp_next, threadIdx.x);
             if ((int)threadIdx.x + K::THREADS < n_flags) f1 = *flag_addr(grp_next, threadIdx.x + K::THREADS);
         }
+        // BULK (one row per CTA, N >= 4096): the transformed row is assembled in the exchange buffer, free after the
+        // last exchange, and leaves as ONE bulk store of the TMA unit while the CTA goes on to the next row (the
+        // 16 direct stores per thread came in a burst that filled the store queue with every warp waiting behind it).
+        constexpr bool BULK = K::RPC == 1 && LOG2N >= 12;
+        if (BULK && it > 0) {
+            if (threadIdx.x == 0) bulk_wait_read();       // the previous row's store has read the buffer
+            __syncthreads();
+        }
         fft_thread<T, LOG2N>(v, t, sm, 1, 0, tw);
+        if constexpr (BULK) {
 #pragma unroll
-        for (int e = 0; e < 16; ++e) g[t + K::NT * ((e + 8) & 15)] = v[e];
+            for (int e = 0; e < 16; ++e) sm[t + K::NT * ((e + 8) & 15)] = v[e];
+            fence_proxy_async_smem();
+            __syncthreads();
+            if (threadIdx.x == 0) bulk_store(g, sm, (uint32_t)(K::N * sizeof(C)));
+        } else {
+#pragma unroll
+            for (int e = 0; e < 16; ++e) g[t + K::NT * ((e + 8) & 15)] = v[e];
+        }
         if (has_next) {
             unsigned char* nx = &s_to[cur ^ 1][0][0];
             const int i0 = threadIdx.x, i1 = threadIdx.x + K::THREADS;
@@ -100,6 +117,7 @@ k_fft_rows(typename cplx_of<T>::type* __restrict__ stack,
         __syncthreads();
         grp = grp_next;
     }
+    if (K::RPC == 1 && LOG2N >= 12 && threadIdx.x == 0) bulk_wait_read();      // shared memory stays valid until the last store has read it
 }
 
 template <typename T, int LOG2N> struct ColCfg {

@@ -44,6 +44,17 @@ __device__ __forceinline__ void tma_load_5d(void* smem_dst, const CUtensorMap* m
         : "memory");
 }
 
+// ---- bulk store shared -> global (TMA unit, no tensor map): one thread issues, the CTA moves on ------------
+__device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory"); }
+__device__ __forceinline__ void bulk_store(void* gdst, const void* smem_src, uint32_t bytes)
+{
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;\n" ::"l"(gdst), "r"(smem_u32(smem_src)), "r"(bytes)
+                 : "memory");
+    asm volatile("cp.async.bulk.commit_group;\n" ::: "memory");
+}
+// all earlier bulk stores of this thread have READ their shared-memory source (it may be overwritten)
+__device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;\n" ::: "memory"); }
+
 // ---- TMEM as a thread-private scratch file --------------------------------------------------
 // Shape 32x32b: thread i of a warp addresses TMEM lane 32*(warp%4)+i; .xN moves N consecutive
 // 32-bit columns of that lane to / from N registers.
