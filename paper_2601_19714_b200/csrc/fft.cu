@@ -14,7 +14,10 @@ template <typename T, int LOG2N> struct RowCfg {
     static constexpr int N = 1 << LOG2N, NT = N / 16;
     static constexpr int THREADS = NT >= 256 ? NT : 256;
     static constexpr int RPC = THREADS / NT;                       // rows per CTA
-    static constexpr size_t SMEM = (size_t)RPC * (N + N / 16) * 2 * sizeof(T);
+    static constexpr size_t SMEM_EX = (size_t)RPC * (N + N / 16) * 2 * sizeof(T);
+    // one row per CTA and one CTA per SM anyway (512 threads and more): a second buffer for HALF of the output row
+    static constexpr bool HALF_OUT = RPC == 1 && THREADS >= 512;
+    static constexpr size_t SMEM = SMEM_EX + (HALF_OUT ? (size_t)N * sizeof(T) : 0);
 };
 
 // Work list of the row pass: the groups of RPC consecutive rows (slot-major) with at least one occupied row.
@@ -89,16 +92,37 @@ k_fft_rows(typename cplx_of<T>::type* __restrict__ stack,
             if ((int)threadIdx.x < n_flags) f0 = *flag_addr(grp_next, threadIdx.x);
             if ((int)threadIdx.x + K::THREADS < n_flags) f1 = *flag_addr(grp_next, threadIdx.x + K::THREADS);
         }
-        // BULK (one row per CTA, N >= 4096): the transformed row is assembled in the exchange buffer, free after the
-        // last exchange, and leaves as ONE bulk store of the TMA unit while the CTA goes on to the next row (the
-        // 16 direct stores per thread came in a burst that filled the store queue with every warp waiting behind it).
+        // BULK (one row per CTA, N >= 4096): the transformed row is assembled in shared memory and leaves by bulk stores
+        // of the TMA unit while the CTA goes on to the next row (the 16 direct stores per thread came in a burst that
+        // filled the store queue with every warp waiting behind it).  With three CTAs per SM (N = 4096) the row is
+        // assembled in the exchange buffer, free after the last exchange, and the next row's first exchange waits
+        // until the store has read it (the other CTAs run meanwhile).  With one CTA per SM that wait was 16 % of the
+        // kernel (the store drains at the SM's share of the HBM write rate): there the first half of the row goes to
+        // a buffer of its own, which nothing touches for a whole row, and only the second half to the exchange buffer.
         constexpr bool BULK = K::RPC == 1 && LOG2N >= 12;
         if (BULK && it > 0) {
-            if (threadIdx.x == 0) bulk_wait_read();       // the previous row's store has read the buffer
+            if (threadIdx.x == 0) { if (K::HALF_OUT) bulk_wait_read_but_last(); else bulk_wait_read(); }
             __syncthreads();
         }
         fft_thread<T, LOG2N>(v, t, sm, 1, 0, tw);
-        if constexpr (BULK) {
+        if constexpr (BULK && K::HALF_OUT) {
+            C* out_lo = reinterpret_cast<C*>(smem_raw + K::SMEM_EX);
+            if (it > 0) {
+                if (threadIdx.x == 0) bulk_wait_read();      // (long done: issued a whole row ago)
+                __syncthreads();
+            }
+#pragma unroll
+            for (int e = 0; e < 16; ++e) {
+                const int i = t + K::NT * ((e + 8) & 15);
+                if (i < K::N / 2) out_lo[i] = v[e]; else sm[i - K::N / 2] = v[e];
+            }
+            fence_proxy_async_smem();
+            __syncthreads();
+            if (threadIdx.x == 0) {
+                bulk_store(g + K::N / 2, sm, (uint32_t)(K::N / 2 * sizeof(C)));      // first: the one the next row waits for
+                bulk_store(g, out_lo, (uint32_t)(K::N / 2 * sizeof(C)));
+            }
+        } else if constexpr (BULK) {
 #pragma unroll
             for (int e = 0; e < 16; ++e) sm[t + K::NT * ((e + 8) & 15)] = v[e];
             fence_proxy_async_smem();

@@ -54,6 +54,8 @@ __device__ __forceinline__ void bulk_store(void* gdst, const void* smem_src, uin
 }
 // all earlier bulk stores of this thread have READ their shared-memory source (it may be overwritten)
 __device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;\n" ::: "memory"); }
+// ... all but the most recent one
+__device__ __forceinline__ void bulk_wait_read_but_last() { asm volatile("cp.async.bulk.wait_group.read 1;\n" ::: "memory"); }
 
 // ---- TMEM as a thread-private scratch file --------------------------------------------------
 // Shape 32x32b: thread i of a warp addresses TMEM lane 32*(warp%4)+i; .xN moves N consecutive
