@@ -15,9 +15,11 @@ template <typename T, int LOG2N> struct RowCfg {
     static constexpr int THREADS = NT >= 256 ? NT : 256;
     static constexpr int RPC = THREADS / NT;                       // rows per CTA
     static constexpr size_t SMEM_EX = (size_t)RPC * (N + N / 16) * 2 * sizeof(T);
-    // one row per CTA and one CTA per SM anyway (512 threads and more): a second buffer for HALF of the output row
+    // one row per CTA and one CTA per SM anyway (512 threads and more): a second buffer for 5/8 of the output row
+    // (what fits beside the exchange buffer)
     static constexpr bool HALF_OUT = RPC == 1 && THREADS >= 512;
-    static constexpr size_t SMEM = SMEM_EX + (HALF_OUT ? (size_t)N * sizeof(T) : 0);
+    static constexpr int N_OWN = 5 * N / 8;                          // elements of the row that leave from the buffer of their own
+    static constexpr size_t SMEM = SMEM_EX + (HALF_OUT ? (size_t)N_OWN * 2 * sizeof(T) : 0);
 };
 
 // Work list of the row pass: the groups of RPC consecutive rows (slot-major) with at least one occupied row.
@@ -97,8 +99,8 @@ k_fft_rows(typename cplx_of<T>::type* __restrict__ stack,
         // filled the store queue with every warp waiting behind it).  With three CTAs per SM (N = 4096) the row is
         // assembled in the exchange buffer, free after the last exchange, and the next row's first exchange waits
         // until the store has read it (the other CTAs run meanwhile).  With one CTA per SM that wait was 16 % of the
-        // kernel (the store drains at the SM's share of the HBM write rate): there the first half of the row goes to
-        // a buffer of its own, which nothing touches for a whole row, and only the second half to the exchange buffer.
+        // kernel (the store drains at the SM's share of the HBM write rate): there the first 5/8 of the row go to
+        // a buffer of their own, which nothing touches for a whole row, and only the rest to the exchange buffer.
         constexpr bool BULK = K::RPC == 1 && LOG2N >= 12;
         if (BULK && it > 0) {
             if (threadIdx.x == 0) { if (K::HALF_OUT) bulk_wait_read_but_last(); else bulk_wait_read(); }
@@ -114,13 +116,13 @@ k_fft_rows(typename cplx_of<T>::type* __restrict__ stack,
 #pragma unroll
             for (int e = 0; e < 16; ++e) {
                 const int i = t + K::NT * ((e + 8) & 15);
-                if (i < K::N / 2) out_lo[i] = v[e]; else sm[i - K::N / 2] = v[e];
+                if (i < K::N_OWN) out_lo[i] = v[e]; else sm[i - K::N_OWN] = v[e];
             }
             fence_proxy_async_smem();
             __syncthreads();
             if (threadIdx.x == 0) {
-                bulk_store(g + K::N / 2, sm, (uint32_t)(K::N / 2 * sizeof(C)));      // first: the one the next row waits for
-                bulk_store(g, out_lo, (uint32_t)(K::N / 2 * sizeof(C)));
+                bulk_store(g + K::N_OWN, sm, (uint32_t)((K::N - K::N_OWN) * sizeof(C)));      // first: the one the next row waits for
+                bulk_store(g, out_lo, (uint32_t)(K::N_OWN * sizeof(C)));
             }
         } else if constexpr (BULK) {
 #pragma unroll
