@@ -221,13 +221,21 @@ def measure(cfg, args, rank, world, headline):
     value = n_vis_total * steps / (ms_max * 1e-3) / 1e6
 
     # ---- second loop: the library brackets every launch with CUDA events on the stream it launches on
+    # (read back after every step: the per-kernel figure is the MEDIAN over the profiled steps -- a single disturbed
+    # step, seen on this pool when the clock sampler's nvidia-smi starts up under the loop, does not move it; the
+    # per-step values of the larger kernels are kept in stages.kernel_ms_steps)
     psteps = max(1, min(steps, 5))
     plan.rick_profile(True)
+    per_step, prev = [], {}
     for _ in range(psteps):
         step()
-    prof = plan.rick_profile_read()
+        cur = plan.rick_profile_read()
+        per_step.append({k: v[0] - prev.get(k, (0.0, 0))[0] for k, v in cur.items() if v[1]})
+        prev = cur
+    prof = cur
     plan.rick_profile(False)
-    kms = {k: v[0] / psteps for k, v in prof.items() if v[1]}
+    import statistics
+    kms = {k: statistics.median(d.get(k, 0.0) for d in per_step) for k, v in prof.items() if v[1]}
     prof_step_ms = sum(kms.values())
 
     model, sizes = byte_model(wl, st, prof, psteps)
@@ -296,6 +304,7 @@ def measure(cfg, args, rank, world, headline):
         "occupied_tiles_frac": st["occ_tiles"] / (st["n_planes"] * (wl.n // 16) ** 2),
         "image_s": ms_per_step * 1e-3,
         "kernel_ms_per_step": {k: round(v, 4) for k, v in kms.items()},
+        "kernel_ms_steps": {k: [round(d.get(k, 0.0), 3) for d in per_step] for k, v in kms.items() if v >= 0.05 * prof_step_ms},
         "profiled_step_ms": prof_step_ms,
     }
 
