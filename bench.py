@@ -138,19 +138,22 @@ def byte_model(wl, st, prof, steps):
 
 def load_traffic(cfg):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu captures
-    (profiles/traffic.json, written when a capture is summarised): only valid for the kernels as they
-    were when captured, so the file names the sha256 of the csrc tree it was taken at and this returns
-    {} when the sources have changed since."""
-    path = os.path.join(ROOT, "profiles", "traffic.json")
-    try:
-        with open(path) as f:
-            d = json.load(f)
-    except (OSError, ValueError):
-        return {}
+    (profiles/r2_traffic.csv, written when a capture is summarised; profiles/r2_traffic.md says how): only valid
+    for the kernels as they were when captured, so every row names the sha256 of the csrc tree it was taken at
+    and rows of another tree are ignored."""
+    import csv
+    path = os.path.join(ROOT, "profiles", "r2_traffic.csv")
     from paper_2601_19714_b200 import benchutil as bu
-    if d.get("csrc_sha256") != bu.csrc_sha256(ROOT):
+    out = {}
+    try:
+        sha = bu.csrc_sha256(ROOT)
+        with open(path) as f:
+            for row in csv.DictReader(f):
+                if row["csrc_sha256"] == sha and row["config"] == str(cfg):
+                    out[row["kernel_class"]] = float(row["dram_bytes_per_launch"])
+    except (OSError, KeyError, ValueError):
         return {}
-    return d.get("configs", {}).get(str(cfg), {})
+    return out
 
 
 def measure(cfg, args, rank, world, headline):

@@ -127,7 +127,7 @@ def aggregate_replicas(units_per_rank: float, ms_local: float, device="cpu") -> 
 
 
 def csrc_sha256(root: str) -> str:
-    """Hash of the kernel sources: ncu traffic figures in profiles/traffic.json are valid only for the
+    """Hash of the kernel sources: ncu traffic figures in profiles/r2_traffic.csv are valid only for the
     sources they were captured at."""
     import hashlib
     d = os.path.join(root, "paper_2601_19714_b200", "csrc")
