@@ -434,6 +434,25 @@ def test_long_columns_two_pass(prec, pb, tol):
     assert st["n_gridded"] == o["stats"]["n_gridded"]
 
 
+def test_fp32_grid_n4096_bulk_row_store():
+    """fp32 grid at N = 4096: one row per CTA, the row leaves by a bulk store from the exchange buffer (the fp64
+    twin of this path is what configs[1] runs); generic column pass + correction."""
+    rick = _rick()
+    wl = synth.make_config(2, n_times=3, n_wplanes=3, n_src=6)
+    assert wl.n == 4096
+    wl.grid_prec = "f32"
+    o = _oracle(wl)
+    for pb in (0, 2):
+        plan = rick.plan_from_workload(wl, plane_batch=pb)
+        vis, uvw, wgt = rick.to_device(wl)
+        img = plan.rick_image(vis, uvw, wgt, wl.freq_hz).cpu().numpy()
+        img2 = plan.rick_image(vis, uvw, wgt, wl.freq_hz).cpu().numpy()
+        plan.destroy()
+        e = _close(img, o["image"], TOL32, f"fp32 N=4096 plane_batch={pb}")
+        _close(img2, o["image"], TOL32, f"fp32 N=4096 plane_batch={pb}, second call")
+        print(f"fp32 N=4096 plane_batch={pb}: rel L2 {e:.2e}")
+
+
 def test_fp32_long_columns_sparse_and_dense_paths():
     """fp32 grid, N = 8192: rick_image takes the single fused column pass over the occupied rows when every
     plane has at most N/2 of them, and the two-pass kernels otherwise -- decided on the device.  Both against
