@@ -74,6 +74,9 @@ struct rick_plan_s {
     // row_dirty[slot][row] = 1 when that row of the resident slot may hold non-zero data.  Rows that
     // are neither are zero in HBM and stay untouched by zero-fill, gridder and the row pass.
     unsigned char* row_occ; size_t row_occ_cap;
+    // win_mask[pg]: bit k = some row of the k-th 32nd of the plane (rows k N/32 ..) is occupied; written by the row
+    // pass's launcher, read by the fused N = 8192 column pass (which fetches occupied windows only)
+    uint32_t* win_mask; size_t win_mask_cap;
     unsigned char* row_dirty;
     // tile occupancy: tile_occ[pg][tv][tu] = 1 when the footprint of some
     // visibility of global plane pg reaches the B x B tile (tv, tu); rebuilt by every sort.  In rick_image

@@ -40,6 +40,21 @@ __global__ void __launch_bounds__(256) k_row_list(const unsigned char* __restric
     if (any) list[base + __popc(m & ((1u << lane) - 1u))] = gidx;
 }
 
+// win_mask[plane]: bit k = some row of rows [k N/32, (k+1) N/32) is occupied.  One CTA of 32 warps per plane.
+__global__ void __launch_bounds__(1024) k_window_mask(const unsigned char* __restrict__ occ, int N, uint32_t* __restrict__ mask)
+{
+    __shared__ uint32_t s_mask;
+    if (threadIdx.x == 0) s_mask = 0;
+    __syncthreads();
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, win = N >> 5;
+    const unsigned char* o = occ + (size_t)blockIdx.x * N + (size_t)warp * win;
+    bool any = false;
+    for (int i = lane; i < win; i += 32) any |= o[i] != 0;
+    if (__any_sync(0xffffffffu, any) && lane == 0) atomicOr(&s_mask, 1u << warp);
+    __syncthreads();
+    if (threadIdx.x == 0) mask[blockIdx.x] = s_mask;
+}
+
 template <typename T, int LOG2N>
 __global__ void __launch_bounds__(RowCfg<T, LOG2N>::THREADS, (RowCfg<T, LOG2N>::THREADS <= 256 ? 3 : 1))
 k_fft_rows(typename cplx_of<T>::type* __restrict__ stack,
@@ -198,6 +213,9 @@ static int launch_fft(rick_plan_t* p, int plane_first, int n_planes, int which) 
         RICK_CUDA(p, cudaMemsetAsync(count, 0, sizeof(unsigned int), p->stream));
         RICK_KERNEL(p, RK_ROW_OCC, k_row_list<<<(n_groups + 255) / 256, 256, 0, p->stream>>>(
             p->row_occ + (size_t)plane_first * p->N, n_groups, KR::RPC, p->row_list, count));
+        if (p->cols13_ok)      // the fused N = 8192 column pass fetches occupied windows of 256 rows only
+            RICK_KERNEL(p, RK_ROW_OCC, k_window_mask<<<n_planes, 1024, 0, p->stream>>>(
+                p->row_occ + (size_t)plane_first * p->N, p->N, p->win_mask + plane_first));
         int per_sm = 1;
         RICK_CUDA(p, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_fft_rows<T, LOG2N>, KR::THREADS, KR::SMEM));
         if (per_sm < 1) per_sm = 1;

@@ -315,10 +315,36 @@ k_cols12_wcorrect(const __grid_constant__ CUtensorMap tmap, const double2* __res
 constexpr int C13_N = 2 * C12_N;
 constexpr uint32_t C13_STAGE_BYTES = (uint32_t)C13_N * 16u;          // 131072: one column
 
+constexpr uint32_t C13_WIN_BYTES = C13_STAGE_BYTES / 32;            // a window of 256 rows of one column: 4 KB
+
+// Fetch the occupied windows of (column, plane) into the staging: called by the EIGHT warps first_warp .. first_warp + 7,
+// lanes 0 .. 3 of each issue one window (32 copies issued by one warp held that warp, and its group, up).  mask bit
+// k = e + 16 e2 <-> rows 256 k .. 256 k + 255 <-> staging bytes [4096 k, 4096 (k + 1)).  Windows with no occupied
+// row are zero in HBM and are neither fetched nor read.  (A copy may complete before the
+// expect_tx of the one arriving thread: the barrier's pending arrival keeps the phase open.)
+__device__ __forceinline__ void col13_issue(const double2* stg, unsigned long long* full, const CUtensorMap* tmap_all,
+                                            const CUtensorMap* tmap_win, uint32_t mask, int col, int slot, int first_warp)
+{
+    const int lane = threadIdx.x & 31, wq = (int)(threadIdx.x >> 5) - first_warp;
+    if (mask == 0xffffffffu) {
+        if (wq == 0 && lane == 0) {
+            mbar_arrive_expect_tx(full, C13_STAGE_BYTES);
+            tma_load_5d(const_cast<double2*>(stg), tmap_all, full, 2 * col, 0, 0, 0, 2 * slot);
+        }
+        return;
+    }
+    if (wq == 0 && lane == 0) mbar_arrive_expect_tx(full, (uint32_t)__popc(mask) * C13_WIN_BYTES);
+    const int k = 4 * wq + lane;
+    if (lane < 4 && ((mask >> k) & 1u))
+        tma_load_5d(const_cast<double2*>(stg) + k * (int)(C13_WIN_BYTES / 16), tmap_win, full, 2 * col, 0, 0, k & 15,
+                    2 * slot + (k >> 4));
+}
+
 __device__ __forceinline__ void col13_fft_g(double2 (&v)[16], const RolesG& R, const double2* __restrict__ stg,
                                             double* __restrict__ ex, const double2* __restrict__ twN,
                                             unsigned long long* full, unsigned long long* empty, uint32_t& parity,
-                                            bool issue_next, const CUtensorMap* tmap, int next_col, int next_plane)
+                                            bool issue_next, const CUtensorMap* tmap, const CUtensorMap* tmap_win,
+                                            uint32_t mask, uint32_t mask_next, int next_col, int next_plane)
 {
     // group 1: W_N^n for n = t1 + 256 e is W_N^t1 times the constant e^{2 pi i e / 32}
     double2 wb;
@@ -327,22 +353,31 @@ __device__ __forceinline__ void col13_fft_g(double2 (&v)[16], const RolesG& R, c
         named_bar_sync(3, 512);                  // group 0 has read the staging of this item
     }
     mbar_wait(full, parity);
-    // staging order [e2][e][w][hh] (16-byte elements): row = w + 16 hh + 256 e + 4096 e2
+    // staging order [e2][e][w][hh] (16-byte elements): row = w + 16 hh + 256 e + 4096 e2; windows the mask leaves
+    // out were not fetched and count as zero
     const double2* s0 = stg + R.w * 16 + R.hh;
+    const double2 zero = make_double2(0.0, 0.0);
     if (R.g == 0) {
 #pragma unroll
-        for (int e = 0; e < 16; ++e) v[e] = cadd(s0[(16 + e) * 256], s0[e * 256]);
+        for (int e = 0; e < 16; ++e) {
+            const double2 hi = (mask >> (16 + e)) & 1u ? s0[(16 + e) * 256] : zero;
+            const double2 lo = (mask >> e) & 1u ? s0[e * 256] : zero;
+            v[e] = cadd(hi, lo);
+        }
     } else {
 #pragma unroll
-        for (int e = 0; e < 16; ++e) v[e] = csub(s0[(16 + e) * 256], s0[e * 256]);
+        for (int e = 0; e < 16; ++e) {
+            const double2 hi = (mask >> (16 + e)) & 1u ? s0[(16 + e) * 256] : zero;
+            const double2 lo = (mask >> e) & 1u ? s0[e * 256] : zero;
+            v[e] = csub(hi, lo);
+        }
     }
     if (R.g == 0) named_bar_arrive(3, 512);
     __syncwarp();
     if ((threadIdx.x & 31) == 0) mbar_arrive(empty);
-    if (threadIdx.x == 256 && issue_next) {
+    if (R.g == 1 && issue_next) {                     // group 1 is the last to read the staging
         mbar_wait(empty, parity);
-        mbar_arrive_expect_tx(full, C13_STAGE_BYTES);
-        tma_load_5d(const_cast<double2*>(stg), tmap, full, 2 * next_col, 0, 0, 0, 2 * next_plane);
+        col13_issue(stg, full, tmap, tmap_win, mask_next, next_col, next_plane, 8);
     }
     parity ^= 1u;
     if (R.g == 1) {
@@ -374,7 +409,8 @@ __device__ __forceinline__ void col13_fft_g(double2 (&v)[16], const RolesG& R, c
 }
 
 __global__ void __launch_bounds__(C12_THREADS, 1)
-k_cols13_wcorrect(const __grid_constant__ CUtensorMap tmap, const double2* __restrict__ twN, int n_planes,
+k_cols13_wcorrect(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ CUtensorMap tmap_win,
+                  const uint32_t* __restrict__ wmask, const double2* __restrict__ twN, int n_planes,
                   int z_first, double dl, const WRange* __restrict__ wr, double* __restrict__ image,
                   int accumulate, const double* __restrict__ taper, int col_begin, int col_end, int slot_first)
 {
@@ -401,10 +437,10 @@ k_cols13_wcorrect(const __grid_constant__ CUtensorMap tmap, const double2* __res
     const uint32_t tStep = tS + 64;
 
     int col = col_begin + (int)blockIdx.x;
-    if (threadIdx.x == 0 && col < col_end) {
-        mbar_arrive_expect_tx(full, C13_STAGE_BYTES);
-        tma_load_5d(stg, &tmap, full, 2 * col, 0, 0, 0, 2 * (slot_first + n_planes - 1));
-    }
+    // wmask[plane]: the occupied 256-row windows of the batch's planes (k_window_mask, fft.cu)
+    const uint32_t mask_top = wmask[n_planes - 1];
+    uint32_t mask = mask_top;
+    if (warp < 8 && col < col_end) col13_issue(stg, full, &tmap, &tmap_win, mask, col, slot_first + n_planes - 1, 0);
     uint32_t parity = 0;
     const double dw = wr->dw;
     const double w_first = wr->w_min + ((double)z_first + 0.5) * dw;
@@ -432,9 +468,11 @@ k_cols13_wcorrect(const __grid_constant__ CUtensorMap tmap, const double2* __res
         tmem_wait_st();
         for (int plane = n_planes - 1; plane >= 0; --plane) {
             const bool more = plane > 0 || col + (int)gridDim.x < col_end;
+            const uint32_t mask_next = plane > 0 ? wmask[plane - 1] : mask_top;
             double2 v[16];
-            col13_fft_g(v, R, stg, ex, twN, full, empty, parity, more, &tmap, plane > 0 ? col : col + (int)gridDim.x,
-                        slot_first + (plane > 0 ? plane - 1 : n_planes - 1));
+            col13_fft_g(v, R, stg, ex, twN, full, empty, parity, more, &tmap, &tmap_win, mask, mask_next,
+                        plane > 0 ? col : col + (int)gridDim.x, slot_first + (plane > 0 ? plane - 1 : n_planes - 1));
+            mask = mask_next;
             if (plane == n_planes - 1) {
 #pragma unroll
                 for (int k = 0; k < 4; ++k) {
@@ -536,6 +574,9 @@ int rick_cols12_init(rick_plan_t* p)
         const cuuint64_t strides[4] = {16 * rowB, rowB, 256 * rowB, 4096 * rowB};
         const cuuint32_t box[5] = {2, 16, 16, 16, 2};
         if ((rc = encode_map(p, p->cols12_tmap_sw, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE))) return rc;
+        // the same view with a box of ONE window of 256 rows (e, e2 fixed): planes with empty windows are fetched window by window
+        const cuuint32_t box_win[5] = {2, 16, 16, 1, 1};
+        if ((rc = encode_map(p, p->cols12_tmap, dims, strides, box_win, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE))) return rc;
         RICK_CUDA(p, cudaFuncSetAttribute(k_cols13_wcorrect, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C12_SMEM));
         p->cols13_ok = 1;
         return RICK_OK;
@@ -570,8 +611,10 @@ int rick_cols12_wcorrect(rick_plan_t* p, int img, int z_first, int n_planes, dou
     const CUtensorMap tm = *reinterpret_cast<const CUtensorMap*>(p->cols12_tmap_sw);
     const int n = strip_end - strip_begin;
     if (p->cols13_ok) {
+        const CUtensorMap tm_win = *reinterpret_cast<const CUtensorMap*>(p->cols12_tmap);
+        // (the row pass of these planes has just written their window masks)
         RICK_KERNEL(p, RK_COLS_WCORRECT, k_cols13_wcorrect<<<n < p->n_sm ? n : p->n_sm, C12_THREADS, C12_SMEM, p->stream>>>(
-            tm, (const double2*)p->twiddle, n_planes, p->z0 + z_first, p->dl, p->wrange + img, image, accumulate,
+            tm, tm_win, p->win_mask + (size_t)img * p->Nw + z_first, (const double2*)p->twiddle, n_planes, p->z0 + z_first, p->dl, p->wrange + img, image, accumulate,
             fuse_taper ? p->taper : nullptr, strip_begin, strip_end, slot_first));
         return RICK_OK;
     }

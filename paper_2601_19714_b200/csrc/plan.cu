@@ -112,7 +112,7 @@ extern "C" int rick_plan_destroy(rick_plan_t* p)
     free_dev(p->twiddle); free_dev(p->twiddle2); free_dev(p->taper); free_dev(p->stack); free_dev(p->image);
     free_dev(p->items); free_dev(p->items_a); free_dev(p->items_b);
     free_dev(p->os_small); free_dev(p->os_gbase); free_dev(p->os_status); free_dev(p->plane_start); free_dev(p->chan_scale);
-    free_dev(p->row_occ); free_dev(p->row_dirty); free_dev(p->tile_occ); free_dev(p->row_list);
+    free_dev(p->row_occ); free_dev(p->win_mask); free_dev(p->row_dirty); free_dev(p->tile_occ); free_dev(p->row_list);
     free_dev(p->wrange); free_dev(p->counters);
     rick_sparse_free(p);
     free_dev(p->st_vis); free_dev(p->st_uvw); free_dev(p->st_wgt); free_dev(p->st_img);
@@ -342,6 +342,11 @@ static int prepare(rick_plan_t* p, const double* chan_freq_hz, int32_t n_chan, i
         p->row_occ_cap = 0;
         if ((rc = grow(p, &p->row_occ, occ_bytes))) return rc;
         p->row_occ_cap = occ_bytes;
+    }
+    if ((size_t)(n_pl - 1) > p->win_mask_cap) {
+        p->win_mask_cap = 0;
+        if ((rc = grow(p, &p->win_mask, (size_t)(n_pl - 1)))) return rc;
+        p->win_mask_cap = (size_t)(n_pl - 1);
     }
     const size_t tocc_bytes = (size_t)(n_pl - 1) * p->T * p->T;
     if (tocc_bytes > p->tile_occ_cap) {

@@ -434,6 +434,49 @@ def test_long_columns_two_pass(prec, pb, tol):
     assert st["n_gridded"] == o["stats"]["n_gridded"]
 
 
+def test_n8192_fp64_occupied_windows_only():
+    """N = 8192 fp64: the fused column pass fetches and reads only the 256-row windows of a plane that hold an occupied
+    row (one 32-bit mask per plane).  Here the planes differ as much as they can: plane 0 holds short v only (a few
+    central windows), planes 1..3 hold nothing at all (mask 0), plane 4 holds the long baselines; a second call on
+    the SAME plan then images the unmodified set (every mask changes, rows of the first call are stale)."""
+    rick = _rick()
+    wl = synth.make_config(3, n_times=4, n_wplanes=5, n_src=6)
+    assert wl.n == 8192 and wl.grid_prec == "f64"
+    orig = wl.uvw_m.copy()
+    uvw = orig.copy()
+    R = uvw.shape[0]
+    uvw[: R // 2, 2] = -100.0
+    uvw[R // 2:, 2] = 100.0
+    uvw[: R // 2, 1] *= 0.05
+    wl.uvw_m = uvw
+    ix = oracle.index(wl.uvw_m, wl.freq_hz, wl.n, wl.n_wplanes, wl.support, wl.pixel_rad, 16)
+    keep = ix["key"] != np.uint64(0xFFFFFFFFFFFFFFFF)
+    h = wl.support // 2
+    wins = []
+    for z in range(wl.n_wplanes):
+        v = ix["iv"][keep & (ix["ip"] == z)]
+        occ = np.zeros(32, bool)
+        for d in range(-h, h + 1):
+            occ[np.clip(v + d, 0, wl.n - 1) >> 8] = True
+        wins.append(int(occ.sum()))
+    print("occupied windows per plane:", wins)
+    assert wins[1] == wins[2] == wins[3] == 0 and 0 < wins[0] < wins[4] <= 32     # the case this test is for
+    o = _oracle(wl)
+    plan = rick.plan_from_workload(wl)
+    vis, uvw_d, wgt = rick.to_device(wl)
+    img = plan.rick_image(vis, uvw_d, wgt, wl.freq_hz).cpu().numpy()
+    st = plan.rick_get_stats()
+    e = _close(img, o["image"], TOL64, "two occupied planes of five")
+    assert st["n_gridded"] == o["stats"]["n_gridded"]
+    wl.uvw_m = orig
+    o2 = _oracle(wl)
+    vis, uvw_d, wgt = rick.to_device(wl)
+    img2 = plan.rick_image(vis, uvw_d, wgt, wl.freq_hz).cpu().numpy()
+    plan.destroy()
+    e2 = _close(img2, o2["image"], TOL64, "same plan, unmodified set")
+    print(f"N=8192 fp64 window masks: rel L2 {e:.2e} (planes 1..3 empty), {e2:.2e} (second set on the same plan)")
+
+
 def test_fp32_grid_n4096_bulk_row_store():
     """fp32 grid at N = 4096: one row per CTA, the row leaves by a bulk store from the exchange buffer (the fp64
     twin of this path is what configs[1] runs); generic column pass + correction."""
