@@ -123,7 +123,9 @@ def byte_model(wl, st, prof, steps):
                                       flops=fft_flops(N * P) + 8.0 * N * N * P, dense_bytes=stack + img, alu=True)
         m["taper"] = dict(bytes=2 * img)
     elif fused:        # single pass over the stack fused with a5 (+ a6): the planes are never written
-        m["fft_cols_wcorrect"] = dict(bytes=stack + img + rmw, flops=fft_flops(N * P) + 8.0 * N * N * P,
+        # (N = 8192: only the windows of N/32 rows that hold an occupied row are fetched)
+        read = int(st["occ_windows"]) * (N // 32) * N * E if N == 8192 else stack
+        m["fft_cols_wcorrect"] = dict(bytes=read + img + rmw, flops=fft_flops(N * P) + 8.0 * N * N * P,
                                       dense_bytes=stack + img)
     elif N >= 8192:    # two passes: A in place (reads occupied rows, writes every row), B fused with a5 (+ a6)
         m["fft_cols"] = dict(bytes=occ_rows * N * E + stack, flops=fft_flops(N * P) * (math.log2(N) - 4) / math.log2(N),

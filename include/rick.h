@@ -111,6 +111,8 @@ typedef struct {
     int64_t occ_tiles;   /* (plane, B x B tile) pairs some footprint reaches: what the zero-fill clears
                           * and the row pass reads, out of n_planes * (N/B)^2                    */
     int64_t n_planes;    /* planes of the last call: N_w, or C * N_w for a cube                 */
+    int64_t occ_windows; /* (plane, window of N/32 consecutive rows) pairs with an occupied row, out of
+                          * 32 * n_planes: what the fused N = 8192 fp64 column pass fetches     */
 } rick_stats;
 
 /* Create a plan: validates `d`, allocates the plane stack

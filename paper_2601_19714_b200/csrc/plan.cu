@@ -852,12 +852,19 @@ extern "C" int rick_get_stats(rick_plan_t* p, rick_stats* out)
     // occupancy of the last sort: what the pruned passes move
     out->occ_rows = 0;
     out->occ_tiles = 0;
+    out->occ_windows = 0;
     out->n_planes = (int64_t)p->n_img * p->Nw;
     if (p->row_occ && p->tile_occ && p->n_img > 0) {
         const size_t nr = (size_t)p->n_img * p->Nw * p->N, nt = (size_t)p->n_img * p->Nw * p->T * p->T;
         std::vector<unsigned char> h(nr > nt ? nr : nt);
         RICK_CUDA(p, cudaMemcpy(h.data(), p->row_occ, nr, cudaMemcpyDeviceToHost));
         for (size_t i = 0; i < nr; ++i) out->occ_rows += h[i] != 0;
+        const size_t win = (size_t)p->N / 32;
+        for (size_t w0 = 0; win && w0 < nr; w0 += win) {
+            bool any = false;
+            for (size_t i = w0; i < w0 + win; ++i) any |= h[i] != 0;
+            out->occ_windows += any;
+        }
         RICK_CUDA(p, cudaMemcpy(h.data(), p->tile_occ, nt, cudaMemcpyDeviceToHost));
         for (size_t i = 0; i < nt; ++i) out->occ_tiles += h[i] != 0;
     }

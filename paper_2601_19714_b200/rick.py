@@ -42,7 +42,7 @@ class Stats(C.Structure):
     _fields_ = [("n_vis", C.c_int64), ("n_gridded", C.c_int64), ("n_dropped", C.c_int64),
                 ("sum_w", C.c_double), ("w_min", C.c_double), ("w_max", C.c_double),
                 ("n_launches", C.c_int64), ("occ_rows", C.c_int64), ("occ_tiles", C.c_int64),
-                ("n_planes", C.c_int64)]
+                ("n_planes", C.c_int64), ("occ_windows", C.c_int64)]
 
 
 class RickError(RuntimeError):
