@@ -278,13 +278,19 @@ def measure(cfg, args, rank, world, headline):
         if "flops" in mk:      # secondary ceiling: the FFT's own arithmetic on the plain FMA pipe
             r["fft_tflops"] = mk["flops"] / (ms * 1e-3) / 1e12
             r["fft_frac_of_fma_peak"] = r["fft_tflops"] / alu_peak_tflops
-        if mk.get("alu"):
-            # this kernel moves a small fraction of the stack (the occupied rows) and is bound by instruction issue
-            # on the plain FMA pipe: its roofline is the arithmetic one (5 N log2 N flop per transform + the Horner
-            # step against lanes x 2 flop x clock); the HBM figures stay beside it
+        t_hbm = mk["bytes"] / (peaks["hbm_gbs"] * 1e9)
+        t_alu = mk["flops"] / (alu_peak_tflops * 1e12) if "flops" in mk else 0.0
+        if mk.get("alu") or t_alu > t_hbm:
+            # The roof is the lower of the two at the kernel's arithmetic intensity.  A kernel that skips the known-zero
+            # part of the stack (the occupied rows of the fp32 pass, the occupied windows of the N = 8192 fp64 pass) moves
+            # so few bytes that its arithmetic floor (5 N log2 N flop per transform + the Horner step against lanes x
+            # 2 flop x clock) lies above its HBM floor: its roofline is the arithmetic one; the HBM
+            # figures stay beside it.
             r.update({"bound": "alu", "hbm_gb_s_moved": r["achieved"], "hbm_frac": r["frac"],
                       "achieved": r["fft_tflops"], "peak": alu_peak_tflops, "unit": "TFLOP/s",
-                      "frac": r["fft_frac_of_fma_peak"], "peak_source": "148 SMs x 128 fp32 lanes x 2 flop x 1.965 GHz"})
+                      "frac": r["fft_frac_of_fma_peak"],
+                      "peak_source": "148 SMs x %d %s lanes x 2 flop x 1.965 GHz" % (128 if f32 else 64, "fp32" if f32 else "fp64"),
+                      "floor_ms": {"hbm": round(t_hbm * 1e3, 3), "alu": round(t_alu * 1e3, 3)}})
         rooflines.append(r)
 
     def ms_of(*names):

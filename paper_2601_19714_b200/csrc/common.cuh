@@ -77,6 +77,7 @@ struct rick_plan_s {
     // win_mask[pg]: bit k = some row of the k-th 32nd of the plane (rows k N/32 ..) is occupied; written by the row
     // pass's launcher, read by the fused N = 8192 column pass (which fetches occupied windows only)
     uint32_t* win_mask; size_t win_mask_cap;
+    uint32_t* cols_arrivals; size_t cols_arrivals_cap;   // pacing counters of the fused N = 8192 column pass (one per item of a CTA)
     unsigned char* row_dirty;
     // tile occupancy: tile_occ[pg][tv][tu] = 1 when the footprint of some
     // visibility of global plane pg reaches the B x B tile (tv, tu); rebuilt by every sort.  In rick_image

@@ -317,15 +317,49 @@ constexpr uint32_t C13_STAGE_BYTES = (uint32_t)C13_N * 16u;          // 131072: 
 
 constexpr uint32_t C13_WIN_BYTES = C13_STAGE_BYTES / 32;            // a window of 256 rows of one column: 4 KB
 
+// Pacing.  A 16-byte piece of a column sits in a 128-byte line with the pieces of the seven neighbouring columns,
+// which seven other SMs fetch, and an L2 miss on this access pattern fills far more than the piece from DRAM (measured
+// with the copies alone: 126 bytes of DRAM traffic per 16-byte piece when every SM walks a plane of its own, 1.03 x the
+// useful bytes when all walk the same plane).  The stack is read once only as long as the CTAs work
+// on the same plane at about the same time.  While the pass was bound by its feed they did by themselves (a CTA that
+// ran ahead missed in L2 and fell back); with the known-zero windows skipped most planes are bound by their arithmetic,
+// nothing couples the CTAs any more, they drift apart by whole planes and DRAM delivered 2.5 x the bytes.  So the CTAs
+// pace each other: arrivals[i] counts the CTAs that have issued their item number i (one RED per CTA and item), and a
+// CTA issues its item i only once every CTA that has an item i - C13_PACE_SLACK has issued it.  One word is polled, and
+// it is fetched at the top of the item, long before the copy it gates.  The wait is bounded: if the others do not show
+// up (CTAs of the grid not resident) the warp stops pacing for good -- the result does not depend on it.
+constexpr int C13_PACE_SLACK = 2;
+struct Pace {
+    uint32_t* arrivals;               // [items per CTA], zeroed before the launch; null = no pacing
+    int n_planes, n_cols;             // of the launch: item i belongs to column round i / n_planes
+    bool on;
+};
+__device__ __forceinline__ uint32_t pace_load(const Pace& pc, int item)            // arrivals of the item that gates `item`
+{
+    return pc.on && item >= C13_PACE_SLACK ? *(volatile uint32_t*)(pc.arrivals + (item - C13_PACE_SLACK)) : 0u;
+}
+__device__ __forceinline__ void pace_wait(Pace& pc, int item, uint32_t seen)
+{
+    if (!pc.on || item < C13_PACE_SLACK) return;
+    const int round = (item - C13_PACE_SLACK) / pc.n_planes, full = pc.n_cols / (int)gridDim.x;
+    const uint32_t need = round < full ? gridDim.x : (round == full ? (uint32_t)(pc.n_cols % (int)gridDim.x) : 0u);
+    for (int spin = 0; spin < (1 << 16) && seen < need; ++spin) seen = pace_load(pc, item);
+    if (seen < need) pc.on = false;
+}
+
 // Fetch the occupied windows of (column, plane) into the staging: called by the EIGHT warps first_warp .. first_warp + 7,
 // lanes 0 .. 3 of each issue one window (32 copies issued by one warp held that warp, and its group, up).  mask bit
 // k = e + 16 e2 <-> rows 256 k .. 256 k + 255 <-> staging bytes [4096 k, 4096 (k + 1)).  Windows with no occupied
 // row are zero in HBM and are neither fetched nor read.  (A copy may complete before the
-// expect_tx of the one arriving thread: the barrier's pending arrival keeps the phase open.)
+// expect_tx of the one arriving thread: the barrier's pending arrival keeps the phase open.)  `item` = the number of
+// this item among the CTA's items, `seen` = pace_load(pc, item) fetched earlier.
 __device__ __forceinline__ void col13_issue(const double2* stg, unsigned long long* full, const CUtensorMap* tmap_all,
-                                            const CUtensorMap* tmap_win, uint32_t mask, int col, int slot, int first_warp)
+                                            const CUtensorMap* tmap_win, uint32_t mask, int col, int slot, int first_warp,
+                                            Pace& pc, int item, uint32_t seen)
 {
     const int lane = threadIdx.x & 31, wq = (int)(threadIdx.x >> 5) - first_warp;
+    pace_wait(pc, item, seen);
+    if (pc.arrivals && wq == 0 && lane == 0) atomicAdd(pc.arrivals + item, 1u);
     if (mask == 0xffffffffu) {
         if (wq == 0 && lane == 0) {
             mbar_arrive_expect_tx(full, C13_STAGE_BYTES);
@@ -344,11 +378,14 @@ __device__ __forceinline__ void col13_fft_g(double2 (&v)[16], const RolesG& R, c
                                             double* __restrict__ ex, const double2* __restrict__ twN,
                                             unsigned long long* full, unsigned long long* empty, uint32_t& parity,
                                             bool issue_next, const CUtensorMap* tmap, const CUtensorMap* tmap_win,
-                                            uint32_t mask, uint32_t mask_next, int next_col, int next_plane)
+                                            uint32_t mask, uint32_t mask_next, int next_col, int next_plane, Pace& pc,
+                                            int next_item)
 {
     // group 1: W_N^n for n = t1 + 256 e is W_N^t1 times the constant e^{2 pi i e / 32}
     double2 wb;
+    uint32_t seen = 0;
     if (R.g == 1) {
+        if (issue_next) seen = pace_load(pc, next_item);       // (consumed after the staging read)
         wb = twN[R.t1];
         named_bar_sync(3, 512);                  // group 0 has read the staging of this item
     }
@@ -377,7 +414,7 @@ __device__ __forceinline__ void col13_fft_g(double2 (&v)[16], const RolesG& R, c
     if ((threadIdx.x & 31) == 0) mbar_arrive(empty);
     if (R.g == 1 && issue_next) {                     // group 1 is the last to read the staging
         mbar_wait(empty, parity);
-        col13_issue(stg, full, tmap, tmap_win, mask_next, next_col, next_plane, 8);
+        col13_issue(stg, full, tmap, tmap_win, mask_next, next_col, next_plane, 8, pc, next_item, seen);
     }
     parity ^= 1u;
     if (R.g == 1) {
@@ -412,7 +449,8 @@ __global__ void __launch_bounds__(C12_THREADS, 1)
 k_cols13_wcorrect(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ CUtensorMap tmap_win,
                   const uint32_t* __restrict__ wmask, const double2* __restrict__ twN, int n_planes,
                   int z_first, double dl, const WRange* __restrict__ wr, double* __restrict__ image,
-                  int accumulate, const double* __restrict__ taper, int col_begin, int col_end, int slot_first)
+                  int accumulate, const double* __restrict__ taper, int col_begin, int col_end, int slot_first,
+                  uint32_t* arrivals)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     unsigned char* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
@@ -440,7 +478,12 @@ k_cols13_wcorrect(const __grid_constant__ CUtensorMap tmap, const __grid_constan
     // wmask[plane]: the occupied 256-row windows of the batch's planes (k_window_mask, fft.cu)
     const uint32_t mask_top = wmask[n_planes - 1];
     uint32_t mask = mask_top;
-    if (warp < 8 && col < col_end) col13_issue(stg, full, &tmap, &tmap_win, mask, col, slot_first + n_planes - 1, 0);
+    Pace pc = {arrivals, n_planes, col_end - col_begin, arrivals != nullptr};
+    int item = 0;                                // items this CTA has issued
+    if (col < col_end) {
+        if (warp < 8) col13_issue(stg, full, &tmap, &tmap_win, mask, col, slot_first + n_planes - 1, 0, pc, 0, 0u);
+        item = 1;
+    }
     uint32_t parity = 0;
     const double dw = wr->dw;
     const double w_first = wr->w_min + ((double)z_first + 0.5) * dw;
@@ -471,7 +514,8 @@ k_cols13_wcorrect(const __grid_constant__ CUtensorMap tmap, const __grid_constan
             const uint32_t mask_next = plane > 0 ? wmask[plane - 1] : mask_top;
             double2 v[16];
             col13_fft_g(v, R, stg, ex, twN, full, empty, parity, more, &tmap, &tmap_win, mask, mask_next,
-                        plane > 0 ? col : col + (int)gridDim.x, slot_first + (plane > 0 ? plane - 1 : n_planes - 1));
+                        plane > 0 ? col : col + (int)gridDim.x, slot_first + (plane > 0 ? plane - 1 : n_planes - 1), pc, item);
+            item += more;
             mask = mask_next;
             if (plane == n_planes - 1) {
 #pragma unroll
@@ -578,6 +622,13 @@ int rick_cols12_init(rick_plan_t* p)
         const cuuint32_t box_win[5] = {2, 16, 16, 1, 1};
         if ((rc = encode_map(p, p->cols12_tmap, dims, strides, box_win, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE))) return rc;
         RICK_CUDA(p, cudaFuncSetAttribute(k_cols13_wcorrect, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C12_SMEM));
+        // pacing counters (k_cols13_wcorrect, "Pacing"): one per item of a CTA, at most ceil(N / n_sm) columns x the
+        // resident planes of one launch
+        if (!p->cols_arrivals) {
+            const size_t cap = (size_t)((C13_N + p->n_sm - 1) / p->n_sm) * (size_t)p->slots;
+            RICK_CUDA(p, cudaMalloc(&p->cols_arrivals, sizeof(uint32_t) * cap));
+            p->cols_arrivals_cap = cap;
+        }
         p->cols13_ok = 1;
         return RICK_OK;
     }
@@ -613,9 +664,15 @@ int rick_cols12_wcorrect(rick_plan_t* p, int img, int z_first, int n_planes, dou
     if (p->cols13_ok) {
         const CUtensorMap tm_win = *reinterpret_cast<const CUtensorMap*>(p->cols12_tmap);
         // (the row pass of these planes has just written their window masks)
-        RICK_KERNEL(p, RK_COLS_WCORRECT, k_cols13_wcorrect<<<n < p->n_sm ? n : p->n_sm, C12_THREADS, C12_SMEM, p->stream>>>(
-            tm, tm_win, p->win_mask + (size_t)img * p->Nw + z_first, (const double2*)p->twiddle, n_planes, p->z0 + z_first, p->dl, p->wrange + img, image, accumulate,
-            fuse_taper ? p->taper : nullptr, strip_begin, strip_end, slot_first));
+        // the pacing counters of this launch: one per item of a CTA
+        const int grid = n < p->n_sm ? n : p->n_sm;
+        const size_t n_items = (size_t)((n + grid - 1) / grid) * (size_t)n_planes;
+        if (n_items > p->cols_arrivals_cap) { p->err = "k_cols13_wcorrect: pacing counters too small"; return RICK_ERR_STATE; }
+        RICK_CUDA(p, cudaMemsetAsync(p->cols_arrivals, 0, sizeof(uint32_t) * n_items, p->stream));
+        RICK_KERNEL(p, RK_COLS_WCORRECT, k_cols13_wcorrect<<<grid, C12_THREADS, C12_SMEM, p->stream>>>(
+            tm, tm_win, p->win_mask + (size_t)img * p->Nw + z_first, (const double2*)p->twiddle, n_planes, p->z0 + z_first, p->dl,
+            p->wrange + img, image, accumulate, fuse_taper ? p->taper : nullptr, strip_begin, strip_end, slot_first,
+            p->cols_arrivals));
         return RICK_OK;
     }
     RICK_KERNEL(p, RK_COLS_WCORRECT, k_cols12_wcorrect<<<n < p->n_sm ? n : p->n_sm, C12_THREADS, C12_SMEM, p->stream>>>(

@@ -112,7 +112,7 @@ extern "C" int rick_plan_destroy(rick_plan_t* p)
     free_dev(p->twiddle); free_dev(p->twiddle2); free_dev(p->taper); free_dev(p->stack); free_dev(p->image);
     free_dev(p->items); free_dev(p->items_a); free_dev(p->items_b);
     free_dev(p->os_small); free_dev(p->os_gbase); free_dev(p->os_status); free_dev(p->plane_start); free_dev(p->chan_scale);
-    free_dev(p->row_occ); free_dev(p->win_mask); free_dev(p->row_dirty); free_dev(p->tile_occ); free_dev(p->row_list);
+    free_dev(p->row_occ); free_dev(p->win_mask); free_dev(p->cols_arrivals); free_dev(p->row_dirty); free_dev(p->tile_occ); free_dev(p->row_list);
     free_dev(p->wrange); free_dev(p->counters);
     rick_sparse_free(p);
     free_dev(p->st_vis); free_dev(p->st_uvw); free_dev(p->st_wgt); free_dev(p->st_img);
