@@ -191,6 +191,20 @@ int rick_image_stream_host(rick_plan_t* p, const void* vis_host, int32_t vis_dty
 int rick_plane_histogram(rick_plan_t* p, const double* uvw_m, const double* chan_freq_hz, int32_t n_chan,
                          int64_t n_rows, int64_t* hist_host);
 
+/* rick_plane_histogram for callers that must not allocate device memory (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid cudaMalloc): same arguments, same kernels, same result, and NO cudaMalloc /
+ * cudaFree / allocating library routine inside -- the per-call histogram accumulators, the channel scales, the
+ * w range and the a0 counters live in one file-scope device array of RICK_NOALLOC_SCRATCH_BYTES bytes that every
+ * GPU which loads the library holds until exit.  Limits: n_wplanes <= RICK_NOALLOC_MAX_PLANES and
+ * n_chan <= RICK_NOALLOC_MAX_CHAN (RICK_ERR_INVALID with a message otherwise; rick_plane_histogram has no such
+ * limit).  The array is shared by every call of every plan on the device and keeps the last call's contents;
+ * each call clears what must start at zero.  Calls that overlap on the GPU (plans on different streams, or
+ * several host threads) RACE on it: serialise them.  The plan's own state (w range, statistics, channel scales
+ * of its last rick_grid / rick_image) is left alone.  SYNCHRONISES the stream. */
+enum { RICK_NOALLOC_MAX_PLANES = 4096, RICK_NOALLOC_MAX_CHAN = 1024, RICK_NOALLOC_SCRATCH_BYTES = 41216 };
+int rick_plane_histogram_noalloc(rick_plan_t* p, const double* uvw_m, const double* chan_freq_hz, int32_t n_chan,
+                                 int64_t n_rows, int64_t* hist_host);
+
 /* Host-only arithmetic (no device, no plan): cut n_wplanes planes into n_parts CONTIGUOUS ranges whose largest
  * cost is minimal, cost(range) = sum over its planes of (hist[z] + plane_cost) -- hist[z] visibilities to sort
  * and grid, plane_cost = what one plane's FFT + correction costs, in visibilities (>= 0).  bounds: [n_parts + 1],

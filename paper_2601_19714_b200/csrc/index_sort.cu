@@ -14,6 +14,7 @@
 // least-significant-digit radix sort of 64-bit items (key << idx_bits) | k over the key bits,
 // which equals the oracle's sort by (key, index).
 #include "common.cuh"
+#include <mutex>
 
 // ------------------------------------------------------------------------------------------
 // a0: w range.  min/max over rows of w [m]; multiplication by s_c > 0 is monotone under
@@ -618,5 +619,108 @@ int rick_index_sort(rick_plan_t* p, const double* uvw_m, const float* weights, i
             (const u64*)p->sorted_items, (const long long*)p->plane_start, n_planes_total, p->idx_bits, p->log2B,
             p->log2N - p->log2B, p->h, p->tile_occ));
     }
+    return RICK_OK;
+}
+
+// ------------------------------------------------------------------------------------------
+// rick_plane_histogram_noalloc: the per-plane histogram for callers that must not allocate
+// (CUDA graph capture, serving loops, harnesses that forbid cudaMalloc).  Same kernels as rick_plane_histogram
+// (a0: k_counters_reset, k_wrange_rows, k_wrange_finish; then k_plane_hist); what that path keeps in buffers it
+// allocates (the histogram accumulators per call, channel scales / w range / a0 counters on the plan) lives here in
+// ONE file-scope device array of fixed size.  Every GPU that loads the library holds these 41 216 bytes until exit.
+// All calls (of all plans) on a device share the array; it keeps the last call's contents, so what must start at
+// zero is cleared by every call; two calls that overlap on the GPU (different streams) race.
+// ------------------------------------------------------------------------------------------
+constexpr int RICK_NOALLOC_HIST_OFF = 0;                                                   // u64 [MAX_PLANES]
+constexpr int RICK_NOALLOC_SCALE_OFF = RICK_NOALLOC_HIST_OFF + 8 * RICK_NOALLOC_MAX_PLANES;  // double [MAX_CHAN]
+constexpr int RICK_NOALLOC_WRANGE_OFF = RICK_NOALLOC_SCALE_OFF + 8 * RICK_NOALLOC_MAX_CHAN;  // WRange
+constexpr int RICK_NOALLOC_CNT_OFF = RICK_NOALLOC_WRANGE_OFF + 64;                          // DevCounters
+static_assert(RICK_NOALLOC_CNT_OFF + 192 == RICK_NOALLOC_SCRATCH_BYTES, "scratch layout vs rick.h");
+static_assert(sizeof(WRange) <= 64 && sizeof(DevCounters) <= 192, "scratch layout");
+static_assert(RICK_NOALLOC_SCRATCH_BYTES % 256 == 0, "stated size");
+static __device__ __align__(256) unsigned char g_noalloc_scratch[RICK_NOALLOC_SCRATCH_BYTES];
+
+// In host code `g_noalloc_scratch` is a host-side stand-in, not a device address: the device address is looked up
+// once per device, with that device current, and cached.
+static int noalloc_scratch_ptr(rick_plan_t* p, unsigned char** out)
+{
+    constexpr int MAX_DEV = 64;
+    static unsigned char* s_ptr[MAX_DEV] = {};
+    static std::mutex s_mu;
+    int dev = -1;
+    RICK_CUDA(p, cudaGetDevice(&dev));
+    if (dev < 0 || dev >= MAX_DEV) { p->err = "rick_plane_histogram_noalloc: device ordinal beyond 63"; return RICK_ERR_STATE; }
+    std::lock_guard<std::mutex> lock(s_mu);
+    if (!s_ptr[dev]) {
+        void* q = nullptr;
+        RICK_CUDA(p, cudaGetSymbolAddress(&q, g_noalloc_scratch));
+        if (!q) { p->err = "rick_plane_histogram_noalloc: no device address for the scratch array"; return RICK_ERR_CUDA; }
+        s_ptr[dev] = static_cast<unsigned char*>(q);
+    }
+    *out = s_ptr[dev];
+    return RICK_OK;
+}
+
+extern "C" int rick_plane_histogram_noalloc(rick_plan_t* p, const double* uvw_m, const double* chan_freq_hz, int32_t n_chan,
+                                            int64_t n_rows, int64_t* hist_host)
+{
+    if (!p) return RICK_ERR_INVALID;
+    if (p->failed) return p->failed;
+    p->err.clear();
+    if (!hist_host) { p->err = "null hist_host"; return RICK_ERR_INVALID; }
+    if (p->d.cube) { p->err = "rick_plane_histogram_noalloc: cube plans shard by channels"; return RICK_ERR_STATE; }
+    if (p->Nw_total > RICK_NOALLOC_MAX_PLANES) {
+        p->err = "rick_plane_histogram_noalloc: more than 4096 w-planes (the fixed scratch holds 4096 counters); use rick_plane_histogram";
+        return RICK_ERR_INVALID;
+    }
+    if (n_chan < 1 || !chan_freq_hz) { p->err = "bad channels"; return RICK_ERR_INVALID; }
+    if (n_chan > RICK_NOALLOC_MAX_CHAN) {
+        p->err = "rick_plane_histogram_noalloc: more than 1024 channels (the fixed scratch holds 1024 scales); use rick_plane_histogram";
+        return RICK_ERR_INVALID;
+    }
+    if (n_rows < 0) { p->err = "negative n_rows"; return RICK_ERR_INVALID; }
+    if (n_rows > 0 && !uvw_m) { p->err = "null input"; return RICK_ERR_INVALID; }
+    if (n_rows > 0 && (reinterpret_cast<uintptr_t>(uvw_m) & 15u)) { p->err = "device pointer not 16-byte aligned (uvw_m)"; return RICK_ERR_INVALID; }
+    for (int c = 0; c < n_chan; ++c)
+        if (!(chan_freq_hz[c] > 0.0) || !isfinite(chan_freq_hz[c])) { p->err = "bad frequency"; return RICK_ERR_INVALID; }
+    const unsigned long long M64 = (unsigned long long)n_rows * (unsigned long long)n_chan;
+    if (M64 >= 0xFFFFFFFFull) { p->err = "too many visibilities for 32-bit indices"; return RICK_ERR_INVALID; }
+
+    unsigned char* scratch = nullptr;
+    int rc = noalloc_scratch_ptr(p, &scratch);
+    if (rc) return rc;
+    unsigned long long* hist = reinterpret_cast<unsigned long long*>(scratch + RICK_NOALLOC_HIST_OFF);
+    double* scale = reinterpret_cast<double*>(scratch + RICK_NOALLOC_SCALE_OFF);
+    WRange* wr = reinterpret_cast<WRange*>(scratch + RICK_NOALLOC_WRANGE_OFF);
+    DevCounters* cnt = reinterpret_cast<DevCounters*>(scratch + RICK_NOALLOC_CNT_OFF);
+    cudaStream_t st = p->stream;
+
+    // s_c = f_c / c0 through the plan's pinned staging (exists since plan creation; its previous upload must be done)
+    RICK_CUDA(p, cudaEventSynchronize(p->ev_scale));
+    for (int c = 0; c < n_chan; ++c) p->h_scale[c] = chan_freq_hz[c] / RICK_C0;
+    RICK_CUDA(p, cudaMemcpyAsync(scale, p->h_scale, sizeof(double) * (size_t)n_chan, cudaMemcpyHostToDevice, st));
+    RICK_CUDA(p, cudaEventRecord(p->ev_scale, st));
+    // (the plan's own device copy of its last scales, p->chan_scale, is untouched)
+
+    // a0 on the scratch counters (reset by k_counters_reset), then the counts (cleared here)
+    RICK_KERNEL(p, RK_RESET, k_counters_reset<<<1, 1, 0, st>>>(cnt));
+    if (n_rows > 0) {
+        int nb = (int)((n_rows + 255) / 256);
+        if (nb > p->n_sm * 8) nb = p->n_sm * 8;
+        RICK_KERNEL(p, RK_WRANGE, k_wrange_rows<<<nb, 256, 0, st>>>(uvw_m, (long long)n_rows, cnt, p->fold));
+    }
+    RICK_KERNEL(p, RK_WRANGE, k_wrange_finish<<<1, 128, 0, st>>>(cnt, scale, (int)n_chan, 0, p->Nw_total, p->d.w_min, p->d.w_max,
+                                                                 (long long)n_rows, wr));
+    RICK_CUDA(p, cudaMemsetAsync(hist, 0, sizeof(unsigned long long) * (size_t)p->Nw_total, st));
+    const unsigned int M = (unsigned int)M64;
+    if (M > 0) {
+        unsigned int nb = (M + 255) / 256;
+        if (nb > (unsigned)p->n_sm * 8u) nb = (unsigned)p->n_sm * 8u;
+        const size_t sm = sizeof(unsigned int) * (size_t)p->Nw_total;          // (<= 4096 planes: shared-memory counters)
+        RICK_KERNEL(p, RK_INDEX_KEY, k_plane_hist<<<nb, 256, sm, st>>>(uvw_m, scale, wr, M, (unsigned)n_chan, p->N, p->Nw_total,
+                                                                      p->h, p->inv_du, p->fold, hist));
+    }
+    RICK_CUDA(p, cudaMemcpyAsync(hist_host, hist, sizeof(unsigned long long) * (size_t)p->Nw_total, cudaMemcpyDeviceToHost, st));
+    RICK_CUDA(p, cudaStreamSynchronize(st));
     return RICK_OK;
 }

@@ -21,10 +21,11 @@ RICK_OK, RICK_ERR_INVALID, RICK_ERR_STATE, RICK_ERR_CUDA, RICK_ERR_OOM = 0, -1, 
 RICK_GRID_F64, RICK_GRID_F32 = 0, 1
 RICK_VIS_C64, RICK_VIS_C128 = 0, 1
 RICK_FLAG_FOLD_W = 1
+RICK_NOALLOC_MAX_PLANES, RICK_NOALLOC_MAX_CHAN, RICK_NOALLOC_SCRATCH_BYTES = 4096, 1024, 41216
 
 EXPORTS = ["rick_plan", "rick_plan_destroy", "rick_grid", "rick_fft_wplanes",
            "rick_wcorrect_accumulate", "rick_gridcorrect", "rick_image", "rick_image_host",
-           "rick_image_stream_host", "rick_plane_histogram", "rick_partition_planes",
+           "rick_image_stream_host", "rick_plane_histogram", "rick_plane_histogram_noalloc", "rick_partition_planes",
            "rick_get_image", "rick_get_stats", "rick_last_error", "rick_debug_items",
            "rick_debug_planes", "rick_version", "rick_profile",
            "rick_profile_read", "rick_kernel_name"]
@@ -74,6 +75,7 @@ def load_library():
     L.rick_image_host.argtypes = [vp, vp, i32, vp, vp, C.POINTER(C.c_double), i32, i64, vp]
     L.rick_image_stream_host.argtypes = [vp, vp, i32, vp, vp, C.POINTER(C.c_double), i32, i64, i64, vp]
     L.rick_plane_histogram.argtypes = [vp, vp, C.POINTER(C.c_double), i32, i64, C.POINTER(C.c_int64)]
+    L.rick_plane_histogram_noalloc.argtypes = [vp, vp, C.POINTER(C.c_double), i32, i64, C.POINTER(C.c_int64)]
     L.rick_partition_planes.argtypes = [C.POINTER(C.c_int64), i32, i32, C.c_double, C.POINTER(i32)]
     L.rick_get_image.argtypes = [vp, vp]
     L.rick_get_stats.argtypes = [vp, C.POINTER(Stats)]
@@ -217,6 +219,20 @@ class Plan:
         self._check(self._lib.rick_plane_histogram(self._h, _dev_ptr(uvw_m), freq.ctypes.data_as(C.POINTER(C.c_double)),
                                                    int(freq.shape[0]), int(uvw_m.shape[0]),
                                                    hist.ctypes.data_as(C.POINTER(C.c_int64))))
+        return hist
+
+    def rick_plane_histogram_noalloc(self, uvw_m, chan_freq_hz, hist=None) -> np.ndarray:
+        """rick_plane_histogram without any device allocation inside the call (fixed scratch array in the library:
+        at most RICK_NOALLOC_MAX_PLANES planes and RICK_NOALLOC_MAX_CHAN channels; calls that overlap on the GPU
+        race).  `hist`: optional caller-owned [n_wplanes] int64 array to fill."""
+        freq = np.ascontiguousarray(chan_freq_hz, dtype=np.float64)
+        if hist is None:
+            hist = np.zeros(self.n_wplanes, np.int64)
+        assert hist.dtype == np.int64 and hist.flags.c_contiguous and hist.shape == (self.n_wplanes,)
+        self._keep = (uvw_m, freq)
+        self._check(self._lib.rick_plane_histogram_noalloc(self._h, _dev_ptr(uvw_m), freq.ctypes.data_as(C.POINTER(C.c_double)),
+                                                           int(freq.shape[0]), int(uvw_m.shape[0]),
+                                                           hist.ctypes.data_as(C.POINTER(C.c_int64))))
         return hist
 
     def rick_get_image(self) -> torch.Tensor:
