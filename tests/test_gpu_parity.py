@@ -477,6 +477,32 @@ def test_n8192_fp64_occupied_windows_only():
     print(f"N=8192 fp64 window masks: rel L2 {e:.2e} (planes 1..3 empty), {e2:.2e} (second set on the same plan)")
 
 
+def test_n8192_fp64_cube_image_groups_on_the_fused_column_pass():
+    """Cube at N = 8192 fp64: three channel images resident as one group (slots of image j start at j N_w), the fused
+    single column pass with its window masks and pacing counters per image; channel 1 also gets a w range of its
+    own.  Every channel against the oracle, device and host-buffer entry."""
+    rick = _rick()
+    import torch
+    wl = synth.make_config(5, n_times=3, n=8192, n_chan=3, n_wplanes=3, n_src=6)
+    assert wl.cube == 1 and wl.grid_prec == "f64"
+    o = _oracle(wl)
+    plan = rick.plan_from_workload(wl)
+    vis, uvw, wgt = rick.to_device(wl)
+    cube = plan.rick_image(vis, uvw, wgt, wl.freq_hz).cpu().numpy()
+    st = plan.rick_get_stats()
+    hv = torch.from_numpy(np.ascontiguousarray(wl.vis)).pin_memory()
+    hu = torch.from_numpy(wl.uvw_m).pin_memory()
+    hout = torch.full((3, wl.n, wl.n), float("nan"), dtype=torch.float64).pin_memory()
+    plan.rick_image_host(hv, hu, None, wl.freq_hz, hout)
+    plan.destroy()
+    for c in range(3):
+        e = _close(cube[c], o["image"][c], TOL64, f"channel {c}")
+        _close(hout[c].numpy(), o["image"][c], TOL64, f"channel {c}, host entry")
+        print(f"N=8192 fp64 cube channel {c}: rel L2 {e:.2e}")
+    ix = oracle.index(wl.uvw_m, wl.freq_hz, wl.n, wl.n_wplanes, wl.support, wl.pixel_rad, 16, cube=1)
+    assert st["n_gridded"] == int((ix["key"] != np.uint64(0xFFFFFFFFFFFFFFFF)).sum())
+
+
 def test_fp32_grid_n4096_bulk_row_store():
     """fp32 grid at N = 4096: one row per CTA, the row leaves by a bulk store from the exchange buffer (the fp64
     twin of this path is what configs[1] runs); generic column pass + correction."""
