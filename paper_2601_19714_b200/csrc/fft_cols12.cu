@@ -326,9 +326,10 @@ constexpr uint32_t C13_WIN_BYTES = C13_STAGE_BYTES / 32;            // a window 
 // nothing couples the CTAs any more, they drift apart by whole planes and DRAM delivered 2.5 x the bytes.  So the CTAs
 // pace each other: arrivals[i] counts the CTAs that have issued their item number i (one RED per CTA and item), and a
 // CTA issues its item i only once every CTA that has an item i - C13_PACE_SLACK has issued it.  One word is polled, and
-// it is fetched at the top of the item, long before the copy it gates.  The wait is bounded: if the others do not show
-// up (CTAs of the grid not resident) the warp stops pacing for good -- the result does not depend on it.
+// it is fetched at the top of the item, long before the copy it gates.  The wait is bounded (0.3 ms): if the others do
+// not show up (CTAs of the grid not resident) the warp stops pacing for good -- the result does not depend on it.
 constexpr int C13_PACE_SLACK = 2;
+constexpr unsigned long long C13_PACE_TIMEOUT_NS = 300000ull;
 struct Pace {
     uint32_t* arrivals;               // [items per CTA], zeroed before the launch; null = no pacing
     int n_planes, n_cols;             // of the launch: item i belongs to column round i / n_planes
@@ -343,7 +344,15 @@ __device__ __forceinline__ void pace_wait(Pace& pc, int item, uint32_t seen)
     if (!pc.on || item < C13_PACE_SLACK) return;
     const int round = (item - C13_PACE_SLACK) / pc.n_planes, full = pc.n_cols / (int)gridDim.x;
     const uint32_t need = round < full ? gridDim.x : (round == full ? (uint32_t)(pc.n_cols % (int)gridDim.x) : 0u);
-    for (int spin = 0; spin < (1 << 16) && seen < need; ++spin) seen = pace_load(pc, item);
+    if (seen >= need) return;
+    // (rare path) bounded in TIME: ~40 item periods.  CTAs of the grid that are not resident yet -- another kernel holds
+    // their SMs -- must not stall the ones that are.
+    unsigned long long t0, t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t0));
+    do {
+        seen = pace_load(pc, item);
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    } while (seen < need && t - t0 < C13_PACE_TIMEOUT_NS);
     if (seen < need) pc.on = false;
 }
 

@@ -477,6 +477,35 @@ def test_n8192_fp64_occupied_windows_only():
     print(f"N=8192 fp64 window masks: rel L2 {e:.2e} (planes 1..3 empty), {e2:.2e} (second set on the same plan)")
 
 
+def test_n8192_fp64_two_plans_on_two_streams_at_once():
+    """Two plans imaging at the same time on two streams: the CTAs of the second fused column pass find no free SM
+    until those of the first retire, so its pacing (CTAs wait for each other's arrival counters) meets CTAs that are
+    not resident -- the bounded wait must let it through, and both images must be right."""
+    rick = _rick()
+    import torch, time
+    wl = synth.make_config(3, n_times=4, n_wplanes=3, n_src=6)
+    assert wl.n == 8192 and wl.grid_prec == "f64"
+    o = _oracle(wl)
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    vis, uvw, wgt = rick.to_device(wl)
+    torch.cuda.synchronize()
+    p1, p2 = rick.plan_from_workload(wl, stream=s1), rick.plan_from_workload(wl, stream=s2)
+    out1 = torch.empty((wl.n, wl.n), dtype=torch.float64, device="cuda")
+    out2 = torch.empty_like(out1)
+    t0 = time.perf_counter()
+    for _ in range(3):
+        p1.rick_image(vis, uvw, wgt, wl.freq_hz, out1)
+        p2.rick_image(vis, uvw, wgt, wl.freq_hz, out2)
+    torch.cuda.synchronize()
+    dt = time.perf_counter() - t0
+    e1 = _close(out1.cpu().numpy(), o["image"], TOL64, "plan on stream 1")
+    e2 = _close(out2.cpu().numpy(), o["image"], TOL64, "plan on stream 2")
+    p1.destroy()
+    p2.destroy()
+    print(f"two N=8192 plans on two streams, 3 rounds: {dt * 1e3:.1f} ms, rel L2 {e1:.2e} / {e2:.2e}")
+    assert dt < 5.0          # (a stalled pacing wait would show as seconds)
+
+
 def test_n8192_fp64_cube_image_groups_on_the_fused_column_pass():
     """Cube at N = 8192 fp64: three channel images resident as one group (slots of image j start at j N_w), the fused
     single column pass with its window masks and pacing counters per image; channel 1 also gets a w range of its
