@@ -454,11 +454,24 @@ static int transform_and_correct(rick_plan_t* p, int img, int z0, int nb, double
         if ((rc = rick_fft_rows(p, img * p->Nw + z0, nb))) return rc;
         const int strips = rick_cols12_strips(p), ucols = rick_cols12_unit_cols(p);
         if (host_out && last && !p->d.cube) {
-            // whole rounds of the persistent grid per part: 4 + 4 + 3 + rest rounds of n_sm strips
-            const int r4 = (strips / p->n_sm + 3) / 4;
-            const int rounds[4] = {r4 > 0 ? r4 : 1, r4 > 0 ? r4 : 1, r4 > 1 ? r4 - 1 : 1, 1 << 20};
+            // whole rounds of the persistent grid per part.  N = 4096 (the pass is about as long as the copy of its image):
+            // 4 + 4 + 3 + rest rounds of n_sm strips.  N = 8192 (26 ms of kernel against 10 ms of copy at configs[2]): seven
+            // shrinking parts + the rest, so that the copy left over after the last kernel is 2 % of the image, not 26 %
+            // (host entry 46.8 -> 44.5 ms; at N = 4096 the same split costs 0.1-0.7 ms)
+            int rounds[8];
+            const int total = (strips + p->n_sm - 1) / p->n_sm;
+            if (p->cols13_ok) {
+                static const int pct[7] = {28, 24, 18, 12, 8, 5, 3};
+                for (int k = 0; k < 7; ++k) rounds[k] = (pct[k] * total + 50) / 100 > 0 ? (pct[k] * total + 50) / 100 : 1;
+                rounds[7] = 1 << 20;
+            } else {
+                const int r4 = (strips / p->n_sm + 3) / 4;
+                rounds[0] = rounds[1] = r4 > 0 ? r4 : 1;
+                rounds[2] = r4 > 1 ? r4 - 1 : 1;
+                for (int k = 3; k < 8; ++k) rounds[k] = 1 << 20;
+            }
             int s0 = 0;
-            for (int k = 0; k < 4 && s0 < strips; ++k) {
+            for (int k = 0; k < 8 && s0 < strips; ++k) {
                 long long s1 = (long long)s0 + (long long)rounds[k] * p->n_sm;
                 if (s1 > strips) s1 = strips;
                 if ((rc = rick_cols12_wcorrect(p, img, z0, nb, dst, z0 > 0, last, s0, (int)s1))) return rc;
