@@ -203,8 +203,8 @@ int rick_cols2_wcorrect(rick_plan_t* p, int img, int z_first, int n_planes, doub
 int rick_sparse_init(rick_plan_t* p);
 void rick_sparse_free(rick_plan_t* p);
 int rick_sparse_prepare(rick_plan_t* p);
-int rick_sparse_wcorrect(rick_plan_t* p, int z_first, int n_planes, int accumulate);
-int rick_sparse_finish(rick_plan_t* p, double* image, int fuse_taper);
+int rick_sparse_wcorrect(rick_plan_t* p, int z_first, int n_planes, int accumulate, int col_begin = 0, int col_end = -1);
+int rick_sparse_finish(rick_plan_t* p, double* image, int fuse_taper, int col_begin = 0, int col_end = -1);
 const int* rick_sparse_maxcount(const rick_plan_t* p);
 int rick_sparse_cap(const rick_plan_t* p);
 int rick_cols12_init(rick_plan_t* p);                                    // fft_cols12.cu

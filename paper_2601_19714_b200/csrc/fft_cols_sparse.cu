@@ -126,7 +126,8 @@ __global__ void __launch_bounds__(SparseCfg<LOG2N>::NT, 1)
 k_cols_sparse_wcorrect(const float2* __restrict__ stack, const float2* __restrict__ tw, const int* __restrict__ max_count,
                        const unsigned int* __restrict__ bits, const unsigned int* __restrict__ prefix,
                        const unsigned short* __restrict__ list, const int* __restrict__ count, int plane_first, int n_planes,
-                       int z_first, double dl, const WRange* __restrict__ wr, double* __restrict__ imageT, int accumulate)
+                       int z_first, double dl, const WRange* __restrict__ wr, double* __restrict__ imageT, int accumulate,
+                       int col_begin, int col_end)
 {
     typedef SparseCfg<LOG2N> K;
     if (*max_count > K::CAP) return;            // some plane is too dense for the staging: the two-pass kernels run instead
@@ -159,11 +160,11 @@ k_cols_sparse_wcorrect(const float2* __restrict__ stack, const float2* __restric
         }
     };
 
-    int col = blockIdx.x;
-    if (col < K::N) issue(col, n_planes - 1);
+    int col = col_begin + (int)blockIdx.x;       // columns [col_begin, col_end) of the image
+    if (col < col_end) issue(col, n_planes - 1);
     const double dw = wr->dw;
     const double w_first = wr->w_min + ((double)z_first + 0.5) * dw;
-    for (; col < K::N; col += gridDim.x) {
+    for (; col < col_end; col += gridDim.x) {
         const double l = (double)(col - K::N / 2) * dl;
         // pixel rows of this thread: q_e = t + NT ((e + 8) & 15), for the input rows and the outputs alike
 #pragma unroll
@@ -193,7 +194,7 @@ k_cols_sparse_wcorrect(const float2* __restrict__ stack, const float2* __restric
             }
             __syncthreads();                       // staging and maps consumed: the next item may land
             if (plane > 0) issue(col, plane - 1);
-            else if (col + (int)gridDim.x < K::N) issue(col + (int)gridDim.x, n_planes - 1);
+            else if (col + (int)gridDim.x < col_end) issue(col + (int)gridDim.x, n_planes - 1);
             fft_thread<float, LOG2N>(v, t, sm, 1, 0, tw);
             // Horner in z: S <- P_z + step S
             if (plane == n_planes - 1) {
@@ -252,11 +253,11 @@ k_cols_sparse_wcorrect(const float2* __restrict__ stack, const float2* __restric
 // image[q][p] = imageT[p][q] (/ (taper[p] taper[q])): 32 x 32 tiles through shared memory
 __global__ void __launch_bounds__(256) k_image_transpose_taper(const double* __restrict__ imageT, double* __restrict__ image, int N,
                                                                const double* __restrict__ taper, const int* __restrict__ max_count,
-                                                               int cap)
+                                                               int cap, int p_begin)
 {
     if (*max_count > cap) return;
     __shared__ double tile[32][33];
-    const int p0 = blockIdx.x * 32, q0 = blockIdx.y * 32;
+    const int p0 = p_begin + blockIdx.x * 32, q0 = blockIdx.y * 32;      // image columns p_begin + 32 blockIdx.x ..
     const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
     for (int j = ty; j < 32; j += 8) tile[j][tx] = imageT[(size_t)(p0 + j) * N + q0 + tx];      // [p][q]
     __syncthreads();
@@ -317,28 +318,32 @@ int rick_sparse_prepare(rick_plan_t* p)
 }
 
 // planes z_first .. z_first + n_planes - 1 of the image, resident in slots 0 .. n_planes - 1
-int rick_sparse_wcorrect(rick_plan_t* p, int z_first, int n_planes, int accumulate)
+int rick_sparse_wcorrect(rick_plan_t* p, int z_first, int n_planes, int accumulate, int col_begin, int col_end)
 {
-    if (n_planes <= 0) return RICK_OK;
+    if (col_end < 0) col_end = p->N;
+    if (n_planes <= 0 || col_end <= col_begin) return RICK_OK;
     const int* maxc = p->sp_count + p->Nw;
     if (p->log2N == 13) {
         RICK_KERNEL(p, RK_COLS_WCORRECT, k_cols_sparse_wcorrect<13><<<p->n_sm, SparseCfg<13>::NT, SparseCfg<13>::SMEM, p->stream>>>(
             (const float2*)p->stack, (const float2*)p->twiddle, maxc, p->sp_bits, p->sp_prefix, p->sp_list, p->sp_count, z_first,
-            n_planes, p->z0 + z_first, p->dl, p->wrange, p->sp_imageT, accumulate));
+            n_planes, p->z0 + z_first, p->dl, p->wrange, p->sp_imageT, accumulate, col_begin, col_end));
     } else {
         RICK_KERNEL(p, RK_COLS_WCORRECT, k_cols_sparse_wcorrect<14><<<p->n_sm, SparseCfg<14>::NT, SparseCfg<14>::SMEM, p->stream>>>(
             (const float2*)p->stack, (const float2*)p->twiddle, maxc, p->sp_bits, p->sp_prefix, p->sp_list, p->sp_count, z_first,
-            n_planes, p->z0 + z_first, p->dl, p->wrange, p->sp_imageT, accumulate));
+            n_planes, p->z0 + z_first, p->dl, p->wrange, p->sp_imageT, accumulate, col_begin, col_end));
     }
     return RICK_OK;
 }
 
 // after the last batch: the transposed image becomes the image (divided by the taper when fuse_taper)
-int rick_sparse_finish(rick_plan_t* p, double* image, int fuse_taper)
+// (image columns [col_begin, col_end), multiples of 32; col_end < 0: to the last column)
+int rick_sparse_finish(rick_plan_t* p, double* image, int fuse_taper, int col_begin, int col_end)
 {
-    dim3 grid((unsigned)(p->N / 32), (unsigned)(p->N / 32));
+    if (col_end < 0) col_end = p->N;
+    if (col_end <= col_begin) return RICK_OK;
+    dim3 grid((unsigned)((col_end - col_begin) / 32), (unsigned)(p->N / 32));
     RICK_KERNEL(p, RK_TAPER, k_image_transpose_taper<<<grid, 256, 0, p->stream>>>(p->sp_imageT, image, p->N,
                                                                                  fuse_taper ? p->taper : nullptr,
-                                                                                 p->sp_count + p->Nw, p->N / 2));
+                                                                                 p->sp_count + p->Nw, p->N / 2, col_begin));
     return RICK_OK;
 }

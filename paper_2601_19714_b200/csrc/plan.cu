@@ -490,13 +490,33 @@ static int transform_and_correct(rick_plan_t* p, int img, int z0, int nb, double
         const int two_pass = rick_cols2_on(p);
         if (two_pass) {       // long columns: pass A at full line width, pass B fused with the correction
             if ((rc = rick_fft_rows(p, img * p->Nw + z0, nb))) return rc;
-            if (p->sp_ok) {
-                // fp32 grid: one fused pass over the occupied rows only, when every plane of the image has few
-                // enough of them (decided on the device: either these launches or the two-pass ones below return
-                // at once).  It accumulates a transposed image, turned (and tapered) after the last batch.
-                if (z0 == 0 && (rc = rick_sparse_prepare(p))) return rc;
-                if ((rc = rick_sparse_wcorrect(p, z0, nb, z0 > 0))) return rc;
+            // fp32 grid: one fused pass over the occupied rows only, when every plane of the image has few
+            // enough of them (decided on the device: either these launches or the two-pass ones return at
+            // once).  It accumulates a transposed image, turned (and tapered) after the last batch.
+            if (p->sp_ok && z0 == 0 && (rc = rick_sparse_prepare(p))) return rc;
+            if (p->sp_ok && host_out && last && !p->d.cube) {
+                // last batch through the host entry: the two-pass kernels first (the whole image, or nothing), then the
+                // sparse pass, its transposition and the copy to the host by column ranges -- a short first range so
+                // that the copy engine starts early (the 2.1 GB image of configs[3] takes longer to cross PCIe than
+                // the last batch takes to compute), each range's copy under the next range's kernels
+                if ((rc = rick_fft_cols2(p, img * p->Nw + z0, nb))) return rc;
+                if ((rc = rick_cols2_wcorrect(p, img, z0, nb, dst, z0 > 0, last))) return rc;
+                const int first = p->N / 16, step = (p->N - first + 2) / 3 / 32 * 32 + 32;
+                for (int c0 = 0; c0 < p->N;) {
+                    int c1 = c0 + (c0 == 0 ? first : step);
+                    if (c1 > p->N) c1 = p->N;
+                    if ((rc = rick_sparse_wcorrect(p, z0, nb, z0 > 0, c0, c1))) return rc;
+                    if ((rc = rick_sparse_finish(p, dst, 1, c0, c1))) return rc;
+                    RICK_CUDA(p, cudaEventRecord(p->ev_part, p->stream));
+                    RICK_CUDA(p, cudaStreamWaitEvent(p->stream3, p->ev_part, 0));
+                    RICK_CUDA(p, cudaMemcpy2DAsync(host_out + c0, sizeof(double) * p->N, dst + c0, sizeof(double) * p->N,
+                                                   sizeof(double) * (size_t)(c1 - c0), (size_t)p->N, cudaMemcpyDeviceToHost, p->stream3));
+                    c0 = c1;
+                }
+                *host_done = true;
+                return RICK_OK;
             }
+            if (p->sp_ok && (rc = rick_sparse_wcorrect(p, z0, nb, z0 > 0))) return rc;
             if ((rc = rick_fft_cols2(p, img * p->Nw + z0, nb))) return rc;
             if (p->sp_ok) {
                 if ((rc = rick_cols2_wcorrect(p, img, z0, nb, dst, z0 > 0, last))) return rc;

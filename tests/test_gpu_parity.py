@@ -570,7 +570,14 @@ def test_fp32_long_columns_sparse_and_dense_paths():
         img2 = plan.rick_image(vis, uvw, wgt, wl.freq_hz).cpu().numpy()
         prof = plan.rick_profile_read()
         plan.rick_profile(False)
+        # host-buffer entry: the last batch's sparse pass, its transposition and the copy out run by column ranges
+        import torch
+        hv = torch.from_numpy(np.ascontiguousarray(wl.vis)).pin_memory()
+        hu = torch.from_numpy(wl.uvw_m).pin_memory()
+        hout = torch.full((wl.n, wl.n), float("nan"), dtype=torch.float64).pin_memory()
+        plan.rick_image_host(hv, hu, None, wl.freq_hz, hout)
         plan.destroy()
+        _close(hout.numpy(), o["image"], TOL32, name + " (host entry)")
         idx = oracle.index(wl.uvw_m, wl.freq_hz, wl.n, wl.n_wplanes, wl.support, wl.pixel_rad, 16)
         keep = idx["key"] != np.uint64(0xFFFFFFFFFFFFFFFF)
         # occupied rows per plane as the plan counts them: tile rows (16) of the centre cells plus the halo
