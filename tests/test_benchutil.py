@@ -64,3 +64,32 @@ def test_replica_aggregation_world2_gloo():
         assert p.exitcode == 0
     for rank, units, ms, per_s, mx in res:
         assert units == 2000.0 and ms == 15.0 and abs(per_s - 2000.0 / 0.015) < 1e-6 and mx == 1.0
+
+
+def test_byte_model_counts_what_the_pruned_method_moves():
+    """bench.py's byte model on hand-made counts: the row pass is charged the occupied tiles it reads and the
+    occupied rows it writes; the fused column pass the stack once -- at N = 8192 fp64 only the occupied 256-row
+    windows --, plus the image (and its read-modify-write for every plane batch but the first)."""
+    import types
+    import numpy as np
+    import bench
+    def wl(n, nw, prec, batch=0):
+        return types.SimpleNamespace(n=n, support=7, n_wplanes=nw, n_chan=4, n_rows=1000, n_vis=4000, cube=0,
+                                     grid_prec=prec, plane_batch=batch, weights=None, vis=np.zeros(1, np.complex64))
+    # N = 8192 fp64, 2 planes: 10 occupied windows of 64, 3000 occupied rows, 500 occupied tiles
+    st = dict(n_planes=2, occ_rows=3000, occ_tiles=500, occ_windows=10, n_gridded=3900)
+    prof = {"fft_cols_wcorrect": (1.0, 1), "fft_rows": (1.0, 1), "radix_scatter": (1.0, 4)}
+    m, sizes = bench.byte_model(wl(8192, 2, "f64"), st, prof, 1)
+    E, N = 16, 8192
+    assert m["fft_rows"]["bytes"] == 500 * 16 * 16 * E + 3000 * N * E
+    assert m["fft_cols_wcorrect"]["bytes"] == 10 * 256 * N * E + N * N * 8
+    assert m["fft_cols_wcorrect"]["dense_bytes"] == N * N * 2 * E + N * N * 8 == sizes["stack"] + sizes["image"]
+    assert m["radix_scatter"]["bytes"] == 16 * 4000 * 4
+    # N = 4096 fp64: the whole stack, whatever the windows say
+    st4 = dict(st, occ_windows=1)
+    m4, _ = bench.byte_model(wl(4096, 2, "f64"), st4, prof, 1)
+    assert m4["fft_cols_wcorrect"]["bytes"] == 4096 * 4096 * 2 * 16 + 4096 * 4096 * 8
+    # fp32 sparse fused pass in 2 plane batches: occupied rows gathered, transposed image written, then read + written
+    st32 = dict(n_planes=4, occ_rows=5000, occ_tiles=700, occ_windows=0, n_gridded=3900)
+    m32, _ = bench.byte_model(wl(16384, 4, "f32", batch=2), st32, prof, 1)
+    assert m32["fft_cols_wcorrect"]["bytes"] == 5000 * 16384 * 8 + 16384 * 16384 * 8 * 3 and m32["fft_cols_wcorrect"]["alu"]
